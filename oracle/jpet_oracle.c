@@ -1,0 +1,294 @@
+/*
+ * jpet_oracle.c - plain fp64 CPU oracle for the list-mode MLEM iteration of arXiv:1502.07478
+ * ("GPU accelerated image reconstruction in a two-strip J-PET tomograph").
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, load or call it.  It shares no code, header, table or
+ * helper with paper_1502_07478_b200/csrc (the CUDA path) and neither includes the other.
+ *
+ * It is written to be checked against the paper by eye: every function cites the passage it follows and
+ * uses the paper's notation (tilde quantities carry the suffix _t).  No blocking, fusion, factoring of
+ * common sub-expressions across pixels, or reordering beyond what the paper states.  The only
+ * parallelism is the paper's own CPU scheme: OpenMP over events, one private rho_new per thread, summed
+ * after the loop.
+ *
+ * Readings of the paper where it is garbled or silent are the R-numbers of SURVEY.md section 8(c),
+ * listed again in DESIGN.md ("Readings").  Pins for every function: tests/test_oracle_*.py.
+ * Parity status: all functions pinned (none "parity unpinned"); what stays unpinned is only whether
+ * Eq. 7 models the real detector, which no synthetic test can decide.
+ *
+ * Geometry: image plane (y, z); strips are the segments y = +R ("u") and y = -R ("d"), |z| <= L/2
+ * (PAPER.md:34-40, :52, :77).  Lengths in mm.  Pixel (iy, iz) has its centre at
+ *   y = (iy - (n_y-1)/2) * pixel,  z = (iz - (n_z-1)/2) * pixel     (row-major, z fastest).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define JO_PI 3.14159265358979323846264338327950288
+
+/* ---- pixel centres (SURVEY.md 8(b) grid convention; "center of pixel i") ---------------- */
+static double jo_pixel_y(int iy, int n_y, double pixel) { return ((double)iy - 0.5 * (double)(n_y - 1)) * pixel; }
+static double jo_pixel_z(int iz, int n_z, double pixel) { return ((double)iz - 0.5 * (double)(n_z - 1)) * pixel; }
+
+/* ---- Eq. 1: path difference of an emission at (e_y, e_z) whose photons hit z_u, z_d ----- */
+double jo_eq1_delta_l(double e_y, double e_z, double z_u, double z_d, double R)
+{
+    return sqrt((R - e_y) * (R - e_y) + (z_u - e_z) * (z_u - e_z))
+         - sqrt((R + e_y) * (R + e_y) + (z_d - e_z) * (z_d - e_z));
+}
+
+/* ---- Eq. 2, first forms; R-bar == R (R1), the "y" in the z~ line is y~ (R3) ---------
+ * out = { tan(theta~), y~, z~ }                                                                         */
+void jo_eq2(double z_u_t, double z_d_t, double dl_t, double R, double out[3])
+{
+    double tan_t = (z_u_t - z_d_t) / (2.0 * R);
+    double y_t = -0.5 * dl_t / sqrt(1.0 + tan_t * tan_t);
+    double z_t = 0.5 * (z_u_t + z_d_t + 2.0 * y_t * tan_t);
+    out[0] = tan_t;
+    out[1] = y_t;
+    out[2] = z_t;
+}
+
+/* ---- Eq. 4: sensitivity of the point (y, z); negative values (points no LOR through
+ * both strips can see) are clamped to 0 (R13).                                                          */
+double jo_sensitivity(double y, double z, double R, double L)
+{
+    double hi1 = (0.5 * L - z) / (R - y);
+    double hi2 = (0.5 * L + z) / (R + y);
+    double lo1 = -(0.5 * L + z) / (R - y);
+    double lo2 = (-0.5 * L + z) / (R + y);
+    double s = (atan(fmin(hi1, hi2)) - atan(fmax(lo1, lo2))) / JO_PI;
+    return s > 0.0 ? s : 0.0;
+}
+
+void jo_sensitivity_image(double R, double L, int n_y, int n_z, double pixel, double *s)
+{
+    for (int iy = 0; iy < n_y; ++iy)
+        for (int iz = 0; iz < n_z; ++iz)
+            s[(size_t)iy * n_z + iz] = jo_sensitivity(jo_pixel_y(iy, n_y, pixel), jo_pixel_z(iz, n_z, pixel), R, L);
+}
+
+/* ---- b C^-1 b (first line of B.3), diagonal C (R6) -------------------------------------- */
+double jo_bCb(double dy, double dz, double tan_t, double sigma_z, double sigma_dl)
+{
+    double cos2 = 1.0 / (1.0 + tan_t * tan_t);
+    double u = dz - dy * tan_t;
+    return 2.0 * u * u / (sigma_z * sigma_z) + 4.0 * dy * dy / (sigma_dl * sigma_dl * cos2);
+}
+
+/* ---- Eq. 7-12: reconstruction kernel P(e~ | pixel at (y, z)) ----------------------
+ * Vectors o, a, b are Eq. 8, 9, 10 written out; C^-1 = diag(1/sz^2, 1/sz^2, 1/sdl^2) (Eq. 12, gamma=0,
+ * PAPER.md:124).  a3_coef multiplies the third component of a: 2 gives a = d e/d theta (default, R5),
+ * 1 gives Eq. 9 exactly as printed.  Prefactor: det^(1/2) of the INVERSE covariance over 2 pi^2 (R4).
+ * No truncation here: the 3-sigma rule is applied by the caller.                                        */
+double jo_kernel(double y, double z, double tan_t, double y_t, double z_t,
+                 double R, double sigma_z, double sigma_dl, double a3_coef)
+{
+    double dy = y - y_t;                       /* Eq. 11 */
+    double dz = z - z_t;
+    double icos = sqrt(1.0 + tan_t * tan_t);   /* cos^-1(theta~) */
+    double icos2 = icos * icos;                /* cos^-2(theta~) */
+    double Cinv[3] = { 1.0 / (sigma_z * sigma_z), 1.0 / (sigma_z * sigma_z), 1.0 / (sigma_dl * sigma_dl) };
+
+    double o[3], a[3], b[3];
+    o[0] = -(dy + y_t - R) * tan_t * icos2;                       /* Eq. 8 */
+    o[1] = -(dy + y_t + R) * tan_t * icos2;
+    o[2] = -(dy + y_t) * icos * (1.0 + 2.0 * tan_t * tan_t);
+    a[0] = -(dy + y_t - R) * icos2;                               /* Eq. 9 */
+    a[1] = -(dy + y_t + R) * icos2;
+    a[2] = -a3_coef * (dy + y_t) * icos * tan_t;
+    b[0] = dz - dy * tan_t;                                       /* Eq. 10 */
+    b[1] = dz - dy * tan_t;
+    b[2] = -2.0 * dy * icos;
+
+    double aCa = 0.0, oCb = 0.0, bCb = 0.0, bCa = 0.0;
+    for (int k = 0; k < 3; ++k) {
+        aCa += a[k] * Cinv[k] * a[k];
+        oCb += o[k] * Cinv[k] * b[k];
+        bCb += b[k] * Cinv[k] * b[k];
+        bCa += b[k] * Cinv[k] * a[k];
+    }
+    double D = aCa + 2.0 * oCb;
+    if (!(D > 0.0)) return 0.0;                                   /* R17 */
+    double sqrt_det_Cinv = sqrt(Cinv[0] * Cinv[1] * Cinv[2]);
+    return sqrt_det_Cinv / (2.0 * JO_PI * JO_PI * sqrt(D)) * exp(-0.5 * (bCb - bCa * bCa / D));   /* Eq. 7 */
+}
+
+/* ---- convenience for quadrature tests: P(e~_j | pixel (y, z)) for many events (double [n][3]) ---------
+ * Eq. 2 then Eq. 7 per event; inside3s[j] = 1 when the pixel centre is inside event j's 3-sigma ellipse. */
+void jo_kernel_events(const double *events, int64_t n, double y, double z, double R, double sigma_z,
+                      double sigma_dl, double a3_coef, double *P_out, unsigned char *inside3s)
+{
+    for (int64_t j = 0; j < n; ++j) {
+        double e[3];
+        jo_eq2(events[3 * j + 0], events[3 * j + 1], events[3 * j + 2], R, e);
+        P_out[j] = jo_kernel(y, z, e[0], e[1], e[2], R, sigma_z, sigma_dl, a3_coef);
+        if (inside3s) inside3s[j] = jo_bCb(y - e[1], z - e[2], e[0], sigma_z, sigma_dl) <= 9.0;
+    }
+}
+
+/* ---- Appendix B: circumscribed half-extents of the 3-sigma ellipse ----------------
+ * Ellipse A dy^2 + 2 C dy dz + B dz^2 = 3^2 with A, B, C read off B.3 (R8, R9).  out = { h_y, h_z }.   */
+void jo_bbox_half_extents(double tan_t, double sigma_z, double sigma_dl, double out[2])
+{
+    double icos2 = 1.0 + tan_t * tan_t;
+    double A = 2.0 * tan_t * tan_t / (sigma_z * sigma_z) + 4.0 * icos2 / (sigma_dl * sigma_dl);
+    double B = 2.0 / (sigma_z * sigma_z);
+    double C = -2.0 * tan_t / (sigma_z * sigma_z);
+    out[0] = 3.0 / sqrt(A - C * C / B);                            /* B.2 */
+    out[1] = 3.0 / sqrt(B - C * C / A);
+}
+
+/* ---- Listing 1 with Eq. 3's s(i) in the denominator (R11, R12) --------------------
+ * One MLEM iteration.
+ *   events   : float32 [n][3] = (z_u~, z_d~, dl~), the very array the GPU gets, widened to double here
+ *   rho_in   : double [n_y*n_z];  rho_out: double [n_y*n_z]
+ *   brute    : 0 = loop over the clipped bounding box (Listing 1), 1 = scan the whole image; both apply
+ *              the same centre-in-ellipse test  b C^-1 b <= 9  (R8, R10) and must agree
+ *   counters : n_evals = sum over events of |ellipse(e_j)|, n_skipped = events with an empty pixel set
+ *              or a non-positive / non-finite denominator (R16)
+ * Steps (SURVEY.md 8(c) algorithm):  w = s*rho;  per event: Eq. 2, pixel set, P, denominator = sum P*w,
+ * rho_new[i] += P_i / denominator;  finally rho_out = rho_in * rho_new where s > 0, else 0.
+ * Returns 0, or -1 on allocation failure / bad arguments.                                               */
+int jo_mlem_iterate(const float *events, int64_t n, double R, double L, double sigma_z, double sigma_dl,
+                    int n_y, int n_z, double pixel, double a3_coef, const double *rho_in, double *rho_out,
+                    int brute, int n_threads, uint64_t *n_evals_out, uint64_t *n_skipped_out)
+{
+    if (n < 0 || n_y <= 0 || n_z <= 0 || !(pixel > 0.0) || !rho_in || !rho_out || (n > 0 && !events)) return -1;
+    const size_t M = (size_t)n_y * (size_t)n_z;
+    double *s = (double *)malloc(M * sizeof(double));
+    double *w = (double *)malloc(M * sizeof(double));
+    if (!s || !w) { free(s); free(w); return -1; }
+    jo_sensitivity_image(R, L, n_y, n_z, pixel, s);
+    for (size_t i = 0; i < M; ++i) w[i] = s[i] * rho_in[i];
+
+#ifdef _OPENMP
+    if (n_threads <= 0) n_threads = omp_get_max_threads();
+#else
+    n_threads = 1;
+#endif
+    double *rho_new_all = (double *)calloc(M * (size_t)n_threads, sizeof(double));   /* Listing 1 lines 1-3 */
+    if (!rho_new_all) { free(s); free(w); return -1; }
+    uint64_t n_evals = 0, n_skipped = 0;
+    int failed = 0;
+
+#ifdef _OPENMP
+#pragma omp parallel num_threads(n_threads) reduction(+ : n_evals, n_skipped) reduction(| : failed)
+#endif
+    {
+#ifdef _OPENMP
+        int tid = omp_get_thread_num();
+#else
+        int tid = 0;
+#endif
+        double *rho_new = rho_new_all + (size_t)tid * M;           /* private copy */
+        size_t cap = 1024;
+        double *kernel = (double *)malloc(cap * sizeof(double));    /* Listing 1: kernel[i] cache */
+        int *pix = (int *)malloc(cap * sizeof(int));
+        if (!kernel || !pix) failed = 1;
+
+#ifdef _OPENMP
+#pragma omp for schedule(static)
+#endif
+        for (int64_t j = 0; j < n; ++j) {                           /* Listing 1 line 4 */
+            if (failed) continue;
+            double e[3];
+            jo_eq2((double)events[3 * j + 0], (double)events[3 * j + 1], (double)events[3 * j + 2], R, e);
+            double tan_t = e[0], y_t = e[1], z_t = e[2];
+            if (!isfinite(tan_t) || !isfinite(y_t) || !isfinite(z_t)) { n_skipped++; continue; }
+
+            int iy0 = 0, iy1 = n_y - 1, iz0 = 0, iz1 = n_z - 1;
+            if (!brute) {                                           /* bounding box in pixel space */
+                double h[2];
+                jo_bbox_half_extents(tan_t, sigma_z, sigma_dl, h);
+                double fy0 = ceil((y_t - h[0]) / pixel + 0.5 * (double)(n_y - 1));
+                double fy1 = floor((y_t + h[0]) / pixel + 0.5 * (double)(n_y - 1));
+                double fz0 = ceil((z_t - h[1]) / pixel + 0.5 * (double)(n_z - 1));
+                double fz1 = floor((z_t + h[1]) / pixel + 0.5 * (double)(n_z - 1));
+                if (fy0 > (double)iy0) iy0 = fy0 > (double)n_y ? n_y : (int)fy0;
+                if (fy1 < (double)iy1) iy1 = fy1 < -1.0 ? -1 : (int)fy1;
+                if (fz0 > (double)iz0) iz0 = fz0 > (double)n_z ? n_z : (int)fz0;
+                if (fz1 < (double)iz1) iz1 = fz1 < -1.0 ? -1 : (int)fz1;
+            }
+
+            double denominator = 0.0;                               /* Listing 1 line 5 */
+            size_t cnt = 0;
+            for (int iy = iy0; iy <= iy1; ++iy) {                   /* Listing 1 line 6 */
+                for (int iz = iz0; iz <= iz1; ++iz) {
+                    double y = jo_pixel_y(iy, n_y, pixel), z = jo_pixel_z(iz, n_z, pixel);
+                    if (!(jo_bCb(y - y_t, z - z_t, tan_t, sigma_z, sigma_dl) <= 9.0)) continue;   /* centre inside 3 sigma */
+                    if (cnt == cap) {
+                        cap *= 2;
+                        double *k2 = (double *)realloc(kernel, cap * sizeof(double));
+                        int *p2 = (int *)realloc(pix, cap * sizeof(int));
+                        if (k2) kernel = k2;
+                        if (p2) pix = p2;
+                        if (!k2 || !p2) { failed = 1; break; }
+                    }
+                    int i = iy * n_z + iz;
+                    kernel[cnt] = jo_kernel(y, z, tan_t, y_t, z_t, R, sigma_z, sigma_dl, a3_coef);   /* line 7 */
+                    pix[cnt] = i;
+                    denominator += kernel[cnt] * w[i];              /* line 8, with s(i) of Eq. 3 */
+                    cnt++;
+                }
+                if (failed) break;
+            }
+            if (failed) continue;
+            n_evals += cnt;
+            if (cnt == 0 || !(denominator > 0.0) || !isfinite(denominator)) { n_skipped++; continue; }   /* R16 */
+            for (size_t c = 0; c < cnt; ++c)                        /* lines 10-11; rho(i) pulled out (R11) */
+                rho_new[pix[c]] += kernel[c] / denominator;
+        }
+        free(kernel);
+        free(pix);
+    }
+
+    if (!failed) {
+        for (size_t i = 0; i < M; ++i) {                            /* sum of the thread copies */
+            double acc = 0.0;
+            for (int t = 0; t < n_threads; ++t) acc += rho_new_all[(size_t)t * M + i];
+            rho_out[i] = s[i] > 0.0 ? rho_in[i] * acc : 0.0;        /* Eq. 3; masked where s = 0 (R13) */
+        }
+        if (n_evals_out) *n_evals_out = n_evals;
+        if (n_skipped_out) *n_skipped_out = n_skipped;
+    }
+    free(rho_new_all);
+    free(s);
+    free(w);
+    return failed ? -1 : 0;
+}
+
+/* ---- n_iter iterations from rho_init (NULL => all ones, R18); counters are those of the LAST iteration */
+int jo_reconstruct(const float *events, int64_t n, double R, double L, double sigma_z, double sigma_dl,
+                   int n_y, int n_z, double pixel, double a3_coef, const double *rho_init, double *rho_out,
+                   int n_iter, int n_threads, uint64_t *n_evals_out, uint64_t *n_skipped_out)
+{
+    if (n_iter < 0 || n_y <= 0 || n_z <= 0 || !rho_out) return -1;
+    const size_t M = (size_t)n_y * (size_t)n_z;
+    double *cur = (double *)malloc(M * sizeof(double));
+    if (!cur) return -1;
+    for (size_t i = 0; i < M; ++i) cur[i] = rho_init ? rho_init[i] : 1.0;
+    int rc = 0;
+    for (int it = 0; it < n_iter && rc == 0; ++it) {
+        rc = jo_mlem_iterate(events, n, R, L, sigma_z, sigma_dl, n_y, n_z, pixel, a3_coef, cur, rho_out,
+                             0, n_threads, n_evals_out, n_skipped_out);
+        memcpy(cur, rho_out, M * sizeof(double));
+    }
+    if (n_iter == 0) memcpy(rho_out, cur, M * sizeof(double));
+    free(cur);
+    return rc;
+}
+
+int jo_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
