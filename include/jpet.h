@@ -1,0 +1,134 @@
+/*
+ * jpet.h - C-ABI boundary of the B200 (sm_100a) list-mode MLEM hot path for the two-strip J-PET detector
+ * (arXiv:1502.07478; line numbers below are /root/reference/PAPER.md).
+ *
+ * One MLEM iteration (Eq. 3) is, per event e~_j = (z_u~, z_d~, dl~):
+ *   1. direct reconstruction of (tan theta~, y~, z~)  (Eq. 2) and the pixel set E_j whose
+ *      centres lie inside the 3-sigma ellipse b C^-1 b <= 9  (App. B :251-269);
+ *   2. P(e~_j | i) for i in E_j  (Eq. 7-12, diagonal C) and the denominator
+ *      sum_i P(e~_j|i) s(i) rho(i);
+ *   3. back-projection  acc(i) += P(e~_j|i) / denominator_j  (Listing 1 line 10);
+ *   4. rho_out(l) = rho_in(l) * acc(l) where s(l) > 0, else 0, with s the sensitivity of Eq. 4
+ *      (PAPER.md:75-81).  Equivalent to Eq. 5-6 on rho' = s rho.
+ * Every step runs in hand-written CUDA kernels; there is no CPU fallback.  All functions return JPET_OK (0)
+ * or a negative error code and never throw; jpet_last_error() gives the text for the calling thread.
+ *
+ * Conventions
+ *   - lengths in mm; image plane (y, z); strips at y = +R (upper, "u") and y = -R (lower, "d"), |z| <= L/2;
+ *   - images are float32, row-major [n_y][n_z] (z fastest); pixel (iy, iz) has its centre at
+ *       y = (iy - (n_y-1)/2) * pixel,   z = (iz - (n_z-1)/2) * pixel;
+ *   - events are float32 [n][3] = (z_u~, z_d~, dl~), C-contiguous; never modified;
+ *   - "_dev" pointers are CUDA device pointers on the current device, "_host" pointers are host memory
+ *     (pinned memory makes the copies asynchronous; pageable memory works but serialises);
+ *   - every buffer is owned by the caller; the library owns only its internal workspace
+ *     (sensitivity image, w = s*rho, accumulator replicas, counters, staging buffers), which it grows on
+ *     demand and frees in jpet_release();
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-pointer
+ *     calls are asynchronous on that stream and never synchronise the device; host-pointer calls return
+ *     after their result has landed in the host buffer;
+ *   - the library keeps one workspace per process and is not re-entrant: calls must not overlap in time
+ *     from several host threads.
+ *   - arithmetic is fp32 (accumulation: fp32 atomics into several accumulator replicas that are summed in a
+ *     fixed order); the sensitivity image is evaluated in fp64 and rounded once to fp32.
+ */
+#ifndef JPET_H
+#define JPET_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define JPET_OK 0
+#define JPET_E_INVAL (-1)   /* NULL pointer, n < 0, non-positive R/L/sigma/pixel/n_y/n_z, grid reaching |y| >= R
+                               (Eq. 4 divides by R -+ y), sigmas so large against R that Eq. 7's square root
+                               could go non-positive inside the 3-sigma ellipse, or a sequencing error
+                               (accumulate/end without begin) */
+#define JPET_E_CUDA (-2)    /* a CUDA call failed (allocation, launch, copy); text in jpet_last_error() */
+
+typedef struct { float R; float L; } jpet_geometry;               /* strips y = +-R, |z| <= L/2 */
+typedef struct { float sigma_z; float sigma_dl; } jpet_sigmas;    /* C^-1 = diag(1/sz^2, 1/sz^2, 1/sdl^2), gamma = 0
+                                                                     (Eq. 12 and PAPER.md:124) */
+typedef struct { int32_t n_y; int32_t n_z; float pixel; } jpet_grid;   /* centred on the origin, see above */
+
+/* Sensitivity image, Eq. 4 at every pixel centre, clamped to >= 0 (pixels no LOR through both
+ * strips can see).  s_dev: float32 [n_y*n_z], written. */
+int jpet_sensitivity(const jpet_geometry *geometry, const jpet_grid *grid, float *s_dev, void *cuda_stream);
+
+/* One MLEM iteration, Eq. 3 = steps 1-4 above.
+ *   events_dev : float32 [n][3]; n >= 0 (n == 0 gives rho_out = 0, the empty sum over j)
+ *   rho_in_dev : float32 [n_y*n_z], read;  rho_out_dev: float32 [n_y*n_z], written; the two may alias
+ * Events with a non-finite component, with no pixel centre inside their ellipse, or with a non-positive
+ * denominator are skipped and counted (jpet_get_counters).  Events are processed in internal batches of at
+ * most 10^7 launched back to back on the stream. */
+int jpet_mlem_iterate(const float *events_dev, int64_t n, const jpet_geometry *geometry, const jpet_sigmas *sigmas,
+                      const jpet_grid *grid, const float *rho_in_dev, float *rho_out_dev, void *cuda_stream);
+
+/* n_iter iterations starting from rho_init_dev (NULL => all ones); n_iter == 0 copies the start image.
+ * rho_out_dev may alias rho_init_dev. */
+int jpet_reconstruct(const float *events_dev, int64_t n, const jpet_geometry *geometry, const jpet_sigmas *sigmas,
+                     const jpet_grid *grid, const float *rho_init_dev, float *rho_out_dev, int32_t n_iter,
+                     void *cuda_stream);
+
+/* The same iteration split in three so that a caller can stream event batches (BASELINE config 5):
+ *   begin      : w = s * rho_in, accumulators and counters zeroed
+ *   accumulate : steps 1-3 for one batch of events (device pointer); any number of calls
+ *   end        : step 4 into rho_out_dev (rho_in_dev must hold the same image that was given to begin)
+ * begin/accumulate*\/end on one stream is exactly jpet_mlem_iterate. */
+int jpet_mlem_begin(const jpet_geometry *geometry, const jpet_sigmas *sigmas, const jpet_grid *grid,
+                    const float *rho_in_dev, void *cuda_stream);
+int jpet_mlem_accumulate(const float *events_dev, int64_t n_batch, void *cuda_stream);
+int jpet_mlem_end(const float *rho_in_dev, float *rho_out_dev, void *cuda_stream);
+
+/* Host-buffer forms (the end-to-end path): events and images live in host memory; the call copies the events
+ * to the device in chunks of `chunk_events` (<= 0: library default) on a copy stream that runs ahead of the
+ * compute stream, runs the iteration(s) and copies rho back.  Returns when rho_out_host is complete.
+ * For n_iter > 1 the events are uploaded once if they fit the staging budget (4 GiB), else once per iteration. */
+int jpet_mlem_iterate_host(const float *events_host, int64_t n, const jpet_geometry *geometry,
+                           const jpet_sigmas *sigmas, const jpet_grid *grid, const float *rho_in_host,
+                           float *rho_out_host, int64_t chunk_events);
+int jpet_reconstruct_host(const float *events_host, int64_t n, const jpet_geometry *geometry,
+                          const jpet_sigmas *sigmas, const jpet_grid *grid, const float *rho_init_host,
+                          float *rho_out_host, int32_t n_iter, int64_t chunk_events);
+
+/* Counters of the most recent iteration on `cuda_stream` (synchronises that stream):
+ *   n_evals   = sum_j |E_j|  - unique (event, pixel-centre-inside-ellipse) pairs, the "kernel evaluations"
+ *   n_skipped = events skipped as described above
+ * Either pointer may be NULL. */
+int jpet_get_counters(uint64_t *n_evals_host, uint64_t *n_skipped_host, void *cuda_stream);
+
+/* Counts |E_j| without evaluating the kernel (for evals/s when no iteration has been run).  Synchronises. */
+int jpet_count_evals(const float *events_dev, int64_t n, const jpet_geometry *geometry, const jpet_sigmas *sigmas,
+                     const jpet_grid *grid, uint64_t *n_evals_host, uint64_t *n_skipped_host, void *cuda_stream);
+
+/* Coefficient of the third component of vector a in Eq. 9.  2 (default) makes a = d e/d theta,
+ * consistent with Eq. 8 and Eq. 10; 1 is the equation exactly as printed (reading R5). */
+int jpet_set_a3_coef(float k);
+float jpet_get_a3_coef(void);
+
+/* Tuning knobs (do not change results beyond fp32 summation order).  name/value pairs:
+ *   "replicas"   number of accumulator replicas in L2 (1..64, default chosen from the image size)
+ *   "variant"    event-kernel variant id; -1 = automatic
+ *   "ctas_per_sm" override for the persistent grid size; 0 = automatic
+ * Returns JPET_E_INVAL for an unknown name or a value out of range. */
+int jpet_set_option(const char *name, int64_t value);
+int64_t jpet_get_option(const char *name);
+
+/* Number of kernels this library has launched since load (for bench.py's gpu_launches). */
+uint64_t jpet_launch_count(void);
+
+/* Frees the internal workspace (device and pinned host memory).  Safe to call at any time between calls. */
+void jpet_release(void);
+
+/* Text of the last error on the calling thread ("" if none).  The pointer stays valid until the next call. */
+const char *jpet_last_error(void);
+
+/* ABI version of this header: bumped whenever a signature changes. */
+int jpet_abi_version(void);
+#define JPET_ABI_VERSION 1
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* JPET_H */

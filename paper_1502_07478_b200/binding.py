@@ -1,0 +1,233 @@
+"""Thin ctypes binding of include/jpet.h - argument marshalling only; every step runs in the CUDA kernels.
+
+PyTorch appears here only as the owner of device memory and streams (tensor.data_ptr(), the current stream's
+handle).  There is no CPU fallback: if libjpet.so is missing or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import build as _build
+
+JPET_OK, JPET_E_INVAL, JPET_E_CUDA = 0, -1, -2
+
+EXPORTS = (
+    "jpet_sensitivity", "jpet_mlem_iterate", "jpet_reconstruct", "jpet_mlem_begin", "jpet_mlem_accumulate",
+    "jpet_mlem_end", "jpet_mlem_iterate_host", "jpet_reconstruct_host", "jpet_get_counters", "jpet_count_evals",
+    "jpet_set_a3_coef", "jpet_get_a3_coef", "jpet_set_option", "jpet_get_option", "jpet_launch_count",
+    "jpet_release", "jpet_last_error", "jpet_abi_version",
+)
+
+
+class Geometry(ctypes.Structure):
+    _fields_ = [("R", ctypes.c_float), ("L", ctypes.c_float)]
+
+
+class Sigmas(ctypes.Structure):
+    _fields_ = [("sigma_z", ctypes.c_float), ("sigma_dl", ctypes.c_float)]
+
+
+class Grid(ctypes.Structure):
+    _fields_ = [("n_y", ctypes.c_int32), ("n_z", ctypes.c_int32), ("pixel", ctypes.c_float)]
+
+
+class JpetError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"jpet error {code}: {text}")
+        self.code = code
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load(build_if_missing: bool = True) -> ctypes.CDLL:
+    """Loads libjpet.so (building it in-tree with nvcc if it is missing and nvcc is there). Raises loudly otherwise."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if not os.path.exists(path):
+        if not build_if_missing:
+            raise FileNotFoundError(f"{path} is missing: run python -m paper_1502_07478_b200.build")
+        path = _build.build()
+    lib = ctypes.CDLL(path)
+    p, i32, i64, u64p = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.POINTER(ctypes.c_uint64)
+    G, S, Gr = ctypes.POINTER(Geometry), ctypes.POINTER(Sigmas), ctypes.POINTER(Grid)
+    sigs = {
+        "jpet_sensitivity": (ctypes.c_int, [G, Gr, p, p]),
+        "jpet_mlem_iterate": (ctypes.c_int, [p, i64, G, S, Gr, p, p, p]),
+        "jpet_reconstruct": (ctypes.c_int, [p, i64, G, S, Gr, p, p, i32, p]),
+        "jpet_mlem_begin": (ctypes.c_int, [G, S, Gr, p, p]),
+        "jpet_mlem_accumulate": (ctypes.c_int, [p, i64, p]),
+        "jpet_mlem_end": (ctypes.c_int, [p, p, p]),
+        "jpet_mlem_iterate_host": (ctypes.c_int, [p, i64, G, S, Gr, p, p, i64]),
+        "jpet_reconstruct_host": (ctypes.c_int, [p, i64, G, S, Gr, p, p, i32, i64]),
+        "jpet_get_counters": (ctypes.c_int, [u64p, u64p, p]),
+        "jpet_count_evals": (ctypes.c_int, [p, i64, G, S, Gr, u64p, u64p, p]),
+        "jpet_set_a3_coef": (ctypes.c_int, [ctypes.c_float]),
+        "jpet_get_a3_coef": (ctypes.c_float, []),
+        "jpet_set_option": (ctypes.c_int, [ctypes.c_char_p, i64]),
+        "jpet_get_option": (i64, [ctypes.c_char_p]),
+        "jpet_launch_count": (ctypes.c_uint64, []),
+        "jpet_release": (None, []),
+        "jpet_last_error": (ctypes.c_char_p, []),
+        "jpet_abi_version": (ctypes.c_int, []),
+    }
+    for name, (res, args) in sigs.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = lib
+    return lib
+
+
+def _check(rc: int) -> None:
+    if rc != JPET_OK:
+        raise JpetError(rc, load().jpet_last_error().decode())
+
+
+def _stream_handle(stream) -> int:
+    if stream is None:
+        import torch
+
+        return int(torch.cuda.current_stream().cuda_stream)
+    return int(getattr(stream, "cuda_stream", stream))
+
+
+def _dev_f32(t, numel: int | None, what: str) -> int:
+    import torch
+
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+        raise TypeError(f"{what} must be a contiguous float32 CUDA tensor")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{what} must hold {numel} elements, has {t.numel()}")
+    return t.data_ptr()
+
+
+def _host_f32(t, numel: int | None, what: str) -> int:
+    import torch
+
+    if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+        raise TypeError(f"{what} must be a contiguous float32 CPU tensor (pinned for asynchronous copies)")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{what} must hold {numel} elements, has {t.numel()}")
+    return t.data_ptr()
+
+
+def _structs(R, L, sigma_z, sigma_dl, n_y, n_z, pixel):
+    return Geometry(R, L), Sigmas(sigma_z, sigma_dl), Grid(n_y, n_z, pixel)
+
+
+def _events_ptr(events, dev: bool):
+    if events.dim() != 2 or events.shape[1] != 3:
+        raise ValueError("events must be [n, 3]")
+    return (_dev_f32 if dev else _host_f32)(events, None, "events"), int(events.shape[0])
+
+
+# ---- the calls, same names as include/jpet.h ---------------------------------------------------------------
+def jpet_sensitivity(R, L, n_y, n_z, pixel, s_dev, stream=None):
+    g, _, gr = _structs(R, L, 1.0, 1.0, n_y, n_z, pixel)
+    _check(load().jpet_sensitivity(g, gr, _dev_f32(s_dev, n_y * n_z, "s_dev"), _stream_handle(stream)))
+    return s_dev
+
+
+def jpet_mlem_iterate(events_dev, R, L, sigma_z, sigma_dl, n_y, n_z, pixel, rho_in_dev, rho_out_dev, stream=None):
+    g, s, gr = _structs(R, L, sigma_z, sigma_dl, n_y, n_z, pixel)
+    ev, n = _events_ptr(events_dev, True)
+    _check(load().jpet_mlem_iterate(ev, n, g, s, gr, _dev_f32(rho_in_dev, n_y * n_z, "rho_in_dev"),
+                                    _dev_f32(rho_out_dev, n_y * n_z, "rho_out_dev"), _stream_handle(stream)))
+    return rho_out_dev
+
+
+def jpet_reconstruct(events_dev, R, L, sigma_z, sigma_dl, n_y, n_z, pixel, rho_init_dev, rho_out_dev, n_iter, stream=None):
+    g, s, gr = _structs(R, L, sigma_z, sigma_dl, n_y, n_z, pixel)
+    ev, n = _events_ptr(events_dev, True)
+    init = None if rho_init_dev is None else _dev_f32(rho_init_dev, n_y * n_z, "rho_init_dev")
+    _check(load().jpet_reconstruct(ev, n, g, s, gr, init, _dev_f32(rho_out_dev, n_y * n_z, "rho_out_dev"),
+                                   int(n_iter), _stream_handle(stream)))
+    return rho_out_dev
+
+
+def jpet_mlem_begin(R, L, sigma_z, sigma_dl, n_y, n_z, pixel, rho_in_dev, stream=None):
+    g, s, gr = _structs(R, L, sigma_z, sigma_dl, n_y, n_z, pixel)
+    _check(load().jpet_mlem_begin(g, s, gr, _dev_f32(rho_in_dev, n_y * n_z, "rho_in_dev"), _stream_handle(stream)))
+
+
+def jpet_mlem_accumulate(events_dev, stream=None):
+    ev, n = _events_ptr(events_dev, True)
+    _check(load().jpet_mlem_accumulate(ev, n, _stream_handle(stream)))
+
+
+def jpet_mlem_end(rho_in_dev, rho_out_dev, stream=None):
+    _check(load().jpet_mlem_end(_dev_f32(rho_in_dev, None, "rho_in_dev"), _dev_f32(rho_out_dev, None, "rho_out_dev"),
+                                _stream_handle(stream)))
+    return rho_out_dev
+
+
+def jpet_mlem_iterate_host(events_host, R, L, sigma_z, sigma_dl, n_y, n_z, pixel, rho_in_host, rho_out_host, chunk_events=0):
+    g, s, gr = _structs(R, L, sigma_z, sigma_dl, n_y, n_z, pixel)
+    ev, n = _events_ptr(events_host, False)
+    _check(load().jpet_mlem_iterate_host(ev, n, g, s, gr, _host_f32(rho_in_host, n_y * n_z, "rho_in_host"),
+                                         _host_f32(rho_out_host, n_y * n_z, "rho_out_host"), int(chunk_events)))
+    return rho_out_host
+
+
+def jpet_reconstruct_host(events_host, R, L, sigma_z, sigma_dl, n_y, n_z, pixel, rho_init_host, rho_out_host, n_iter,
+                          chunk_events=0):
+    g, s, gr = _structs(R, L, sigma_z, sigma_dl, n_y, n_z, pixel)
+    ev, n = _events_ptr(events_host, False)
+    init = None if rho_init_host is None else _host_f32(rho_init_host, n_y * n_z, "rho_init_host")
+    _check(load().jpet_reconstruct_host(ev, n, g, s, gr, init, _host_f32(rho_out_host, n_y * n_z, "rho_out_host"),
+                                        int(n_iter), int(chunk_events)))
+    return rho_out_host
+
+
+def jpet_get_counters(stream=None):
+    """(n_evals, n_skipped) of the most recent iteration; synchronises the stream."""
+    a, b = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    _check(load().jpet_get_counters(ctypes.byref(a), ctypes.byref(b), _stream_handle(stream)))
+    return int(a.value), int(b.value)
+
+
+def jpet_count_evals(events_dev, R, L, sigma_z, sigma_dl, n_y, n_z, pixel, stream=None):
+    g, s, gr = _structs(R, L, sigma_z, sigma_dl, n_y, n_z, pixel)
+    ev, n = _events_ptr(events_dev, True)
+    a, b = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    _check(load().jpet_count_evals(ev, n, g, s, gr, ctypes.byref(a), ctypes.byref(b), _stream_handle(stream)))
+    return int(a.value), int(b.value)
+
+
+def jpet_set_a3_coef(k: float) -> None:
+    _check(load().jpet_set_a3_coef(float(k)))
+
+
+def jpet_get_a3_coef() -> float:
+    return float(load().jpet_get_a3_coef())
+
+
+def jpet_set_option(name: str, value: int) -> None:
+    _check(load().jpet_set_option(name.encode(), int(value)))
+
+
+def jpet_get_option(name: str) -> int:
+    return int(load().jpet_get_option(name.encode()))
+
+
+def jpet_launch_count() -> int:
+    return int(load().jpet_launch_count())
+
+
+def jpet_release() -> None:
+    load().jpet_release()
+
+
+def jpet_last_error() -> str:
+    return load().jpet_last_error().decode()
+
+
+def jpet_abi_version() -> int:
+    return int(load().jpet_abi_version())

@@ -1,0 +1,323 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the fp64 CPU oracle, element by element on
+the same seeded events.  Tolerances are north_star's: max |rho_gpu - rho_oracle| / max(rho_oracle) <= 1e-4
+after 1 iteration and <= 1e-3 after 10.  Run on the B200 box with  pytest -m gpu.
+"""
+import numpy as np
+import pytest
+
+from paper_1502_07478_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_1 = 1e-4    # one iteration, relative to the image maximum (BASELINE.json north_star)
+TOL_10 = 1e-3   # ten iterations
+
+
+@pytest.fixture(scope="module")
+def jp():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; there is no CPU fallback")
+    import paper_1502_07478_b200 as jp
+
+    jp.binding.load(build_if_missing=False)   # the in-tree .so must be the one that runs
+    yield jp
+    jp.jpet_set_option("variant", -1)
+    jp.jpet_set_option("replicas", 0)
+    jp.jpet_set_a3_coef(2.0)
+
+
+def geom(cfg):
+    return (cfg.R, cfg.L, cfg.sigma_z, cfg.sigma_dl, cfg.n_y, cfg.n_z, cfg.pixel)
+
+
+def gpu_iterate(jp, ev, cfg, rho_in, n_iter=1):
+    import torch
+
+    ev_d = torch.from_numpy(np.ascontiguousarray(ev)).cuda()
+    rho = torch.from_numpy(np.ascontiguousarray(rho_in, dtype=np.float32)).cuda().reshape(-1)
+    out = torch.empty_like(rho)
+    if n_iter == 1:
+        jp.jpet_mlem_iterate(ev_d, *geom(cfg), rho, out)
+    else:
+        jp.jpet_reconstruct(ev_d, *geom(cfg), rho, out, n_iter)
+    counters = jp.jpet_get_counters()
+    return out.cpu().numpy().astype(np.float64).reshape(cfg.n_y, cfg.n_z), counters
+
+
+def rel_err(got, want):
+    return float(np.max(np.abs(got - want)) / np.max(want))
+
+
+# ------------------------------------------------------------------------------------------------------
+def test_sensitivity_all_grids(jp, oracle):
+    import torch
+
+    for cfg in synth.CONFIGS.values():
+        s = torch.empty(cfg.n_y * cfg.n_z, device="cuda")
+        jp.jpet_sensitivity(cfg.R, cfg.L, cfg.n_y, cfg.n_z, cfg.pixel, s)
+        want = oracle.sensitivity_image(cfg.R, cfg.L, cfg.n_y, cfg.n_z, cfg.pixel)
+        got = s.cpu().numpy().reshape(cfg.n_y, cfg.n_z)
+        assert np.max(np.abs(got - want)) <= 6e-8 * want.max()          # one fp32 rounding of the fp64 value
+        assert ((got == 0) == (want == 0)).all()
+
+
+@pytest.mark.parametrize("a3", [2.0, 1.0])
+def test_cfg1_one_iteration(jp, oracle, a3):
+    cfg = synth.CONFIGS["cfg1"]
+    ev = synth.config_events(cfg)
+    jp.jpet_set_a3_coef(a3)
+    rng = np.random.default_rng(0)
+    for rho in (np.ones((cfg.n_y, cfg.n_z)), rng.uniform(0.2, 3.0, (cfg.n_y, cfg.n_z)).astype(np.float32)):
+        got, (ne, ns) = gpu_iterate(jp, ev, cfg, rho)
+        want, one, ons = oracle.mlem_iterate(ev, *geom(cfg), rho, a3_coef=a3)
+        assert rel_err(got, want) <= TOL_1
+        assert ns == ons == 0
+        assert abs(ne - one) <= 1e-5 * one + 2          # ellipse-boundary ties may flip between fp32 and fp64 (R20)
+    jp.jpet_set_a3_coef(2.0)
+
+
+def test_a3_coefficient_is_honoured(jp, oracle):
+    """k=1 and k=2 images differ by ~3.5e-5 of max on config 1: the GPU must track each."""
+    cfg = synth.CONFIGS["cfg1"]
+    ev = synth.config_events(cfg)
+    ones = np.ones((cfg.n_y, cfg.n_z))
+    jp.jpet_set_a3_coef(1.0)
+    g1, _ = gpu_iterate(jp, ev, cfg, ones)
+    jp.jpet_set_a3_coef(2.0)
+    g2, _ = gpu_iterate(jp, ev, cfg, ones)
+    o1, _, _ = oracle.mlem_iterate(ev, *geom(cfg), ones, a3_coef=1.0)
+    o2, _, _ = oracle.mlem_iterate(ev, *geom(cfg), ones, a3_coef=2.0)
+    d_or = (o1 - o2) / o2.max()
+    d_gpu = (g1 - g2) / o2.max()
+    assert np.max(np.abs(d_or)) > 1e-5
+    assert np.max(np.abs(d_gpu - d_or)) < 0.3 * np.max(np.abs(d_or))
+
+
+def test_cfg1_ten_iterations(jp, oracle):
+    cfg = synth.CONFIGS["cfg1"]
+    ev = synth.config_events(cfg)
+    got, _ = gpu_iterate(jp, ev, cfg, np.ones((cfg.n_y, cfg.n_z)), n_iter=10)
+    want, _, _ = oracle.reconstruct(ev, *geom(cfg), 10)
+    assert rel_err(got, want) <= TOL_10
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("name,n", [("cfg1", 7777), ("cfg2", 30011), ("cfg4", 5003)])
+def test_every_kernel_variant(jp, oracle, variant, name, n):
+    """Each event-kernel shape (segment width, warps per event, cached iterations) on small, medium and
+    large ellipses; on config 4 the narrow variants overflow their register cache and take the recompute path."""
+    cfg = synth.CONFIGS[name]
+    ev = synth.config_events(cfg, n=n)
+    rho = np.random.default_rng(1).uniform(0.5, 2.0, (cfg.n_y, cfg.n_z)).astype(np.float32)
+    jp.jpet_set_option("variant", variant)
+    try:
+        got, (ne, ns) = gpu_iterate(jp, ev, cfg, rho)
+        assert jp.jpet_get_option("last_variant") == variant
+    finally:
+        jp.jpet_set_option("variant", -1)
+    want, one, ons = oracle.mlem_iterate(ev, *geom(cfg), rho)
+    assert rel_err(got, want) <= TOL_1
+    assert ns == ons and abs(ne - one) <= 1e-5 * one + 2
+
+
+def test_cfg2_full_size_one_and_ten_iterations(jp, oracle):
+    """BASELINE configs[1] at full size (10^6 events, 200x200), the workload bench.py times."""
+    cfg = synth.CONFIGS["cfg2"]
+    ev = synth.config_events(cfg)
+    ones = np.ones((cfg.n_y, cfg.n_z))
+    got, (ne, ns) = gpu_iterate(jp, ev, cfg, ones)
+    want, one, ons = oracle.mlem_iterate(ev, *geom(cfg), ones)
+    assert rel_err(got, want) <= TOL_1
+    assert ns == ons and abs(ne - one) <= 1e-5 * one
+    got10, _ = gpu_iterate(jp, ev, cfg, ones, n_iter=10)
+    want10, _, _ = oracle.reconstruct(ev, *geom(cfg), 10)
+    assert rel_err(got10, want10) <= TOL_10
+
+
+@pytest.mark.parametrize("name,n", [("cfg3", 1_000_000), ("cfg4", 300_000), ("cfg5", 200_000)])
+def test_large_configs_on_a_prefix(jp, oracle, name, n):
+    """Configs 3-5: the oracle runs one iteration on the first n events of the same array (full grid)."""
+    cfg = synth.CONFIGS[name]
+    ev = synth.config_events(cfg, n=n)
+    ones = np.ones((cfg.n_y, cfg.n_z))
+    got, (ne, ns) = gpu_iterate(jp, ev, cfg, ones)
+    want, one, ons = oracle.mlem_iterate(ev, *geom(cfg), ones)
+    assert rel_err(got, want) <= TOL_1
+    assert ns == ons and abs(ne - one) <= 1e-5 * one
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_full_size_properties(jp, oracle, name):
+    """10^7 events (too many for the oracle in a test): properties that hold at any size -
+    count conservation sum_l s(l) rho_out(l) = N - n_skipped, the evaluation count against
+    jpet_count_evals, invariance under a permutation of the events, and sampled pixels against the oracle
+    run on the few thousand events that can reach them."""
+    import torch
+
+    cfg = synth.CONFIGS[name]
+    ev = synth.config_events(cfg)
+    ev_d = torch.from_numpy(ev).cuda()
+    rho = torch.ones(cfg.n_y * cfg.n_z, device="cuda")
+    out = torch.empty_like(rho)
+    jp.jpet_mlem_iterate(ev_d, *geom(cfg), rho, out)
+    ne, ns = jp.jpet_get_counters()
+    ce, cs = jp.jpet_count_evals(ev_d, *geom(cfg))
+    assert (ne, ns) == (ce, cs)
+    s = oracle.sensitivity_image(cfg.R, cfg.L, cfg.n_y, cfg.n_z, cfg.pixel)
+    got = out.cpu().numpy().astype(np.float64).reshape(cfg.n_y, cfg.n_z)
+    assert abs((s * got).sum() - (len(ev) - ns)) <= 2e-5 * len(ev)
+    perm = torch.randperm(len(ev), device="cuda", generator=torch.Generator(device="cuda").manual_seed(0))
+    out2 = torch.empty_like(rho)
+    jp.jpet_mlem_iterate(ev_d[perm].contiguous(), *geom(cfg), rho, out2)
+    assert float((out2 - out).abs().max() / out.max()) <= TOL_1
+    # sampled pixels: only events whose ellipse can reach the pixel matter for acc(l), but every event's
+    # denominator needs its whole ellipse -> run the oracle on the subset of events near the pixel
+    _, y_t, z_t = _eq2_np(ev, cfg.R)
+    ys = (np.arange(cfg.n_y) - 0.5 * (cfg.n_y - 1)) * cfg.pixel
+    zs = (np.arange(cfg.n_z) - 0.5 * (cfg.n_z - 1)) * cfg.pixel
+    rng = np.random.default_rng(5)
+    hz_max = 3.0 * np.sqrt(cfg.sigma_z**2 / 2 + 0.08 * cfg.sigma_dl**2) + cfg.pixel   # sin^2(theta)/4 <= 0.08 here
+    checked = 0
+    for _ in range(6):
+        iy, iz = int(rng.integers(cfg.n_y // 4, 3 * cfg.n_y // 4)), int(rng.integers(cfg.n_z // 4, 3 * cfg.n_z // 4))
+        near = (np.abs(y_t - ys[iy]) <= 1.5 * cfg.sigma_dl + cfg.pixel) & (np.abs(z_t - zs[iz]) <= hz_max)
+        if near.sum() > 1_200_000 or checked >= 2:
+            continue
+        want, _, _ = oracle.mlem_iterate(ev[near], *geom(cfg), np.ones((cfg.n_y, cfg.n_z)))
+        assert abs(got[iy, iz] - want[iy, iz]) <= TOL_1 * got.max()
+        checked += 1
+    assert checked > 0 or name == "cfg4"   # config 4's ellipses are so wide that every pixel sees > 1.2M events
+
+
+def _eq2_np(ev, R):
+    """Only used to pre-select events near a sampled pixel (test plumbing, generous margins)."""
+    t = (ev[:, 0].astype(np.float64) - ev[:, 1]) / (2 * R)
+    y = -0.5 * ev[:, 2] / np.sqrt(1 + t * t)
+    z = 0.5 * (ev[:, 0].astype(np.float64) + ev[:, 1]) + y * t
+    return t, y, z
+
+
+def test_cfg5_streamed_batches(jp, oracle):
+    """Config 5's shape (512x512, 1 mm): events streamed in batches through begin/accumulate/end equal one
+    jpet_mlem_iterate over the concatenation, and both match the oracle on the same events."""
+    import torch
+
+    cfg = synth.CONFIGS["cfg5"]
+    ev = synth.config_events(cfg, n=150_000)
+    ev_d = torch.from_numpy(ev).cuda()
+    rho = torch.ones(cfg.n_y * cfg.n_z, device="cuda")
+    whole = torch.empty_like(rho)
+    jp.jpet_mlem_iterate(ev_d, *geom(cfg), rho, whole)
+    split = torch.empty_like(rho)
+    jp.jpet_mlem_begin(*geom(cfg), rho)
+    for lo, hi in ((0, 50_001), (50_001, 50_001), (50_001, 149_999), (149_999, 150_000)):
+        jp.jpet_mlem_accumulate(ev_d[lo:hi])
+    jp.jpet_mlem_end(rho, split)
+    ne, ns = jp.jpet_get_counters()
+    want, one, ons = oracle.mlem_iterate(ev, *geom(cfg), np.ones((cfg.n_y, cfg.n_z)))
+    assert float((split - whole).abs().max() / whole.max()) <= 2e-6
+    assert rel_err(split.cpu().numpy().astype(np.float64).reshape(cfg.n_y, cfg.n_z), want) <= TOL_1
+    assert ns == ons and abs(ne - one) <= 1e-5 * one
+    # columns with |z| > L/2 have s = 0 -> rho_out = 0 there (R13)
+    img = split.cpu().numpy().reshape(cfg.n_y, cfg.n_z)
+    assert (img[:, :6] == 0).all() and (img[:, -6:] == 0).all()
+
+
+def test_host_buffer_calls_match_device_calls(jp, oracle):
+    import torch
+
+    cfg = synth.CONFIGS["cfg2"]
+    ev = synth.config_events(cfg, n=123_457)
+    ev_h = torch.from_numpy(ev).pin_memory()
+    rho_h = torch.ones(cfg.n_y * cfg.n_z).pin_memory()
+    out_h = torch.empty(cfg.n_y * cfg.n_z).pin_memory()
+    jp.jpet_mlem_iterate_host(ev_h, *geom(cfg), rho_h, out_h, chunk_events=20_000)
+    want, _, _ = oracle.mlem_iterate(ev, *geom(cfg), np.ones((cfg.n_y, cfg.n_z)))
+    assert rel_err(out_h.numpy().astype(np.float64).reshape(cfg.n_y, cfg.n_z), want) <= TOL_1
+    out3 = torch.empty(cfg.n_y * cfg.n_z)          # pageable memory works too
+    jp.jpet_reconstruct_host(torch.from_numpy(ev), *geom(cfg), None, out3, 3, chunk_events=50_000)
+    want3, _, _ = oracle.reconstruct(ev, *geom(cfg), 3)
+    assert rel_err(out3.numpy().astype(np.float64).reshape(cfg.n_y, cfg.n_z), want3) <= TOL_10
+
+
+def test_edge_cases(jp, oracle):
+    import torch
+
+    cfg = synth.CONFIGS["cfg1"]
+    M = cfg.n_y * cfg.n_z
+    ones = torch.ones(M, device="cuda")
+    out = torch.full((M,), 7.0, device="cuda")
+    # empty event list: rho_out = 0 (empty sum over j)
+    jp.jpet_mlem_iterate(torch.empty((0, 3), device="cuda"), *geom(cfg), ones, out)
+    assert float(out.abs().max()) == 0.0 and jp.jpet_get_counters() == (0, 0)
+    # skipped events: outside the grid, NaN / inf components, all-zero rho under the ellipse
+    bad = np.array([[2000.0, 2000.0, 0.0], [np.nan, 0.0, 0.0], [0.0, np.inf, 0.0], [0.0, 0.0, 5000.0]], np.float32)
+    good = synth.config_events(cfg, n=999)
+    ev = np.concatenate([bad[:2], good, bad[2:]])
+    got, (ne, ns) = gpu_iterate(jp, ev, cfg, np.ones((cfg.n_y, cfg.n_z)))
+    want, one, ons = oracle.mlem_iterate(ev, *geom(cfg), np.ones((cfg.n_y, cfg.n_z)))
+    assert ns == ons == 4 and abs(ne - one) <= 2
+    assert np.isfinite(got).all() and rel_err(got, want) <= TOL_1
+    got0, (_, ns0) = gpu_iterate(jp, good, cfg, np.zeros((cfg.n_y, cfg.n_z)))
+    assert (got0 == 0).all() and ns0 == len(good)
+    # single event against the oracle (ellipse clipped by the grid edge as well)
+    for e in ([120.0, -60.0, -80.0], [-230.0, -180.0, 250.0]):
+        ev1 = np.array([e], np.float32)
+        g1, (ne1, ns1) = gpu_iterate(jp, ev1, cfg, np.ones((cfg.n_y, cfg.n_z)))
+        w1, one1, ons1 = oracle.mlem_iterate(ev1, *geom(cfg), np.ones((cfg.n_y, cfg.n_z)))
+        assert (ne1, ns1) == (one1, ons1) and rel_err(g1, w1) <= 1e-5
+    # in-place: rho_out aliases rho_in
+    rho = torch.ones(M, device="cuda")
+    ev_d = torch.from_numpy(good).cuda()
+    ref = torch.empty(M, device="cuda")
+    jp.jpet_mlem_iterate(ev_d, *geom(cfg), rho, ref)
+    jp.jpet_mlem_iterate(ev_d, *geom(cfg), rho, rho)
+    assert float((rho - ref).abs().max() / ref.max()) <= 2e-6
+    # n_iter = 0 returns the start image; NULL start image means ones
+    out0 = torch.empty(M, device="cuda")
+    jp.jpet_reconstruct(ev_d, *geom(cfg), None, out0, 0)
+    assert float((out0 - 1).abs().max()) == 0.0
+    # 1x1 and non-square grids
+    for n_y, n_z, px in ((1, 1, 50.0), (3, 97, 4.0), (61, 2, 7.0)):
+        g = (cfg.R, cfg.L, cfg.sigma_z, cfg.sigma_dl, n_y, n_z, px)
+        r = np.random.default_rng(3).uniform(0.5, 1.5, (n_y, n_z)).astype(np.float32)
+        o = torch.empty(n_y * n_z, device="cuda")
+        jp.jpet_mlem_iterate(ev_d, *g, torch.from_numpy(r).cuda().reshape(-1), o)
+        cnt = jp.jpet_get_counters()
+        w, one, ons = oracle.mlem_iterate(good, *g, r)
+        assert cnt[1] == ons and abs(cnt[0] - one) <= 2
+        if w.max() > 0:
+            assert rel_err(o.cpu().numpy().astype(np.float64).reshape(n_y, n_z), w) <= TOL_1
+
+
+def test_errors_are_reported_not_swallowed(jp):
+    import torch
+
+    cfg = synth.CONFIGS["cfg1"]
+    M = cfg.n_y * cfg.n_z
+    ones = torch.ones(M, device="cuda")
+    with pytest.raises(jp.JpetError):
+        jp.jpet_mlem_iterate(torch.empty((4, 3), device="cuda"), cfg.R, cfg.L, -1.0, 40.0, cfg.n_y, cfg.n_z, cfg.pixel, ones, ones)
+    with pytest.raises(jp.JpetError):
+        jp.jpet_mlem_accumulate(torch.empty((4, 3), device="cuda"))
+    with pytest.raises(TypeError):
+        jp.jpet_mlem_iterate(torch.empty((4, 3)), *geom(cfg), ones, ones)           # CPU tensor on the device path
+    with pytest.raises(ValueError):
+        jp.jpet_mlem_iterate(torch.empty((4, 3), device="cuda"), *geom(cfg), ones[:-1], ones)
+
+
+def test_replicas_and_determinism_of_the_reduction(jp, oracle):
+    cfg = synth.CONFIGS["cfg2"]
+    ev = synth.config_events(cfg, n=50_000)
+    ones = np.ones((cfg.n_y, cfg.n_z))
+    want, _, _ = oracle.mlem_iterate(ev, *geom(cfg), ones)
+    try:
+        for rep in (1, 3, 16):
+            jp.jpet_set_option("replicas", rep)
+            got, _ = gpu_iterate(jp, ev, cfg, ones)
+            assert jp.jpet_get_option("last_replicas") == rep
+            assert rel_err(got, want) <= TOL_1
+    finally:
+        jp.jpet_set_option("replicas", 0)
