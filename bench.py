@@ -141,7 +141,8 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--events", type=int, default=0, help="override the number of events (0 = the config's)")
     ap.add_argument("--variant", type=int, default=-1)
-    ap.add_argument("--replicas", type=int, default=0)
+    ap.add_argument("--chunk", type=int, default=0)
+    ap.add_argument("--ctas-per-sm", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -173,8 +174,10 @@ def main():
     jp.binding.load(build_if_missing=False)
     if args.variant >= 0:
         jp.jpet_set_option("variant", args.variant)
-    if args.replicas > 0:
-        jp.jpet_set_option("replicas", args.replicas)
+    if args.chunk > 0:
+        jp.jpet_set_option("chunk", args.chunk)
+    if args.ctas_per_sm > 0:
+        jp.jpet_set_option("ctas_per_sm", args.ctas_per_sm)
 
     n_events = args.events or cfg.n_events
     events = synth.config_events(cfg, n=n_events, seed=cfg.seed + rank)     # replicas: same shape, own seed
@@ -213,15 +216,21 @@ def main():
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
+    jp.jpet_set_option("time_kernel", 1)
     launches0 = jp.jpet_launch_count()
-    pairs = []
+    pairs, kern_ms = [], []
     for i in range(args.steps):
         flush.zero_()
         step(args.warmup + i, pairs)
+        ns = jp.jpet_get_option("last_kernel_ns")          # waits for this step's event kernel only
+        if ns > 0:
+            kern_ms.append(ns * 1e-6)
     barrier()
     launches = jp.jpet_launch_count() - launches0
+    jp.jpet_set_option("time_kernel", 0)
     step_ms = [a.elapsed_time(d) for a, _, _, d in pairs]
-    kern_ms = [b.elapsed_time(c) for _, b, c, _ in pairs]
+    acc_ms = [b.elapsed_time(c) for _, b, c, _ in pairs]          # binning + event kernels of the step
+    kern_ms = kern_ms or acc_ms
     total_ms = sum(step_ms)
     if dist is not None:
         t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
@@ -268,10 +277,11 @@ def main():
     peak_evals = n_sm * 8.0 * sm_mhz_peak * 1e6
     kern_s = statistics.mean(kern_ms) * 1e-3
     achieved = n_evals / kern_s
-    roofline = {"bound": "alu", "kernel": "mlem_events_kernel", "achieved": achieved / 1e9, "peak": peak_evals / 1e9,
+    roofline = {"bound": "alu", "kernel": "mlem_rows_kernel", "achieved": achieved / 1e9, "peak": peak_evals / 1e9,
                 "unit": "Geval/s", "frac": achieved / peak_evals, "traffic": None,
                 "peak_source": f"{n_sm} SMs x 16 MUFU/clk / 2 MUFU per eval x {sm_mhz_peak:.0f} MHz ({peak_kind} sm_max_mhz)",
-                "kernel_ms": kern_s * 1e3, "kernel_share_of_step": sum(kern_ms) / sum(step_ms),
+                "kernel_ms": kern_s * 1e3, "kernel_share_of_step": statistics.mean(kern_ms) / statistics.mean(step_ms),
+                "binning_plus_kernels_ms": statistics.mean(acc_ms),
                 "hbm_gbs_algorithmic": (events.nbytes + 8 * M) / kern_s / 1e9, "hbm_peak_gbs": peaks.get("hbm_gbs")}
 
     cpu_baseline = None
@@ -284,7 +294,7 @@ def main():
             "config": {"workload": cfg.name, "grid": [cfg.n_y, cfg.n_z], "pixel_mm": cfg.pixel, "sigma_z": cfg.sigma_z,
                        "sigma_dl": cfg.sigma_dl, "events": n_events, "parallelism": "replicas only" if world > 1 else "1 gpu",
                        "l2": "flushed between steps (256 MiB memset)", "kernel_variant": jp.jpet_get_option("last_variant"),
-                       "acc_replicas": jp.jpet_get_option("last_replicas")},
+                       "tiled": bool(jp.jpet_get_option("last_tiled")), "smem_bytes": jp.jpet_get_option("last_smem_bytes")},
             "kernel_evals_per_s": world * n_evals / (ms_per_step * 1e-3), "kernel_evals_per_iteration": n_evals,
             "px_per_event": n_evals / max(n_events, 1), "events_skipped": n_skipped,
             "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu_baseline, "clocks": clocks}

@@ -28,8 +28,9 @@
  *     after their result has landed in the host buffer;
  *   - the library keeps one workspace per process and is not re-entrant: calls must not overlap in time
  *     from several host threads.
- *   - arithmetic is fp32 (accumulation: fp32 atomics into several accumulator replicas that are summed in a
- *     fixed order); the sensitivity image is evaluated in fp64 and rounded once to fp32.
+ *   - arithmetic is fp32 (accumulation: fp32 partial sums per work item in shared memory, merged into the image
+ *     with fp32 atomics, so the summation order - and the last bits - vary from run to run); the sensitivity
+ *     image is evaluated in fp64 and rounded once to fp32.
  */
 #ifndef JPET_H
 #define JPET_H
@@ -61,7 +62,7 @@ int jpet_sensitivity(const jpet_geometry *geometry, const jpet_grid *grid, float
  *   rho_in_dev : float32 [n_y*n_z], read;  rho_out_dev: float32 [n_y*n_z], written; the two may alias
  * Events with a non-finite component, with no pixel centre inside their ellipse, or with a non-positive
  * denominator are skipped and counted (jpet_get_counters).  Events are processed in internal batches of at
- * most 10^7 launched back to back on the stream. */
+ * most 10^7 (sorted by image sub-tile on the device, then the event kernels) launched back to back on the stream. */
 int jpet_mlem_iterate(const float *events_dev, int64_t n, const jpet_geometry *geometry, const jpet_sigmas *sigmas,
                       const jpet_grid *grid, const float *rho_in_dev, float *rho_out_dev, void *cuda_stream);
 
@@ -75,7 +76,7 @@ int jpet_reconstruct(const float *events_dev, int64_t n, const jpet_geometry *ge
  *   begin      : w = s * rho_in, accumulators and counters zeroed
  *   accumulate : steps 1-3 for one batch of events (device pointer); any number of calls
  *   end        : step 4 into rho_out_dev (rho_in_dev must hold the same image that was given to begin)
- * begin/accumulate*\/end on one stream is exactly jpet_mlem_iterate. */
+ * begin, accumulate (any number of times), end on one stream is exactly jpet_mlem_iterate. */
 int jpet_mlem_begin(const jpet_geometry *geometry, const jpet_sigmas *sigmas, const jpet_grid *grid,
                     const float *rho_in_dev, void *cuda_stream);
 int jpet_mlem_accumulate(const float *events_dev, int64_t n_batch, void *cuda_stream);
@@ -108,9 +109,14 @@ int jpet_set_a3_coef(float k);
 float jpet_get_a3_coef(void);
 
 /* Tuning knobs (do not change results beyond fp32 summation order).  name/value pairs:
- *   "replicas"   number of accumulator replicas in L2 (1..64, default chosen from the image size)
- *   "variant"    event-kernel variant id; -1 = automatic
- *   "ctas_per_sm" override for the persistent grid size; 0 = automatic
+ *   "variant"      event-kernel shape id; -1 = automatic
+ *   "force_direct" 1 = skip the shared-memory tiled path: every event goes through the direct kernel
+ *                  (w from global memory, red.global.add into the image); 0 = automatic
+ *   "chunk"        events per work item of the tiled path; 0 = automatic
+ *   "ctas_per_sm"  cap on resident CTAs per SM for the persistent grid; 0 = automatic
+ *   "time_kernel"  1 = bracket each tiled event-kernel launch with CUDA events on its stream; the duration of the
+ *                  last launch is then read with jpet_get_option("last_kernel_ns") (synchronises on that launch)
+ * jpet_get_option also answers "last_variant", "last_tiled", "last_smem_bytes" (what the last iteration used).
  * Returns JPET_E_INVAL for an unknown name or a value out of range. */
 int jpet_set_option(const char *name, int64_t value);
 int64_t jpet_get_option(const char *name);

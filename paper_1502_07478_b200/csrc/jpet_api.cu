@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <vector>
 
 #include "mlem_kernels.cuh"
 
@@ -20,7 +21,11 @@ using jpet::DevParams;
 thread_local std::string g_err;
 std::atomic<uint64_t> g_launches{0};
 float g_a3_coef = 2.0f;
-int64_t g_opt_replicas = 0;      // 0 = automatic
+int64_t g_opt_force_direct = 0;  // 1 = every event takes the direct (global-memory) path
+int64_t g_opt_chunk = 0;         // events per work item, 0 = automatic
+int64_t g_opt_time_kernel = 0;   // 1 = bracket the tiled event kernel with CUDA events (bench.py's roofline)
+cudaEvent_t g_tk0 = nullptr, g_tk1 = nullptr;
+bool g_tk_valid = false;
 int64_t g_opt_variant = -1;      // -1 = automatic
 int64_t g_opt_ctas_per_sm = 0;   // 0 = automatic
 constexpr int64_t kMaxBatch = 10000000;          // events per launch (BASELINE config 5: 10M-event batches)
@@ -43,25 +48,43 @@ int fail(int code, const char* fmt, ...) {
             return fail(JPET_E_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
     } while (0)
 
+// One batch of events sorted by sub-tile, with its work-item list (device memory).
+struct BinSet {
+    float* sorted = nullptr;            // [n][3], regular bins first, the direct bin last
+    jpet::WorkItem* items = nullptr;
+    int* meta = nullptr;                // 0: #items, 1: direct start, 2: direct count, 3: work counter
+    int64_t n = 0;
+    size_t cap_events = 0, cap_items = 0;
+    bool owns_sorted = true;
+};
+
 struct Workspace {
     // problem the workspace is currently set up for
     jpet_geometry geom{0, 0};
     jpet_sigmas sig{0, 0};
     jpet_grid grid{0, 0, 0};
-    float a3 = 0;
     bool s_valid = false;
     bool open = false;          // between begin and end
-    int M = 0, n_rep = 0;
+    int M = 0;
     DevParams dp{};
     int variant = 0;
+    size_t smem = 0;
     // device buffers
     float* s = nullptr;
-    float* w = nullptr;
-    float* acc = nullptr;
+    float* wT = nullptr;
+    float* accT = nullptr;
     float* rho_a = nullptr;
     float* rho_b = nullptr;
     unsigned long long* counters = nullptr;
-    size_t cap_M = 0, cap_acc = 0;
+    size_t cap_M = 0;
+    int* bin_of = nullptr;      // scratch of the binning pass
+    size_t cap_bin_of = 0;
+    int* counts = nullptr;      // [nb + 1] counts, then [nb + 1] cursors
+    size_t cap_counts = 0;
+    BinSet scratch;             // used by iterate / accumulate
+    std::vector<BinSet> kept;   // used by reconstruct: one per batch, binned once
+    float* kept_sorted = nullptr;
+    size_t cap_kept_sorted = 0;
     float* stage = nullptr;     // event staging for the host-buffer calls
     size_t cap_stage = 0;       // bytes
     cudaStream_t copy_stream = nullptr, compute_stream = nullptr;
@@ -103,83 +126,89 @@ int ensure_device() {
     return JPET_OK;
 }
 
-int ensure_images(int M, int n_rep) {
+int ensure_images(int M) {
     if ((size_t)M > g_ws.cap_M) {
-        cudaFree(g_ws.s); cudaFree(g_ws.w); cudaFree(g_ws.rho_a); cudaFree(g_ws.rho_b);
-        g_ws.s = g_ws.w = g_ws.rho_a = g_ws.rho_b = nullptr;
+        cudaFree(g_ws.s); cudaFree(g_ws.wT); cudaFree(g_ws.accT); cudaFree(g_ws.rho_a); cudaFree(g_ws.rho_b);
+        g_ws.s = g_ws.wT = g_ws.accT = g_ws.rho_a = g_ws.rho_b = nullptr;
         g_ws.cap_M = 0;
         CUDA_TRY(cudaMalloc(&g_ws.s, sizeof(float) * M));
-        CUDA_TRY(cudaMalloc(&g_ws.w, sizeof(float) * M));
+        CUDA_TRY(cudaMalloc(&g_ws.wT, sizeof(float) * M));
+        CUDA_TRY(cudaMalloc(&g_ws.accT, sizeof(float) * M));
         CUDA_TRY(cudaMalloc(&g_ws.rho_a, sizeof(float) * M));
         CUDA_TRY(cudaMalloc(&g_ws.rho_b, sizeof(float) * M));
         g_ws.cap_M = M;
         g_ws.s_valid = false;
     }
-    if ((size_t)M * n_rep > g_ws.cap_acc) {
-        cudaFree(g_ws.acc);
-        g_ws.acc = nullptr;
-        g_ws.cap_acc = 0;
-        CUDA_TRY(cudaMalloc(&g_ws.acc, sizeof(float) * (size_t)M * n_rep));
-        g_ws.cap_acc = (size_t)M * n_rep;
-    }
     if (!g_ws.counters) CUDA_TRY(cudaMalloc(&g_ws.counters, 2 * sizeof(unsigned long long)));
     return JPET_OK;
 }
 
-// ---- event-kernel variants ------------------------------------------------------------------------------
-struct Variant { int W, NW, NIT, threads; };
+// ---- event-kernel variants: NW warps per CTA, rows split in NH parts, NR row passes, NJ cached pixels,
+// HS = region row stride (compile time, so every shared-memory access has an immediate offset) ---------------
+struct Variant { int NW, NH, NR, NJ, HS; };
 constexpr Variant kVariants[] = {
-    {8, 1, 32, 256},    // 0: warp per event, 8-pixel segments, 128 cached segments
-    {16, 1, 32, 256},   // 1: warp per event, 16-pixel segments, 64 cached segments
-    {16, 4, 32, 256},   // 2: 4 warps per event, 16-pixel segments, 256 cached segments
-    {16, 8, 24, 256},   // 3: 8 warps per event, 16-pixel segments, 384 cached segments
-    {32, 4, 32, 256},   // 4: 4 warps per event, 32-pixel segments, 128 cached segments
-    {8, 2, 32, 256},    // 5: 2 warps per event, 8-pixel segments, 256 cached segments
+    {1, 1, 1, 12, 64},    // 0: <= 32 rows, chords <= 12 px                    (config 1)
+    {2, 1, 1, 20, 64},    // 1: <= 64 rows, chords <= 20 px                    (configs 2, 3)
+    {4, 2, 1, 12, 64},    // 2: <= 64 rows, chords <= 24 px in two halves
+    {4, 1, 1, 36, 128},   // 3: <= 128 rows, chords <= 36 px                   (config 4)
+    {8, 2, 1, 20, 128},   // 4: <= 128 rows, chords <= 40 px in two halves
+    {8, 2, 1, 24, 160},   // 5: <= 128 rows, chords <= 48 px in two halves     (config 5)
+    {4, 1, 1, 44, 160},   // 6: <= 128 rows, chords <= 44 px
+    {1, 1, 2, 20, 64},    // 7: <= 64 rows in two passes of one warp, chords <= 20 px
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
-template <int W, int NW, int NIT, int THREADS>
-int launch_events(const float* events, int64_t n, const DevParams& dp, const float* w, float* acc, int M, int n_rep,
-                  unsigned long long* counters, cudaStream_t stream) {
-    auto kern = jpet::mlem_events_kernel<W, NW, NIT, THREADS>;
-    constexpr int GROUPS = THREADS / (NW * 32);
-    size_t rows_bytes = (size_t)dp.nrow_max * sizeof(jpet::RowRec);
-    size_t seg_bytes = (((size_t)dp.nseg_max * 4 + 15) / 16) * 16;
-    size_t group_bytes = rows_bytes + seg_bytes + 16 * ((NW * 4 + 15) / 16);
-    size_t smem = group_bytes * GROUPS;
-    if (smem > 220 * 1024) return fail(JPET_E_INVAL, "ellipse tables (%zu B) exceed shared memory; use a wider variant", smem);
-    static size_t attr_set = 0;
-    if (smem > 48 * 1024 && smem > attr_set) {
-        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = smem;
+template <int NW, int NH, int NR, int NJ, int HS>
+int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
+    auto kern = jpet::mlem_rows_kernel<NW, NH, NR, NJ, HS>;
+    if (dp.t_max >= 0.f) {     // tiled path
+        if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
+        static size_t attr_set = 0;
+        if (smem > 48 * 1024 && smem > attr_set) {
+            CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            attr_set = smem;
+        }
+        int per_sm = 0;
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NW * 32, smem));
+        if (per_sm < 1) return fail(JPET_E_CUDA, "event kernel does not fit on an SM (%zu B of shared memory)", smem);
+        if (g_opt_ctas_per_sm > 0) per_sm = (int)std::min<int64_t>(per_sm, g_opt_ctas_per_sm);
+        int64_t max_items = bs.n / dp.chunk + (int64_t)dp.nby * dp.nbz + 1;
+        int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(max_items, 1));
+        if (g_opt_time_kernel) {
+            if (!g_tk0) { CUDA_TRY(cudaEventCreate(&g_tk0)); CUDA_TRY(cudaEventCreate(&g_tk1)); }
+            CUDA_TRY(cudaEventRecord(g_tk0, stream));
+        }
+        kern<<<grid, NW * 32, smem, stream>>>(bs.sorted, bs.items, bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.counters);
+        g_launches++;
+        if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk1, stream)); g_tk_valid = true; }
+        CUDA_TRY(cudaGetLastError());
     }
-    int per_sm = 0;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, THREADS, smem));
-    if (per_sm < 1) return fail(JPET_E_CUDA, "event kernel does not fit on an SM");
-    if (g_opt_ctas_per_sm > 0) per_sm = (int)std::min<int64_t>(per_sm, g_opt_ctas_per_sm);
-    int64_t want = (n + GROUPS - 1) / GROUPS;
-    int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(want, 1));
-    kern<<<grid, THREADS, smem, stream>>>(events, (long long)n, dp, w, acc, (long long)M, n_rep, counters);
+    // direct path for the events of the last bin (all events when no region fits shared memory)
+    int dgrid = dp.t_max >= 0.f ? g_ws.sm_count : g_ws.sm_count * 16;
+    jpet::mlem_rows_direct_kernel<<<dgrid, 128, 0, stream>>>(bs.sorted, bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.counters);
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     return JPET_OK;
 }
 
-int dispatch_events(int variant, const float* events, int64_t n, const DevParams& dp, const float* w, float* acc, int M,
-                    int n_rep, unsigned long long* counters, cudaStream_t stream) {
+int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t st) {
     switch (variant) {
-        case 0: return launch_events<8, 1, 32, 256>(events, n, dp, w, acc, M, n_rep, counters, stream);
-        case 1: return launch_events<16, 1, 32, 256>(events, n, dp, w, acc, M, n_rep, counters, stream);
-        case 2: return launch_events<16, 4, 32, 256>(events, n, dp, w, acc, M, n_rep, counters, stream);
-        case 3: return launch_events<16, 8, 24, 256>(events, n, dp, w, acc, M, n_rep, counters, stream);
-        case 4: return launch_events<32, 4, 32, 256>(events, n, dp, w, acc, M, n_rep, counters, stream);
-        case 5: return launch_events<8, 2, 32, 256>(events, n, dp, w, acc, M, n_rep, counters, stream);
+        case 0: return launch_rows<1, 1, 1, 12, 64>(bs, dp, smem, st);
+        case 1: return launch_rows<2, 1, 1, 20, 64>(bs, dp, smem, st);
+        case 2: return launch_rows<4, 2, 1, 12, 64>(bs, dp, smem, st);
+        case 3: return launch_rows<4, 1, 1, 36, 128>(bs, dp, smem, st);
+        case 4: return launch_rows<8, 2, 1, 20, 128>(bs, dp, smem, st);
+        case 5: return launch_rows<8, 2, 1, 24, 160>(bs, dp, smem, st);
+        case 6: return launch_rows<4, 1, 1, 44, 160>(bs, dp, smem, st);
+        case 7: return launch_rows<1, 1, 2, 20, 64>(bs, dp, smem, st);
         default: return fail(JPET_E_INVAL, "unknown kernel variant %d", variant);
     }
 }
 
-// Constants of the event kernel, computed in double and rounded once.
-void make_params(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& gr, float a3, int W, DevParams* out) {
+// Constants of the event kernel (computed in double, rounded once), the tiling of the image into
+// sub-tiles + halo regions, and the kernel variant.
+void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& gr, float a3, DevParams* out, int* variant,
+               size_t* smem_out) {
     DevParams p{};
     const double LH = 0.72134752044448170368;
     double iz2 = 1.0 / ((double)sg.sigma_z * sg.sigma_z), il2 = 1.0 / ((double)sg.sigma_dl * sg.sigma_dl);
@@ -191,35 +220,57 @@ void make_params(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid&
     p.hy_coef = (float)(1.5 * sg.sigma_dl);
     p.half_sz2 = (float)(0.5 * (double)sg.sigma_z * sg.sigma_z);
     p.c1s = (float)(-LH * 2.0 * iz2);
+    p.sq = (float)std::sqrt(LH * 2.0 * iz2);
+    p.inv_sq = (float)(1.0 / std::sqrt(LH * 2.0 * iz2));
     p.c2k = (float)(4.0 * il2);
     p.ak = (float)(-2.0 * iz2);
     p.bk = (float)(2.0 * a3 * il2);
     p.d1k = (float)(2.0 * iz2);
     p.d2k = (float)((double)a3 * a3 * il2);
     p.d3k = (float)(4.0 * il2);
-    // capacities: rows <= 3 sigma_dl / px + 1; pixels <= area/px^2 + longest chord/px + rows (Riemann-sum bound)
-    double rows = std::floor(3.0 * sg.sigma_dl / px) + 3.0;
-    double chord = 2.0 * 3.0 * sg.sigma_z / std::sqrt(2.0) / px + 2.0;
-    double area = 9.0 * M_PI * sg.sigma_z * sg.sigma_dl / (2.0 * std::sqrt(2.0)) / (px * px);
-    rows = std::min(rows, (double)gr.n_y);
-    double pix = area + chord + rows;
-    p.nrow_max = (int)rows;
-    p.nseg_max = (int)(pix / W + rows) + 8;
+    // ellipse extents in pixels: half height 1.5 sigma_dl cos(theta), half width 3 sqrt(sz^2/2 + sdl^2 sin^2/4) (App. B)
+    double t_max = ((double)g.L + 8.0 * sg.sigma_z) / (2.0 * g.R);
+    double sin2 = t_max * t_max / (1.0 + t_max * t_max);
+    double hy = 1.5 * sg.sigma_dl / px;
+    double hz = 3.0 * std::sqrt(0.5 * (double)sg.sigma_z * sg.sigma_z + 0.25 * (double)sg.sigma_dl * sg.sigma_dl * sin2) / px;
+    double chord = 6.0 * sg.sigma_z / std::sqrt(2.0) / px;
+    int rows_max = std::min<int>(gr.n_y, (int)std::floor(2.0 * hy) + 2);
+    int chord_max = std::min<int>(gr.n_z, (int)std::floor(chord) + 2);
+    p.Hy = (int)std::ceil(hy) + 1;
+    p.Hz = (int)std::ceil(hz) + 1;
+    p.t_max = (float)t_max;
+    // variant: smallest shape that holds rows_max rows, chord_max pixels per row, and the region's rows
+    auto fits = [&](const Variant& c) {
+        return rows_max <= c.NW * 32 / c.NH * c.NR && chord_max <= c.NJ * c.NH && 2 * p.Hy + 4 <= c.HS;
+    };
+    int v = -1;
+    if (g_opt_variant >= 0) v = (int)g_opt_variant;
+    else {
+        const int order[] = {0, 1, 3, 5};
+        for (int cand : order)
+            if (fits(kVariants[cand])) { v = cand; break; }
+        if (v < 0) v = 5;
+    }
+    const bool tiles_ok = 2 * p.Hy + 4 <= kVariants[v].HS;     // else: every event takes the direct path
+    p.HS = kVariants[v].HS;
+    p.Sy = std::max(1, p.HS - 2 * p.Hy);
+    p.Sz = 16;
+    // shared memory: w region + accumulator region; shrink the sub-tile width, then give up tiling
+    const size_t budget = 200 * 1024;
+    size_t smem = 0;
+    for (;;) {
+        p.WZ = p.Sz + 2 * p.Hz;
+        smem = 2 * sizeof(float) * (size_t)p.HS * p.WZ;
+        if (smem <= budget / 2 || p.Sz <= 4) break;
+        p.Sz /= 2;
+    }
+    if (smem > budget || !tiles_ok || p.WZ < kVariants[v].NJ + 4 || g_opt_force_direct) { p.t_max = -1.f; smem = 0; }
+    p.nby = (gr.n_y + 2 * p.Hy + p.Sy - 1) / p.Sy;
+    p.nbz = (gr.n_z + 2 * p.Hz + p.Sz - 1) / p.Sz;
+    p.chunk = g_opt_chunk > 0 ? (int)g_opt_chunk : 128;
     *out = p;
-}
-
-int choose_variant(const jpet_sigmas& sg, const jpet_grid& gr) {
-    if (g_opt_variant >= 0) return (int)g_opt_variant;
-    double area = 9.0 * M_PI * sg.sigma_z * sg.sigma_dl / (2.0 * std::sqrt(2.0)) / ((double)gr.pixel * gr.pixel);
-    if (area <= 900.0) return 0;
-    if (area <= 3000.0) return 2;
-    return 3;
-}
-
-int choose_replicas(int M) {
-    if (g_opt_replicas > 0) return (int)g_opt_replicas;
-    (void)M;
-    return 8;
+    *variant = v;
+    *smem_out = smem;
 }
 
 bool same_problem(const jpet_geometry& g, const jpet_grid& gr) {
@@ -227,7 +278,75 @@ bool same_problem(const jpet_geometry& g, const jpet_grid& gr) {
            g_ws.grid.n_z == gr.n_z && g_ws.grid.pixel == gr.pixel;
 }
 
-int grid_for(int M) { return (M + 255) / 256; }
+int grid_for(int64_t M) { return (int)((M + 255) / 256); }
+
+int ensure_binset(BinSet& bs, int64_t n, const DevParams& dp, bool need_sorted) {
+    size_t items_cap = (size_t)(n / dp.chunk) + (size_t)dp.nby * dp.nbz + 2;
+    if (need_sorted && (size_t)n > bs.cap_events) {
+        if (bs.owns_sorted) cudaFree(bs.sorted);
+        bs.sorted = nullptr; bs.cap_events = 0;
+        CUDA_TRY(cudaMalloc(&bs.sorted, sizeof(float) * 3 * (size_t)std::max<int64_t>(n, 1)));
+        bs.cap_events = (size_t)n;
+        bs.owns_sorted = true;
+    }
+    if (items_cap > bs.cap_items) {
+        cudaFree(bs.items);
+        bs.items = nullptr; bs.cap_items = 0;
+        CUDA_TRY(cudaMalloc(&bs.items, sizeof(jpet::WorkItem) * items_cap));
+        bs.cap_items = items_cap;
+    }
+    if (!bs.meta) CUDA_TRY(cudaMalloc(&bs.meta, 4 * sizeof(int)));
+    return JPET_OK;
+}
+
+void free_binset(BinSet& bs) {
+    if (bs.owns_sorted) cudaFree(bs.sorted);
+    cudaFree(bs.items);
+    cudaFree(bs.meta);
+    bs = BinSet{};
+}
+
+// Counting sort of one batch (<= kMaxBatch events) by sub-tile into bs.sorted, and its work items.
+int bin_batch(const float* events, int64_t n, BinSet& bs, const DevParams& dp, cudaStream_t st) {
+    const int nb = dp.nby * dp.nbz;
+    if ((size_t)n > g_ws.cap_bin_of) {
+        cudaFree(g_ws.bin_of);
+        g_ws.bin_of = nullptr; g_ws.cap_bin_of = 0;
+        CUDA_TRY(cudaMalloc(&g_ws.bin_of, sizeof(int) * (size_t)n));
+        g_ws.cap_bin_of = (size_t)n;
+    }
+    if ((size_t)(2 * (nb + 1)) > g_ws.cap_counts) {
+        cudaFree(g_ws.counts);
+        g_ws.counts = nullptr; g_ws.cap_counts = 0;
+        CUDA_TRY(cudaMalloc(&g_ws.counts, sizeof(int) * 2 * (size_t)(nb + 1)));
+        g_ws.cap_counts = (size_t)(2 * (nb + 1));
+    }
+    int* counts = g_ws.counts;
+    int* cursors = g_ws.counts + (nb + 1);
+    CUDA_TRY(cudaMemsetAsync(counts, 0, sizeof(int) * (nb + 1), st));
+    const int per_block = jpet::kBinBlock * jpet::kBinPer;
+    const int blocks = (int)((n + per_block - 1) / per_block);
+    const int use_smem = nb + 1 <= jpet::kBinSmemMax;
+    const size_t hist_bytes = use_smem ? sizeof(int) * (size_t)(nb + 1) : 0;
+    if (n > 0) {
+        jpet::bin_count_kernel<<<blocks, jpet::kBinBlock, hist_bytes, st>>>(events, (int)n, dp, g_ws.bin_of, counts, nb + 1, use_smem);
+        g_launches++;
+    }
+    jpet::bin_scan_kernel<<<1, 1024, 0, st>>>(counts, cursors, bs.items, bs.meta, nb, dp.chunk);
+    g_launches++;
+    if (n > 0) {
+        jpet::bin_scatter_kernel<<<blocks, jpet::kBinBlock, hist_bytes, st>>>(events, (int)n, g_ws.bin_of, cursors, bs.sorted, nb + 1, use_smem);
+        g_launches++;
+    }
+    CUDA_TRY(cudaGetLastError());
+    bs.n = n;
+    return JPET_OK;
+}
+
+int run_binset(BinSet& bs, cudaStream_t st) {
+    CUDA_TRY(cudaMemsetAsync(bs.meta + 3, 0, sizeof(int), st));      // work counter
+    return dispatch_rows(g_ws.variant, bs, g_ws.dp, g_ws.smem, st);
+}
 
 int do_begin(const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr, const float* rho_in, cudaStream_t st) {
     int rc = validate(g, sg, gr);
@@ -236,19 +355,17 @@ int do_begin(const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr,
     if (!rho_in) return fail(JPET_E_INVAL, "NULL rho_in");
     if ((rc = ensure_device())) return rc;
     const int M = gr->n_y * gr->n_z;
-    const int n_rep = choose_replicas(M);
-    if ((rc = ensure_images(M, n_rep))) return rc;
+    if ((rc = ensure_images(M))) return rc;
     if (!same_problem(*g, *gr)) {
         jpet::sensitivity_kernel<<<grid_for(M), 256, 0, st>>>(g_ws.s, gr->n_y, gr->n_z, gr->pixel, g->R, g->L);
         g_launches++;
         CUDA_TRY(cudaGetLastError());
         g_ws.geom = *g; g_ws.grid = *gr; g_ws.s_valid = true;
     }
-    g_ws.sig = *sg; g_ws.a3 = g_a3_coef; g_ws.M = M; g_ws.n_rep = n_rep;
-    g_ws.variant = choose_variant(*sg, *gr);
+    g_ws.sig = *sg; g_ws.M = M;
+    make_plan(*g, *sg, *gr, g_a3_coef, &g_ws.dp, &g_ws.variant, &g_ws.smem);
     if (g_ws.variant < 0 || g_ws.variant >= kNumVariants) return fail(JPET_E_INVAL, "unknown kernel variant");
-    make_params(*g, *sg, *gr, g_a3_coef, kVariants[g_ws.variant].W, &g_ws.dp);
-    jpet::prepass_kernel<<<grid_for(M), 256, 0, st>>>(g_ws.s, rho_in, g_ws.w, g_ws.acc, M, n_rep, g_ws.counters);
+    jpet::prepass_kernel<<<grid_for(M), 256, 0, st>>>(g_ws.s, rho_in, g_ws.wT, g_ws.accT, gr->n_y, gr->n_z, g_ws.counters);
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     g_ws.open = true;
@@ -261,9 +378,10 @@ int do_accumulate(const float* events, int64_t n, cudaStream_t st) {
     if (n > 0 && !events) return fail(JPET_E_INVAL, "NULL events");
     for (int64_t off = 0; off < n; off += kMaxBatch) {
         int64_t nb = std::min(kMaxBatch, n - off);
-        int rc = dispatch_events(g_ws.variant, events + 3 * off, nb, g_ws.dp, g_ws.w, g_ws.acc, g_ws.M, g_ws.n_rep,
-                                 g_ws.counters, st);
+        int rc = ensure_binset(g_ws.scratch, nb, g_ws.dp, true);
         if (rc) return rc;
+        if ((rc = bin_batch(events + 3 * off, nb, g_ws.scratch, g_ws.dp, st))) return rc;
+        if ((rc = run_binset(g_ws.scratch, st))) return rc;
     }
     return JPET_OK;
 }
@@ -271,10 +389,53 @@ int do_accumulate(const float* events, int64_t n, cudaStream_t st) {
 int do_end(const float* rho_in, float* rho_out, cudaStream_t st) {
     if (!g_ws.open) return fail(JPET_E_INVAL, "jpet_mlem_end without jpet_mlem_begin");
     if (!rho_in || !rho_out) return fail(JPET_E_INVAL, "NULL image pointer");
-    jpet::finalise_kernel<<<grid_for(g_ws.M), 256, 0, st>>>(g_ws.s, rho_in, g_ws.acc, rho_out, g_ws.M, g_ws.n_rep);
+    jpet::finalise_kernel<<<grid_for(g_ws.M), 256, 0, st>>>(g_ws.s, rho_in, g_ws.accT, rho_out, g_ws.grid.n_y, g_ws.grid.n_z);
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     g_ws.open = false;
+    return JPET_OK;
+}
+
+// n_iter iterations over device-resident events; the events are binned once (first iteration) and the
+// sorted copy is reused by the others (events never change between iterations).
+int iterate_many(const float* events, int64_t n, const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr,
+                 const float* rho_start, float* rho_out, int n_iter, cudaStream_t st) {
+    const int M = gr->n_y * gr->n_z;
+    const float* cur = rho_start;
+    const int64_t n_batches = (n + kMaxBatch - 1) / kMaxBatch;
+    const bool keep = n_iter > 1;
+    if (keep) {
+        if ((size_t)n > g_ws.cap_kept_sorted) {
+            cudaFree(g_ws.kept_sorted);
+            g_ws.kept_sorted = nullptr; g_ws.cap_kept_sorted = 0;
+            CUDA_TRY(cudaMalloc(&g_ws.kept_sorted, sizeof(float) * 3 * (size_t)n));
+            g_ws.cap_kept_sorted = (size_t)n;
+        }
+        while ((int64_t)g_ws.kept.size() < n_batches) g_ws.kept.emplace_back();
+    }
+    for (int it = 0; it < n_iter; ++it) {
+        float* nxt = (it == n_iter - 1) ? rho_out : (cur == g_ws.rho_a ? g_ws.rho_b : g_ws.rho_a);
+        int rc = do_begin(g, sg, gr, cur, st);
+        if (rc) return rc;
+        if (!keep) {
+            if ((rc = do_accumulate(events, n, st))) { g_ws.open = false; return rc; }
+        } else {
+            for (int64_t b = 0; b < n_batches; ++b) {
+                BinSet& bs = g_ws.kept[b];
+                int64_t off = b * kMaxBatch, nb = std::min(kMaxBatch, n - off);
+                if (it == 0) {
+                    bs.owns_sorted = false;
+                    bs.sorted = g_ws.kept_sorted + 3 * off;
+                    if ((rc = ensure_binset(bs, nb, g_ws.dp, false))) return rc;
+                    if ((rc = bin_batch(events + 3 * off, nb, bs, g_ws.dp, st))) return rc;
+                }
+                if ((rc = run_binset(bs, st))) { g_ws.open = false; return rc; }
+            }
+        }
+        if ((rc = do_end(cur, nxt, st))) return rc;
+        cur = nxt;
+    }
+    (void)M;
     return JPET_OK;
 }
 
@@ -329,7 +490,7 @@ int reconstruct_host_impl(const float* events_host, int64_t n, const jpet_geomet
     if ((n > 0 && !events_host) || !rho_out_host) return fail(JPET_E_INVAL, "NULL host pointer");
     if ((rc = ensure_device())) return rc;
     const int M = gr->n_y * gr->n_z;
-    if ((rc = ensure_images(M, choose_replicas(M)))) return rc;
+    if ((rc = ensure_images(M))) return rc;
     if (chunk <= 0) chunk = 2000000;
     chunk = std::min<int64_t>(chunk, std::max<int64_t>(n, 1));
     const bool fits = (int64_t)sizeof(float) * 3 * n <= kStageBytes;
@@ -345,11 +506,25 @@ int reconstruct_host_impl(const float* events_host, int64_t n, const jpet_geomet
         g_launches++;
         CUDA_TRY(cudaGetLastError());
     }
-    for (int it = 0; it < n_iter; ++it) {
+    if (n_iter > 0) {
+        // first iteration: the upload of chunk c+1 overlaps the binning + event kernels of chunk c
         if ((rc = do_begin(g, sg, gr, cur, ks))) return rc;
-        if ((rc = accumulate_from_host(events_host, n, chunk, fits, fits && it > 0))) return rc;
+        if ((rc = accumulate_from_host(events_host, n, chunk, fits, false))) return rc;
         if ((rc = do_end(cur, nxt, ks))) return rc;
         std::swap(cur, nxt);
+        if (n_iter > 1) {
+            if (fits) {         // events are now resident in the staging buffer: bin once, iterate
+                if ((rc = iterate_many(g_ws.stage, n, g, sg, gr, cur, nxt, n_iter - 1, ks))) return rc;
+                std::swap(cur, nxt);
+            } else {
+                for (int it = 1; it < n_iter; ++it) {
+                    if ((rc = do_begin(g, sg, gr, cur, ks))) return rc;
+                    if ((rc = accumulate_from_host(events_host, n, chunk, false, false))) return rc;
+                    if ((rc = do_end(cur, nxt, ks))) return rc;
+                    std::swap(cur, nxt);
+                }
+            }
+        }
     }
     CUDA_TRY(cudaMemcpyAsync(rho_out_host, cur, sizeof(float) * M, cudaMemcpyDeviceToHost, ks));
     CUDA_TRY(cudaStreamSynchronize(ks));
@@ -417,7 +592,7 @@ int jpet_reconstruct(const float* events_dev, int64_t n, const jpet_geometry* ge
     if ((rc = ensure_device())) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int M = grid->n_y * grid->n_z;
-    if ((rc = ensure_images(M, choose_replicas(M)))) return rc;
+    if ((rc = ensure_images(M))) return rc;
     // ping-pong through the workspace so that rho_out may alias rho_init and is written once per iteration
     const float* cur = rho_init_dev;
     if (!cur) {
@@ -430,14 +605,7 @@ int jpet_reconstruct(const float* events_dev, int64_t n, const jpet_geometry* ge
         if (cur != rho_out_dev) CUDA_TRY(cudaMemcpyAsync(rho_out_dev, cur, sizeof(float) * M, cudaMemcpyDeviceToDevice, st));
         return JPET_OK;
     }
-    for (int it = 0; it < n_iter; ++it) {
-        float* nxt = (it == n_iter - 1) ? rho_out_dev : (cur == g_ws.rho_a ? g_ws.rho_b : g_ws.rho_a);
-        if ((rc = do_begin(geometry, sigmas, grid, cur, st))) return rc;
-        if ((rc = do_accumulate(events_dev, n, st))) { g_ws.open = false; return rc; }
-        if ((rc = do_end(cur, nxt, st))) return rc;
-        cur = nxt;
-    }
-    return JPET_OK;
+    return iterate_many(events_dev, n, geometry, sigmas, grid, cur, rho_out_dev, n_iter, st);
 }
 
 int jpet_mlem_iterate_host(const float* events_host, int64_t n, const jpet_geometry* geometry, const jpet_sigmas* sigmas,
@@ -478,8 +646,9 @@ int jpet_count_evals(const float* events_dev, int64_t n, const jpet_geometry* ge
     CUDA_TRY(cudaMalloc(&d, 2 * sizeof(unsigned long long)));
     CUDA_TRY(cudaMemsetAsync(d, 0, 2 * sizeof(unsigned long long), st));
     DevParams dp;
-    make_params(*geometry, *sigmas, *grid, g_a3_coef, 8, &dp);
-    dp.nrow_max = grid->n_y;
+    int variant = 0;
+    size_t smem = 0;
+    make_plan(*geometry, *sigmas, *grid, g_a3_coef, &dp, &variant, &smem);
     if (n > 0) {
         int blocks = (int)std::min<int64_t>((n + 255) / 256, (int64_t)g_ws.sm_count * 8);
         jpet::count_evals_kernel<<<blocks, 256, 0, st>>>(events_dev, (long long)n, dp, d);
@@ -507,9 +676,16 @@ float jpet_get_a3_coef(void) { return g_a3_coef; }
 int jpet_set_option(const char* name, int64_t value) {
     g_err.clear();
     if (!name) return fail(JPET_E_INVAL, "NULL option name");
-    if (!strcmp(name, "replicas")) {
-        if (value < 0 || value > 64) return fail(JPET_E_INVAL, "replicas must be 0 (auto) .. 64");
-        g_opt_replicas = value;
+    if (!strcmp(name, "force_direct")) {
+        if (value < 0 || value > 1) return fail(JPET_E_INVAL, "force_direct must be 0 or 1");
+        g_opt_force_direct = value;
+    } else if (!strcmp(name, "time_kernel")) {
+        if (value < 0 || value > 1) return fail(JPET_E_INVAL, "time_kernel must be 0 or 1");
+        g_opt_time_kernel = value;
+        g_tk_valid = false;
+    } else if (!strcmp(name, "chunk")) {
+        if (value < 0 || value > (1 << 20)) return fail(JPET_E_INVAL, "chunk must be 0 (auto) .. 2^20");
+        g_opt_chunk = value;
     } else if (!strcmp(name, "variant")) {
         if (value < -1 || value >= kNumVariants) return fail(JPET_E_INVAL, "variant must be -1 (auto) .. %d", kNumVariants - 1);
         g_opt_variant = value;
@@ -524,19 +700,30 @@ int jpet_set_option(const char* name, int64_t value) {
 
 int64_t jpet_get_option(const char* name) {
     if (!name) return -1;
-    if (!strcmp(name, "replicas")) return g_opt_replicas;
+    if (!strcmp(name, "force_direct")) return g_opt_force_direct;
+    if (!strcmp(name, "chunk")) return g_opt_chunk;
+    if (!strcmp(name, "time_kernel")) return g_opt_time_kernel;
+    if (!strcmp(name, "last_kernel_ns")) {      // duration of the last tiled event-kernel launch (synchronises on it)
+        if (!g_tk_valid || cudaEventSynchronize(g_tk1) != cudaSuccess) return -1;
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, g_tk0, g_tk1) != cudaSuccess) return -1;
+        return (int64_t)((double)ms * 1e6);
+    }
     if (!strcmp(name, "variant")) return g_opt_variant;
     if (!strcmp(name, "ctas_per_sm")) return g_opt_ctas_per_sm;
     if (!strcmp(name, "last_variant")) return g_ws.variant;
-    if (!strcmp(name, "last_replicas")) return g_ws.n_rep;
+    if (!strcmp(name, "last_smem_bytes")) return (int64_t)g_ws.smem;
+    if (!strcmp(name, "last_tiled")) return g_ws.dp.t_max >= 0.f;
     return -1;
 }
 
 uint64_t jpet_launch_count(void) { return g_launches.load(); }
 
 void jpet_release(void) {
-    cudaFree(g_ws.s); cudaFree(g_ws.w); cudaFree(g_ws.acc); cudaFree(g_ws.rho_a); cudaFree(g_ws.rho_b);
-    cudaFree(g_ws.counters); cudaFree(g_ws.stage);
+    cudaFree(g_ws.s); cudaFree(g_ws.wT); cudaFree(g_ws.accT); cudaFree(g_ws.rho_a); cudaFree(g_ws.rho_b);
+    cudaFree(g_ws.counters); cudaFree(g_ws.stage); cudaFree(g_ws.bin_of); cudaFree(g_ws.counts); cudaFree(g_ws.kept_sorted);
+    free_binset(g_ws.scratch);
+    for (auto& bs : g_ws.kept) free_binset(bs);
     for (int i = 0; i < 2; ++i) {
         if (g_ws.ev_copy[i]) cudaEventDestroy(g_ws.ev_copy[i]);
         if (g_ws.ev_done[i]) cudaEventDestroy(g_ws.ev_done[i]);

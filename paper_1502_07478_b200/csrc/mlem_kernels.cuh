@@ -4,13 +4,15 @@
 //
 // Kernels
 //   sensitivity_kernel    s(y,z) of Eq. 4, evaluated in fp64, rounded once to fp32, clamped >= 0
-//   prepass_kernel        w = s * rho_in (the s(i) rho(i) factor of Eq. 3's denominator);
-//                         zeroes the accumulator replicas
-//   mlem_events_kernel    steps 1-3: Eq. 2, 3-sigma ellipse rows (App. B
-//                         :251-267), kernel of Eq. 7-12, denominator, scatter
-//   finalise_kernel       acc = sum of replicas; rho_out = rho_in * acc where s > 0 else 0 (Eq. 3)
+//   prepass_kernel        wT = s * rho_in, stored TRANSPOSED (y fastest) - the s(i) rho(i) factor of Eq. 3's
+//                         denominator; zeroes the transposed accumulator
+//   bin_*_kernel          counting sort of the events by the image sub-tile their reconstructed point
+//                         (y~, z~) of Eq. 2 falls in, and the work-item list (sub-tile, chunk of events)
+//   mlem_rows_kernel      steps 1-3: Eq. 2, 3-sigma ellipse rows (App. B
+//                         :251-267), kernel of Eq. 7-12, denominator, back-projection
+//   finalise_kernel       rho_out = rho_in * acc where s > 0 else 0 (Eq. 3)
 //
-// Algebra used by mlem_events_kernel (diagonal C^-1 = diag(iz2, iz2, il2), iz2 = 1/sigma_z^2,
+// Algebra used by mlem_rows_kernel (diagonal C^-1 = diag(iz2, iz2, il2), iz2 = 1/sigma_z^2,
 // il2 = 1/sigma_dl^2; t = tan theta~, sec2 = 1 + t^2; pixel centre (y, z); dy = y - y~, dz = z - z~;
 // u = dz - t dy; k = a3 coefficient).  With o, a, b of Eq. 8-10 written out, the four quadratic forms are
 //   b.C^-1.b = 2 iz2 u^2 + 4 il2 sec2 dy^2                                              (B.3)
@@ -27,9 +29,23 @@
 // Row r of the ellipse is the closed interval |u| <= sqrt((9 - c2)/c1) (B.3 solved for dz), so pixels are
 // enumerated by row spans and no lane is spent on a failed ellipse test (the paper's bbox + test wastes
 // about one third of the lanes).
+//
+// Schedule of mlem_rows_kernel (B200 design, not the paper's warp-per-event/texture scheme):
+//   * one CTA (NW warps) works on one event at a time; THREAD <-> ELLIPSE ROW (optionally a 1/NH part of a
+//     row), so the row constants live in registers and the inner loop walks the row's pixels with no
+//     table look-ups; the P values of the walk stay in registers for the back-projection pass;
+//   * events are pre-sorted by image sub-tile; a CTA takes a work item (sub-tile, chunk of events), stages
+//     the w = s*rho region (sub-tile + halo) in shared memory, accumulates P/denominator into a PRIVATE
+//     shared-memory region with plain (non-atomic) read-modify-writes, and flushes the region once with
+//     red.global.add.f32.  Measured on B200: global red.add tops out at ~2.8e10 warp requests/s, a factor 5-10
+//     below what the SFU/FP32 pipes can produce, so the scatter has to stay on chip;
+//   * regions are stored transposed (y fastest, row stride HS a multiple of 32): lanes are consecutive
+//     image rows, so every shared-memory access of a warp is bank-conflict free whatever the ellipse tilt.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+
+#include <type_traits>
 
 namespace jpet {
 
@@ -42,15 +58,23 @@ struct DevParams {
     float hy_coef;                     // 1.5 sigma_dl: half-height of the ellipse is hy_coef * cos(theta~)
     float half_sz2;                    // sigma_z^2 / 2 = 1 / c1
     float c1s;                         // -LH * 2 iz2
+    float sq, inv_sq;                  // sqrt(-c1s) and its inverse (u is rescaled so the Gaussian term is -u'^2)
     float c2k;                         // 4 il2          (c2 = c2k * sec2 * dy^2)
     float ak;                          // -2 iz2         (alpha = ak sec2 y)
     float bk;                          // 2 k il2        (beta = bk sec2 t y dy)
     float d1k;                         // 2 iz2          (delta term sec2^2 (y^2 + R^2))
     float d2k;                         // k^2 il2        (delta term sec2 t^2 y^2)
     float d3k;                         // 4 il2          (delta term sec2 (1 + 2 t^2) y dy)
-    // table capacities (per event group)
-    int nrow_max, nseg_max;
+    // binning and shared-memory regions (pixel units)
+    int Hy, Hz;                        // halo on each side of a sub-tile
+    int Sy, Sz;                        // sub-tile size
+    int HS, WZ;                        // region: HS rows (y, fastest, multiple of 32) x WZ columns (z)
+    int nby, nbz;                      // bins cover pixel indices [-Hy, n_y + Hy) x [-Hz, n_z + Hz)
+    float t_max;                       // events with |tan theta~| above this go to the direct (global) path
+    int chunk;                         // events per work item
 };
+
+struct WorkItem { int bin, start, count; };
 
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;
@@ -64,9 +88,6 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
 }
 __device__ __forceinline__ void red_add_f32(float* addr, float v) {
     asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
-}
-__device__ __forceinline__ void group_barrier(int id, int nthreads) {
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
 constexpr float kLH = 0.72134752044448170368f;       // log2(e) / 2
@@ -85,23 +106,25 @@ __global__ void sensitivity_kernel(float* __restrict__ s, int n_y, int n_z, doub
     s[i] = v > 0.0 ? (float)v : 0.f;
 }
 
-__global__ void prepass_kernel(const float* __restrict__ s, const float* __restrict__ rho_in, float* __restrict__ w,
-                               float* __restrict__ acc, int M, int n_rep, unsigned long long* __restrict__ counters) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < M) {
-        w[i] = s[i] * rho_in[i];
-        for (int r = 0; r < n_rep; ++r) acc[(size_t)r * M + i] = 0.f;
+// wT[iz * n_y + iy] = s[iy * n_z + iz] * rho_in[...]; accT = 0; counters = 0
+__global__ void prepass_kernel(const float* __restrict__ s, const float* __restrict__ rho_in, float* __restrict__ wT,
+                               float* __restrict__ accT, int n_y, int n_z, unsigned long long* __restrict__ counters) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;   // transposed index: consecutive threads = consecutive iy
+    if (i < n_y * n_z) {
+        int iz = i / n_y, iy = i - iz * n_y;
+        int src = iy * n_z + iz;
+        wT[i] = s[src] * rho_in[src];
+        accT[i] = 0.f;
     }
     if (i < 2) counters[i] = 0ull;
 }
 
-__global__ void finalise_kernel(const float* __restrict__ s, const float* rho_in, const float* __restrict__ acc,
-                                float* rho_out, int M, int n_rep) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= M) return;
-    float a = 0.f;
-    for (int r = 0; r < n_rep; ++r) a += acc[(size_t)r * M + i];
-    rho_out[i] = s[i] > 0.f ? rho_in[i] * a : 0.f;
+__global__ void finalise_kernel(const float* __restrict__ s, const float* rho_in, const float* __restrict__ accT,
+                                float* rho_out, int n_y, int n_z) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;   // row-major index
+    if (i >= n_y * n_z) return;
+    int iy = i / n_z, iz = i - iy * n_z;
+    rho_out[i] = s[i] > 0.f ? rho_in[i] * accT[iz * n_y + iy] : 0.f;
 }
 
 __global__ void ones_kernel(float* x, int M) {
@@ -110,24 +133,14 @@ __global__ void ones_kernel(float* x, int M) {
 }
 
 // ------------------------------------------------------------------------------------------------------
-// Per-row record of the current event (shared memory, one table per event group).
-struct __align__(16) RowRec {
-    float u0;      // u at the first pixel of the row
-    float c2s;     // -LH * c2
-    float betas;   // sqrt(LH) * beta
-    float delta;
-    float alphas;  // sqrt(LH) * alpha
-    float eps;
-    int base;      // linear pixel index of the first pixel of the row
-    int len;       // pixels in the row
-};
-
 struct EventConsts {
     float t, sec2, y_t, z_t;
-    int iy_lo, nrows;   // nrows == 0: event skipped
+    float fy;           // y~ in pixel units (row index, fractional)
+    float hy_px;        // half height of the ellipse in pixels
+    bool finite;
 };
 
-// Eq. 2 and the row range of the 3-sigma ellipse.
+// Eq. 2.
 __device__ __forceinline__ EventConsts event_setup(float zu, float zd, float dl, const DevParams& p) {
     EventConsts e;
     e.t = (zu - zd) * p.inv2R;                      // tan theta~
@@ -135,33 +148,55 @@ __device__ __forceinline__ EventConsts event_setup(float zu, float zd, float dl,
     float cos_t = rsqrtf(e.sec2);
     e.y_t = -0.5f * dl * cos_t;                     // y~
     e.z_t = fmaf(e.y_t, e.t, 0.5f * (zu + zd));     // z~
-    float hy = p.hy_coef * cos_t;                   // 3 sigma_y, sigma_y = sigma_dl cos(theta~) / 2
-    float flo = (e.y_t - hy - p.y0) * p.inv_px;
-    float fhi = (e.y_t + hy - p.y0) * p.inv_px;
-    bool finite = (fabsf(zu) < 1e30f) && (fabsf(zd) < 1e30f) && (fabsf(dl) < 1e30f);   // false for NaN too
-    flo = fminf(fmaxf(flo, -1.f), (float)p.n_y);
-    fhi = fminf(fmaxf(fhi, -1.f), (float)p.n_y);
-    int lo = max(0, __float2int_ru(flo));
-    int hi = min(p.n_y - 1, __float2int_rd(fhi));
-    e.iy_lo = lo;
-    e.nrows = finite ? max(0, hi - lo + 1) : 0;
-    e.nrows = min(e.nrows, p.nrow_max);
+    e.fy = (e.y_t - p.y0) * p.inv_px;
+    e.hy_px = p.hy_coef * cos_t * p.inv_px;         // 3 sigma_y / pixel, sigma_y = sigma_dl cos(theta~) / 2
+    e.finite = (fabsf(zu) < 1e30f) && (fabsf(zd) < 1e30f) && (fabsf(dl) < 1e30f);   // false for NaN too
     return e;
 }
 
-__device__ __forceinline__ RowRec row_setup(const EventConsts& e, int iy, const DevParams& p) {
-    RowRec r;
+// Rows of the ellipse clipped to [row_lo, row_hi]: returns first row and count.
+__device__ __forceinline__ void event_rows(const EventConsts& e, int row_lo, int row_hi, int& iy_lo, int& nrows) {
+    float flo = fminf(fmaxf(e.fy - e.hy_px, -2.0e6f), 2.0e6f);
+    float fhi = fminf(fmaxf(e.fy + e.hy_px, -2.0e6f), 2.0e6f);
+    int lo = max(row_lo, __float2int_ru(flo));
+    int hi = min(row_hi, __float2int_rd(fhi));
+    iy_lo = lo;
+    nrows = e.finite ? max(0, hi - lo + 1) : 0;
+}
+
+struct RowConsts {
+    float u0;      // u at the first pixel of this thread's part of the row
+    float c2s;     // -LH * c2
+    float betas;   // sqrt(LH) * beta
+    float delta;
+    float alphas;  // sqrt(LH) * alpha
+    float eps;
+    int lo;        // first column of the part
+    int len;       // pixels in the part
+};
+
+// Row constants and the span of row iy, clipped to columns [col_lo, col_hi]; part h of NH equal parts.
+template <int NH>
+__device__ __forceinline__ RowConsts row_setup(const EventConsts& e, int iy, int h, int col_lo, int col_hi,
+                                               const DevParams& p) {
+    RowConsts r;
     float y = fmaf((float)iy, p.px, p.y0);
     float dy = y - e.y_t;
     float c2 = p.c2k * e.sec2 * dy * dy;
     float rem = 9.f - c2;                                  // row chord: c1 u^2 <= 9 - c2
     float hw = sqrtf(fmaxf(rem, 0.f) * p.half_sz2);
     float zc = fmaf(e.t, dy, e.z_t);                       // u = 0 on the line z = z~ + t dy
-    float flo = fminf(fmaxf((zc - hw - p.z0) * p.inv_px, -1.f), (float)p.n_z);
-    float fhi = fminf(fmaxf((zc + hw - p.z0) * p.inv_px, -1.f), (float)p.n_z);
-    int lo = max(0, __float2int_ru(flo));
-    int hi = min(p.n_z - 1, __float2int_rd(fhi));
+    float flo = fminf(fmaxf((zc - hw - p.z0) * p.inv_px, -2.0e6f), 2.0e6f);
+    float fhi = fminf(fmaxf((zc + hw - p.z0) * p.inv_px, -2.0e6f), 2.0e6f);
+    int lo = max(col_lo, __float2int_ru(flo));
+    int hi = min(col_hi, __float2int_rd(fhi));
     int len = rem >= 0.f ? max(0, hi - lo + 1) : 0;
+    if (NH > 1) {
+        int part = (len + NH - 1) / NH;
+        int first = min(len, h * part);
+        len = min(len - first, part);
+        lo += first;
+    }
     float ysec = y * e.sec2;
     float alpha = p.ak * ysec;
     r.u0 = fmaf((float)lo, p.px, p.z0) - zc;
@@ -171,14 +206,14 @@ __device__ __forceinline__ RowRec row_setup(const EventConsts& e, int iy, const 
               + p.d3k * ysec * fmaf(2.f * e.t, e.t, 1.f) * dy;
     r.alphas = kSqrtLH * alpha;
     r.eps = 2.f * e.t * alpha;
-    r.base = iy * p.n_z + lo;
+    r.lo = lo;
     r.len = len;
     return r;
 }
 
-// P (up to the constant K) at offset j of a row.
-__device__ __forceinline__ float kernel_value(const RowRec& r, float jpx, float c1s) {
-    float u = r.u0 + jpx;
+// P (up to the constant K) at pixel j of the row part.
+__device__ __forceinline__ float kernel_value(const RowConsts& r, float jf, float px, float c1s) {
+    float u = fmaf(jf, px, r.u0);
     float e2 = fmaf(c1s * u, u, r.c2s);
     float ba = fmaf(r.alphas, u, r.betas);
     float D = fmaf(r.eps, u, r.delta);
@@ -188,173 +223,438 @@ __device__ __forceinline__ float kernel_value(const RowRec& r, float jpx, float 
     return rs * ex2_approx(e2);
 }
 
-// One event group = NW warps working on one event at a time.  A "segment" is W consecutive pixels of one
-// ellipse row; a warp evaluates 32/W segments per iteration.  The first NIT iterations keep P in
-// registers for the scatter pass; later iterations (events larger than the tuned capacity) recompute it.
-template <int W, int NW, int NIT, int THREADS>
-__global__ void __launch_bounds__(THREADS)
-mlem_events_kernel(const float* __restrict__ events, long long n, const __grid_constant__ DevParams p,
-                   const float* __restrict__ w, float* __restrict__ acc, long long rep_stride, int n_rep,
-                   unsigned long long* __restrict__ counters) {
-    constexpr int G = 32 / W;
+// ------------------------------------------------------------------------------------------------------
+// Binning: sub-tile of the event's reconstructed point; NB = nby*nbz is the "direct" bin (events that do
+// not fit a region: non-finite, |tan theta~| > t_max, or centred outside the halo-extended image).
+__device__ __forceinline__ int event_bin(float zu, float zd, float dl, const DevParams& p) {
+    EventConsts e = event_setup(zu, zd, dl, p);
+    float fz = (e.z_t - p.z0) * p.inv_px;
+    bool regular = e.finite && fabsf(e.t) <= p.t_max && e.fy >= (float)(1 - p.Hy) && e.fy < (float)(p.n_y + p.Hy - 1) &&
+                   fz >= (float)(1 - p.Hz) && fz < (float)(p.n_z + p.Hz - 1);
+    if (!regular) return p.nby * p.nbz;
+    int iyc = __float2int_rd(e.fy + 0.5f), izc = __float2int_rd(fz + 0.5f);
+    int by = (iyc + p.Hy) / p.Sy, bz = (izc + p.Hz) / p.Sz;
+    by = min(max(by, 0), p.nby - 1);
+    bz = min(max(bz, 0), p.nbz - 1);
+    return by * p.nbz + bz;
+}
+
+// Histogram of the bins: per-block shared-memory histogram (when it fits), one global atomic per non-empty bin.
+constexpr int kBinBlock = 256, kBinPer = 8, kBinSmemMax = 12288;   // threads, events per thread, max bins in smem
+
+__global__ void __launch_bounds__(kBinBlock)
+bin_count_kernel(const float* __restrict__ events, int n, const __grid_constant__ DevParams p, int* __restrict__ bin_of,
+                 int* __restrict__ counts, int nb1, int use_smem) {
+    extern __shared__ int hist[];
+    const int tid = threadIdx.x;
+    if (use_smem) {
+        for (int b = tid; b < nb1; b += kBinBlock) hist[b] = 0;
+        __syncthreads();
+    }
+    const int base = blockIdx.x * (kBinBlock * kBinPer);
+#pragma unroll
+    for (int q = 0; q < kBinPer; ++q) {
+        const int i = base + q * kBinBlock + tid;
+        if (i < n) {
+            const int b = event_bin(__ldg(events + 3 * (size_t)i), __ldg(events + 3 * (size_t)i + 1), __ldg(events + 3 * (size_t)i + 2), p);
+            bin_of[i] = b;
+            atomicAdd(use_smem ? hist + b : counts + b, 1);
+        }
+    }
+    if (use_smem) {
+        __syncthreads();
+        for (int b = tid; b < nb1; b += kBinBlock) {
+            const int c = hist[b];
+            if (c) atomicAdd(counts + b, c);
+        }
+    }
+}
+
+// One block: exclusive prefix of counts -> starts (and cursors), work items for the regular bins.
+// meta[0] = number of items, meta[1] = start of the direct bin, meta[2] = its count, meta[3] = work counter (zeroed)
+__global__ void bin_scan_kernel(const int* __restrict__ counts, int* __restrict__ cursors, WorkItem* __restrict__ items,
+                                int* __restrict__ meta, int nb, int chunk) {
+    __shared__ int s_ev[1024], s_it[1024];
+    const int tid = threadIdx.x, T = blockDim.x;
+    const int per = (nb + 1 + T - 1) / T;                  // bins per thread, contiguous
+    const int b0 = tid * per, b1 = min(nb + 1, b0 + per);
+    int ev = 0, it = 0;
+    for (int b = b0; b < b1; ++b) {
+        int c = counts[b];
+        ev += c;
+        if (b < nb) it += (c + chunk - 1) / chunk;
+    }
+    s_ev[tid] = ev; s_it[tid] = it;
+    __syncthreads();
+    for (int d = 1; d < T; d <<= 1) {                      // Hillis-Steele inclusive scan
+        int a = tid >= d ? s_ev[tid - d] : 0, c = tid >= d ? s_it[tid - d] : 0;
+        __syncthreads();
+        s_ev[tid] += a; s_it[tid] += c;
+        __syncthreads();
+    }
+    int ev_off = s_ev[tid] - ev, it_off = s_it[tid] - it;
+    for (int b = b0; b < b1; ++b) {
+        int c = counts[b];
+        cursors[b] = ev_off;
+        if (b < nb) {
+            for (int k = 0; k < c; k += chunk) items[it_off++] = WorkItem{b, ev_off + k, min(chunk, c - k)};
+        } else {
+            meta[1] = ev_off;
+            meta[2] = c;
+        }
+        ev_off += c;
+    }
+    if (tid == T - 1) { meta[0] = s_it[tid]; meta[3] = 0; }
+}
+
+// Scatter into bin order: ranks inside the block from a shared-memory histogram, one global cursor atomic per
+// non-empty bin and block.  (The order of events inside a bin depends on block scheduling; sums are fp32.)
+__global__ void __launch_bounds__(kBinBlock)
+bin_scatter_kernel(const float* __restrict__ events, int n, const int* __restrict__ bin_of, int* __restrict__ cursors,
+                   float* __restrict__ sorted, int nb1, int use_smem) {
+    extern __shared__ int hist[];
+    const int tid = threadIdx.x;
+    const int base = blockIdx.x * (kBinBlock * kBinPer);
+    int bin[kBinPer], rank[kBinPer];
+    if (use_smem) {
+        for (int b = tid; b < nb1; b += kBinBlock) hist[b] = 0;
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < kBinPer; ++q) {
+            const int i = base + q * kBinBlock + tid;
+            bin[q] = i < n ? bin_of[i] : -1;
+            rank[q] = bin[q] >= 0 ? atomicAdd(hist + bin[q], 1) : 0;
+        }
+        __syncthreads();
+        for (int b = tid; b < nb1; b += kBinBlock) {
+            const int c = hist[b];
+            if (c) hist[b] = atomicAdd(cursors + b, c);       // count -> base of this block's run in bin b
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int q = 0; q < kBinPer; ++q) {
+        const int i = base + q * kBinBlock + tid;
+        if (i >= n) continue;
+        int pos;
+        if (use_smem) pos = hist[bin[q]] + rank[q];
+        else pos = atomicAdd(cursors + bin_of[i], 1);
+        sorted[3 * (size_t)pos] = __ldg(events + 3 * (size_t)i);
+        sorted[3 * (size_t)pos + 1] = __ldg(events + 3 * (size_t)i + 1);
+        sorted[3 * (size_t)pos + 2] = __ldg(events + 3 * (size_t)i + 2);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Compile-time loop: f(integral_constant<int, J>) for J in [J0, J1) - gives inline asm its immediates.
+template <int J0, int J1, typename F>
+__device__ __forceinline__ void static_for(F&& f) {
+    if constexpr (J0 < J1) {
+        f(std::integral_constant<int, J0>{});
+        static_for<J0 + 1, J1>(f);
+    }
+}
+
+// Shared-memory accessors on 32-bit shared-space addresses with immediate offsets (LDS/STS [R + imm]).
+template <int IMM>
+__device__ __forceinline__ float lds_imm(uint32_t addr) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1 + %2];" : "=f"(v) : "r"(addr), "n"(IMM));
+    return v;
+}
+// acc[addr + IMM] += P * inv for lanes with len > J, predicated (no branch)
+template <int IMM, int J>
+__device__ __forceinline__ void smem_fma_if(uint32_t addr, float P, float inv, int len) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .f32 t;\n\t"
+        "setp.gt.s32 p, %3, %4;\n\t"
+        "@p ld.shared.f32 t, [%0 + %5];\n\t"
+        "@p fma.rn.f32 t, %1, %2, t;\n\t"
+        "@p st.shared.f32 [%0 + %5], t;\n\t}"
+        ::"r"(addr), "f"(P), "f"(inv), "r"(len), "n"(J), "n"(IMM)
+        : "memory");
+}
+
+// Row constants rescaled so that the Gaussian term is -u'^2 with u' = u * sqrt(-c1s) (saves one FMUL per pixel).
+struct RowWalk {
+    float u0s, c2s, betas, delta, alphas, eps;   // alphas, eps divided by sqrt(-c1s); u0s multiplied by it
+    int lo, len;
+};
+
+template <int NH>
+__device__ __forceinline__ RowWalk row_walk_setup(const EventConsts& e, int iy, int h, int col_lo, int col_hi,
+                                                  const DevParams& p) {
+    RowConsts r = row_setup<NH>(e, iy, h, col_lo, col_hi, p);
+    RowWalk w;
+    w.u0s = r.u0 * p.sq;
+    w.c2s = r.c2s;
+    w.betas = r.betas;
+    w.delta = r.delta;
+    w.alphas = r.alphas * p.inv_sq;
+    w.eps = r.eps * p.inv_sq;
+    w.lo = r.lo;
+    w.len = r.len;
+    return w;
+}
+
+__device__ __forceinline__ float kernel_value_scaled(const RowWalk& r, float jf, float pxs) {
+    float u = fmaf(jf, pxs, r.u0s);
+    float D = fmaf(r.eps, u, r.delta);
+    float ba = fmaf(r.alphas, u, r.betas);
+    float rs = rsqrt_approx(D);
+    float e2 = fmaf(-u, u, r.c2s);
+    float bar = ba * rs;
+    e2 = fmaf(bar, bar, e2);
+    return rs * ex2_approx(e2);
+}
+
+// One event on one CTA, tiled path.  w_addr / a_addr: 32-bit shared addresses of the region origins; pixel
+// (iy, iz) lives at base + 4 * ((iz - rz0) * HS + (iy - ry0)).  THREAD <-> ROW (part h of NH).
+template <int NW, int NH, int NR, int NJ, int HS>
+__device__ __forceinline__ void process_event_tiled(float zu, float zd, float dl, const DevParams& p, uint32_t w_addr,
+                                                    uint32_t a_addr, int ry0, int rz0, int row_lo, int row_hi, int col_lo,
+                                                    int col_hi, float* red_s, unsigned long long& my_evals,
+                                                    unsigned long long& my_skipped) {
     constexpr int GT = NW * 32;
-    constexpr int GROUPS = THREADS / GT;
-    constexpr int SEG_PER_IT = G * NW;
-    static_assert(THREADS % GT == 0 && 32 % W == 0, "bad shape");
+    constexpr int RT = GT / NH;                 // threads (rows) per pass
+    constexpr int U = 4;                        // pixels per branch-free block
+    constexpr int NB = (NJ + U - 1) / U;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int h = tid / RT, k = tid - h * RT;   // row part and row slot of this thread
+    const float pxs = p.px * p.sq;
 
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int group = threadIdx.x / GT;
-    const int gtid = threadIdx.x % GT;
-    const int lane = threadIdx.x & 31;
-    const int warp_in_group = gtid >> 5;
-    // per-group layout: RowRec[nrow_max] | uint32 segmap[nseg_max] | float red[NW]
-    const size_t rows_bytes = (size_t)p.nrow_max * sizeof(RowRec);
-    const size_t seg_bytes = (((size_t)p.nseg_max * 4 + 15) / 16) * 16;
-    const size_t group_bytes = rows_bytes + seg_bytes + 16 * ((NW * 4 + 15) / 16);
-    unsigned char* gbase = smem_raw + group * group_bytes;
-    RowRec* rowtab = reinterpret_cast<RowRec*>(gbase);
-    uint32_t* segmap = reinterpret_cast<uint32_t*>(gbase + rows_bytes);
-    float* red = reinterpret_cast<float*>(gbase + rows_bytes + seg_bytes);
+    const EventConsts e = event_setup(zu, zd, dl, p);
+    int iy_lo, nrows;
+    event_rows(e, row_lo, row_hi, iy_lo, nrows);
 
-    float* acc_rep = acc + (size_t)(blockIdx.x % n_rep) * rep_stride;
-    const int sub = lane / W;                       // sub-warp (segment slot) within the warp
-    const int jl = lane % W;                        // pixel within the segment
-    const float jlpx = (float)jl * p.px;
-    const float wpx = (float)W * p.px;
+    float preg[NR][NB * U];
+    int len[NR], wmax[NR];
+    uint32_t off[NR];
+    float denom = 0.f;
+    int cnt = 0;
+#pragma unroll
+    for (int i = 0; i < NR; ++i) {
+        const int r = k + i * RT;
+        RowWalk rc;
+        rc.u0s = 0.f; rc.c2s = 0.f; rc.betas = 0.f; rc.delta = 1.f; rc.alphas = 0.f; rc.eps = 0.f; rc.lo = rz0; rc.len = 0;
+        int iy = ry0;
+        if (r < nrows) { iy = iy_lo + r; rc = row_walk_setup<NH>(e, iy, h, col_lo, col_hi, p); }
+        len[i] = rc.len;
+        off[i] = 4u * (uint32_t)((rc.lo - rz0) * HS + (iy - ry0));
+        cnt += rc.len;
+        wmax[i] = __reduce_max_sync(0xffffffffu, rc.len);
+        const uint32_t wa = w_addr + off[i];
+        static_for<0, NB>([&](auto bc) {
+            constexpr int jb = decltype(bc)::value * U;
+            if (jb < wmax[i]) {                                  // warp-uniform
+                static_for<0, U>([&](auto jc) {
+                    constexpr int j = jb + decltype(jc)::value;
+                    float P = kernel_value_scaled(rc, (float)j, pxs);
+                    P = j < rc.len ? P : 0.f;                    // lanes past their span contribute nothing; the
+                    const float wv = lds_imm<4 * j * HS>(wa);    // read stays inside the (finite) shared arrays
+                    denom = fmaf(P, wv, denom);
+                    preg[i][j] = P;
+                });
+            }
+        });
+        for (int j = NB * U; j < rc.len; ++j) {                  // longer than the register cache (not in tuned configs)
+            float P = kernel_value_scaled(rc, (float)j, pxs);
+            float wv;
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(wv) : "r"(wa + 4u * (uint32_t)(j * HS)));
+            denom = fmaf(P, wv, denom);
+        }
+    }
+    for (int r = k + NR * RT; r < nrows; r += RT) {              // more rows than NR passes (not in tuned configs)
+        RowWalk rc = row_walk_setup<NH>(e, iy_lo + r, h, col_lo, col_hi, p);
+        const uint32_t wa = w_addr + 4u * (uint32_t)((rc.lo - rz0) * HS + (iy_lo + r - ry0));
+        cnt += rc.len;
+        for (int j = 0; j < rc.len; ++j) {
+            float P = kernel_value_scaled(rc, (float)j, pxs);
+            float wv;
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(wv) : "r"(wa + 4u * (uint32_t)(j * HS)));
+            denom = fmaf(P, wv, denom);
+        }
+    }
+    my_evals += (unsigned long long)cnt;
 
+    // ---- denominator: sum over the CTA -------------------------------------------------------------------
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) denom += __shfl_xor_sync(0xffffffffu, denom, d);
+    if (NW > 1) {
+        if (lane == 0) red_s[tid >> 5] = denom;
+        __syncthreads();
+        denom = 0.f;
+#pragma unroll
+        for (int q = 0; q < NW; ++q) denom += red_s[q];
+    } else {
+        __syncwarp();
+    }
+
+    // ---- back-projection: acc += P / denominator (private region: plain read-modify-write) --------------------
+    const bool ok = (denom > 0.f) && (denom < 3.0e38f);
+    if (tid == 0 && !ok) my_skipped += 1ull;
+    if (!ok) return;
+    const float inv = 1.f / denom;
+#pragma unroll
+    for (int i = 0; i < NR; ++i) {
+        const uint32_t aa = a_addr + off[i];
+        static_for<0, NB>([&](auto bc) {
+            constexpr int jb = decltype(bc)::value * U;
+            if (jb < wmax[i]) {
+                static_for<0, U>([&](auto jc) {
+                    constexpr int j = jb + decltype(jc)::value;
+                    smem_fma_if<4 * j * HS, j>(aa, preg[i][j], inv, len[i]);
+                });
+            }
+        });
+        if (len[i] > NB * U) {
+            const int r = k + i * RT;
+            RowWalk rc = row_walk_setup<NH>(e, iy_lo + r, h, col_lo, col_hi, p);
+            for (int j = NB * U; j < rc.len; ++j) {
+                float v = kernel_value_scaled(rc, (float)j, pxs) * inv, t;
+                const uint32_t ad = aa + 4u * (uint32_t)(j * HS);
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(t) : "r"(ad));
+                asm volatile("st.shared.f32 [%0], %1;" ::"r"(ad), "f"(t + v) : "memory");
+            }
+        }
+    }
+    for (int r = k + NR * RT; r < nrows; r += RT) {
+        RowWalk rc = row_walk_setup<NH>(e, iy_lo + r, h, col_lo, col_hi, p);
+        const uint32_t aa = a_addr + 4u * (uint32_t)((rc.lo - rz0) * HS + (iy_lo + r - ry0));
+        for (int j = 0; j < rc.len; ++j) {
+            float v = kernel_value_scaled(rc, (float)j, pxs) * inv, t;
+            const uint32_t ad = aa + 4u * (uint32_t)(j * HS);
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(t) : "r"(ad));
+            asm volatile("st.shared.f32 [%0], %1;" ::"r"(ad), "f"(t + v) : "memory");
+        }
+    }
+}
+
+// Tiled path: work items (sub-tile, chunk of sorted events), private shared-memory region per CTA.
+template <int NW, int NH, int NR, int NJ, int HS>
+__global__ void __launch_bounds__(NW * 32)
+mlem_rows_kernel(const float* __restrict__ sorted, const WorkItem* __restrict__ items, int* __restrict__ meta,
+                 const __grid_constant__ DevParams p, const float* __restrict__ wT, float* __restrict__ accT,
+                 unsigned long long* __restrict__ counters) {
+    constexpr int GT = NW * 32;
+    extern __shared__ __align__(16) float smem[];
+    const int WZ = p.WZ;
+    float* w_s = smem;
+    float* acc_s = smem + HS * WZ;
+    const uint32_t w_addr = (uint32_t)__cvta_generic_to_shared(w_s);
+    const uint32_t a_addr = (uint32_t)__cvta_generic_to_shared(acc_s);
+    __shared__ float red_s[2][NW];
+    __shared__ int item_s;
+    const int tid = threadIdx.x;
+    const int n_items = meta[0];
     unsigned long long my_evals = 0, my_skipped = 0;
-    const long long n_groups = (long long)gridDim.x * GROUPS;
+    int parity = 0;
 
-    for (long long ev = (long long)blockIdx.x * GROUPS + group; ev < n; ev += n_groups) {
-        // ---- step 1: Eq. 2 + row range (all lanes, broadcast loads) -----------------------------------
-        const float zu = __ldg(events + 3 * ev), zd = __ldg(events + 3 * ev + 1), dl = __ldg(events + 3 * ev + 2);
-        const EventConsts e = event_setup(zu, zd, dl, p);
-
-        // ---- row table + segment map (threads <-> rows) ------------------------------------------------
-        int seg_total = 0, px_total = 0;
-        for (int r0 = 0; r0 < e.nrows; r0 += GT) {
-            int r = r0 + gtid;
-            int nseg = 0, len = 0;
-            RowRec rec;
-            if (r < e.nrows) {
-                rec = row_setup(e, e.iy_lo + r, p);
-                len = rec.len;
-                nseg = (len + W - 1) / W;
-                rowtab[r] = rec;
-            }
-            // exclusive scan of nseg over the group's threads
-            int incl = nseg, lsum = len;
+    while (true) {
+        if (tid == 0) item_s = atomicAdd(meta + 3, 1);
+        __syncthreads();
+        const int item = item_s;
+        if (item >= n_items) break;
+        const WorkItem wi = items[item];
+        const int by = wi.bin / p.nbz, bz = wi.bin - by * p.nbz;
+        const int ry0 = by * p.Sy - 2 * p.Hy, rz0 = bz * p.Sz - 2 * p.Hz;        // region origin (pixel indices)
+        const int row_lo = max(0, ry0), row_hi = min(p.n_y - 1, ry0 + p.Sy + 2 * p.Hy - 1);
+        const int col_lo = max(0, rz0), col_hi = min(p.n_z - 1, rz0 + WZ - 1);
+        // stage w (several loads in flight per thread), zero the accumulator region
+        for (int i0 = tid; i0 < HS * WZ; i0 += 4 * GT) {
+            float v[4];
 #pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                int v = __shfl_up_sync(0xffffffffu, incl, d);
-                if (lane >= d) incl += v;
+            for (int q = 0; q < 4; ++q) {
+                const int i = i0 + q * GT;
+                const int c = i / HS, r = i - c * HS;
+                const int iz = rz0 + c, iy = ry0 + r;
+                v[q] = 0.f;
+                if (i < HS * WZ && iz >= col_lo && iz <= col_hi && iy >= row_lo && iy <= row_hi)
+                    v[q] = __ldg(wT + (size_t)iz * p.n_y + iy);
             }
 #pragma unroll
-            for (int d = 16; d > 0; d >>= 1) lsum += __shfl_xor_sync(0xffffffffu, lsum, d);
-            int warp_off = 0, chunk_total = __shfl_sync(0xffffffffu, incl, 31), chunk_px = lsum;
-            if (NW > 1) {   // combine the warps of the group
-                __shared__ int scan_buf[THREADS / 32][2];
-                if (lane == 31) { scan_buf[threadIdx.x >> 5][0] = incl; scan_buf[threadIdx.x >> 5][1] = lsum; }
-                group_barrier(1 + group, GT);
-                chunk_total = 0; chunk_px = 0;
-#pragma unroll
-                for (int k = 0; k < NW; ++k) {
-                    int v = scan_buf[group * NW + k][0];
-                    if (k < warp_in_group) warp_off += v;
-                    chunk_total += v;
-                    chunk_px += scan_buf[group * NW + k][1];
-                }
-                group_barrier(1 + group, GT);
+            for (int q = 0; q < 4; ++q) {
+                const int i = i0 + q * GT;
+                if (i < HS * WZ) { w_s[i] = v[q]; acc_s[i] = 0.f; }
             }
-            int excl = seg_total + warp_off + incl - nseg;
-            for (int s = 0; s < nseg; ++s)
-                if (excl + s < p.nseg_max) segmap[excl + s] = (uint32_t)r | ((uint32_t)s << 16);
-            seg_total += chunk_total;
-            px_total += chunk_px;
         }
-        seg_total = min(seg_total, p.nseg_max);
-        if (NW > 1) group_barrier(1 + group, GT); else __syncwarp();
+        __syncthreads();
+        const float* ev = sorted + 3 * (size_t)wi.start;
+        float zu = __ldg(ev), zd = __ldg(ev + 1), dl = __ldg(ev + 2);
+        for (int q = 0; q < wi.count; ++q) {
+            float nzu = 0.f, nzd = 0.f, ndl = 0.f;
+            if (q + 1 < wi.count) { nzu = __ldg(ev + 3 * (q + 1)); nzd = __ldg(ev + 3 * (q + 1) + 1); ndl = __ldg(ev + 3 * (q + 1) + 2); }
+            process_event_tiled<NW, NH, NR, NJ, HS>(zu, zd, dl, p, w_addr, a_addr, ry0, rz0, row_lo, row_hi, col_lo, col_hi,
+                                                    red_s[parity], my_evals, my_skipped);
+            parity ^= 1;
+            zu = nzu; zd = nzd; dl = ndl;
+        }
+        __syncthreads();
+        // flush the private region into the global transposed accumulator
+        for (int i = tid; i < HS * WZ; i += GT) {
+            const int c = i / HS, r = i - c * HS;
+            const int iz = rz0 + c, iy = ry0 + r;
+            const float v = acc_s[i];
+            if (v != 0.f && iz >= col_lo && iz <= col_hi && iy >= row_lo && iy <= row_hi)
+                red_add_f32(accT + (size_t)iz * p.n_y + iy, v);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) my_evals += __shfl_xor_sync(0xffffffffu, my_evals, d);
+    if ((tid & 31) == 0 && my_evals) atomicAdd(counters + 0, my_evals);
+    if (tid == 0 && my_skipped) atomicAdd(counters + 1, my_skipped);
+}
 
-        // ---- step 2: kernel values + denominator --------------------------------------------------------
-        float preg[NIT];
-        int ireg[NIT];
+// Direct path: events of the "direct" bin (rare: non-finite, extreme angles, far outside the image), or every
+// event when a region does not fit shared memory.  One warp per event, thread <-> row, w read from the global
+// transposed image, back-projection with red.global.add.f32, P recomputed in the second pass.  Simple on purpose.
+__global__ void __launch_bounds__(128)
+mlem_rows_direct_kernel(const float* __restrict__ sorted, const int* __restrict__ meta, const __grid_constant__ DevParams p,
+                        const float* __restrict__ wT, float* __restrict__ accT, unsigned long long* __restrict__ counters) {
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
+    const int start = meta[1], count = meta[2];
+    unsigned long long my_evals = 0, my_skipped = 0;
+    for (int q = warp; q < count; q += n_warps) {
+        const float* ev = sorted + 3 * (size_t)(start + q);
+        const EventConsts e = event_setup(__ldg(ev), __ldg(ev + 1), __ldg(ev + 2), p);
+        int iy_lo, nrows;
+        event_rows(e, 0, p.n_y - 1, iy_lo, nrows);
         float denom = 0.f;
-        const int my_first = warp_in_group * G + sub;
-#pragma unroll
-        for (int it = 0; it < NIT; ++it) {
-            int sidx = it * SEG_PER_IT + my_first;
-            float P = 0.f;
-            int idx = -1;
-            if (sidx < seg_total) {
-                uint32_t m = segmap[sidx];
-                const RowRec rec = rowtab[m & 0xffffu];
-                int j = (int)(m >> 16) * W + jl;
-                if (j < rec.len) {
-                    P = kernel_value(rec, fmaf((float)(m >> 16), wpx, jlpx), p.c1s);
-                    idx = rec.base + j;
-                    denom = fmaf(P, __ldg(w + idx), denom);
-                }
-            }
-            preg[it] = P;
-            ireg[it] = idx;
-        }
-        for (int sidx = NIT * SEG_PER_IT + my_first; sidx < seg_total; sidx += SEG_PER_IT) {   // overflow, uncached
-            uint32_t m = segmap[sidx];
-            const RowRec rec = rowtab[m & 0xffffu];
-            int j = (int)(m >> 16) * W + jl;
-            if (j < rec.len) {
-                float P = kernel_value(rec, fmaf((float)(m >> 16), wpx, jlpx), p.c1s);
-                denom = fmaf(P, __ldg(w + rec.base + j), denom);
-            }
+        for (int r = lane; r < nrows; r += 32) {
+            const RowConsts rc = row_setup<1>(e, iy_lo + r, 0, 0, p.n_z - 1, p);
+            const float* wp = wT + (size_t)rc.lo * p.n_y + (iy_lo + r);
+            my_evals += (unsigned long long)rc.len;
+            for (int j = 0; j < rc.len; ++j) denom = fmaf(kernel_value(rc, (float)j, p.px, p.c1s), __ldg(wp + (size_t)j * p.n_y), denom);
         }
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) denom += __shfl_xor_sync(0xffffffffu, denom, d);
-        if (NW > 1) {
-            if (lane == 0) red[warp_in_group] = denom;
-            group_barrier(1 + group, GT);
-            denom = 0.f;
-#pragma unroll
-            for (int k = 0; k < NW; ++k) denom += red[k];
+        const bool ok = (denom > 0.f) && (denom < 3.0e38f);
+        if (lane == 0 && !ok) my_skipped += 1ull;
+        if (!ok) continue;
+        const float inv = 1.f / denom;
+        for (int r = lane; r < nrows; r += 32) {
+            const RowConsts rc = row_setup<1>(e, iy_lo + r, 0, 0, p.n_z - 1, p);
+            float* ap = accT + (size_t)rc.lo * p.n_y + (iy_lo + r);
+            for (int j = 0; j < rc.len; ++j) red_add_f32(ap + (size_t)j * p.n_y, kernel_value(rc, (float)j, p.px, p.c1s) * inv);
         }
-
-        // ---- step 3: scatter P / denominator -------------------------------------------------------------
-        const bool ok = (seg_total > 0) && (denom > 0.f) && (denom < 3.0e38f);
-        if (ok) {
-            const float inv = 1.f / denom;
-#pragma unroll
-            for (int it = 0; it < NIT; ++it)
-                if (ireg[it] >= 0) red_add_f32(acc_rep + ireg[it], preg[it] * inv);
-            for (int sidx = NIT * SEG_PER_IT + my_first; sidx < seg_total; sidx += SEG_PER_IT) {
-                uint32_t m = segmap[sidx];
-                const RowRec rec = rowtab[m & 0xffffu];
-                int j = (int)(m >> 16) * W + jl;
-                if (j < rec.len) {
-                    float P = kernel_value(rec, fmaf((float)(m >> 16), wpx, jlpx), p.c1s);
-                    red_add_f32(acc_rep + rec.base + j, P * inv);
-                }
-            }
-        }
-        if (gtid == 0) {
-            my_evals += (unsigned long long)px_total;
-            my_skipped += ok ? 0ull : 1ull;
-        }
-        // tables are rewritten by the next event: everyone must be done reading them
-        if (NW > 1) group_barrier(1 + group, GT); else __syncwarp();
     }
-    if (gtid == 0) {
-        if (my_evals) atomicAdd(counters + 0, my_evals);
-        if (my_skipped) atomicAdd(counters + 1, my_skipped);
-    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) my_evals += __shfl_xor_sync(0xffffffffu, my_evals, d);
+    if (lane == 0 && my_evals) atomicAdd(counters + 0, my_evals);
+    if (lane == 0 && my_skipped) atomicAdd(counters + 1, my_skipped);
 }
 
 // |E_j| only (jpet_count_evals): thread per event, rows in a loop, no kernel values.
 __global__ void count_evals_kernel(const float* __restrict__ events, long long n, const __grid_constant__ DevParams p,
                                    unsigned long long* __restrict__ counters) {
     unsigned long long evals = 0, skipped = 0;
-    for (long long ev = (long long)blockIdx.x * blockDim.x + threadIdx.x; ev < n; ev += (long long)gridDim.x * blockDim.x) {
-        EventConsts e = event_setup(events[3 * ev], events[3 * ev + 1], events[3 * ev + 2], p);
-        int cnt = 0;
-        for (int r = 0; r < e.nrows; ++r) cnt += row_setup(e, e.iy_lo + r, p).len;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        EventConsts e = event_setup(events[3 * i], events[3 * i + 1], events[3 * i + 2], p);
+        int iy_lo, nrows, cnt = 0;
+        event_rows(e, 0, p.n_y - 1, iy_lo, nrows);
+        for (int r = 0; r < nrows; ++r) cnt += row_setup<1>(e, iy_lo + r, 0, 0, p.n_z - 1, p).len;
         evals += cnt;
         skipped += cnt == 0;
     }

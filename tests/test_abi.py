@@ -63,7 +63,7 @@ def test_argument_validation_needs_no_gpu():
     assert lib.jpet_mlem_accumulate(None, 0, None) == binding.JPET_E_INVAL   # no begin
     assert lib.jpet_mlem_end(None, None, None) == binding.JPET_E_INVAL
     assert lib.jpet_set_option(b"nonsense", 1) == binding.JPET_E_INVAL
-    assert lib.jpet_set_option(b"replicas", 1000) == binding.JPET_E_INVAL
+    assert lib.jpet_set_option(b"chunk", -5) == binding.JPET_E_INVAL
     assert lib.jpet_set_a3_coef(ctypes.c_float(float("nan"))) == binding.JPET_E_INVAL
     assert abs(lib.jpet_get_a3_coef() - 2.0) < 1e-7
 

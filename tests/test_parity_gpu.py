@@ -24,7 +24,8 @@ def jp():
     jp.binding.load(build_if_missing=False)   # the in-tree .so must be the one that runs
     yield jp
     jp.jpet_set_option("variant", -1)
-    jp.jpet_set_option("replicas", 0)
+    jp.jpet_set_option("force_direct", 0)
+    jp.jpet_set_option("chunk", 0)
     jp.jpet_set_a3_coef(2.0)
 
 
@@ -47,7 +48,8 @@ def gpu_iterate(jp, ev, cfg, rho_in, n_iter=1):
 
 
 def rel_err(got, want):
-    return float(np.max(np.abs(got - want)) / np.max(want))
+    m = float(np.max(want))
+    return float(np.max(np.abs(got - want)) / m) if m > 0 else float(np.max(np.abs(got)))
 
 
 # ------------------------------------------------------------------------------------------------------
@@ -103,11 +105,11 @@ def test_cfg1_ten_iterations(jp, oracle):
     assert rel_err(got, want) <= TOL_10
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7])
 @pytest.mark.parametrize("name,n", [("cfg1", 7777), ("cfg2", 30011), ("cfg4", 5003)])
 def test_every_kernel_variant(jp, oracle, variant, name, n):
-    """Each event-kernel shape (segment width, warps per event, cached iterations) on small, medium and
-    large ellipses; on config 4 the narrow variants overflow their register cache and take the recompute path."""
+    """Each event-kernel shape (warps per CTA, row parts, row passes, cached pixels) on small, medium and large
+    ellipses; on configs 2 and 4 the small shapes overflow their register cache and take the recompute loops."""
     cfg = synth.CONFIGS[name]
     ev = synth.config_events(cfg, n=n)
     rho = np.random.default_rng(1).uniform(0.5, 2.0, (cfg.n_y, cfg.n_z)).astype(np.float32)
@@ -263,7 +265,7 @@ def test_edge_cases(jp, oracle):
     got0, (_, ns0) = gpu_iterate(jp, good, cfg, np.zeros((cfg.n_y, cfg.n_z)))
     assert (got0 == 0).all() and ns0 == len(good)
     # single event against the oracle (ellipse clipped by the grid edge as well)
-    for e in ([120.0, -60.0, -80.0], [-230.0, -180.0, 250.0]):
+    for e in ([120.0, -60.0, -80.0], [-230.0, -180.0, 250.0], [-150.0, -100.0, 280.0]):
         ev1 = np.array([e], np.float32)
         g1, (ne1, ns1) = gpu_iterate(jp, ev1, cfg, np.ones((cfg.n_y, cfg.n_z)))
         w1, one1, ons1 = oracle.mlem_iterate(ev1, *geom(cfg), np.ones((cfg.n_y, cfg.n_z)))
@@ -308,16 +310,24 @@ def test_errors_are_reported_not_swallowed(jp):
         jp.jpet_mlem_iterate(torch.empty((4, 3), device="cuda"), *geom(cfg), ones[:-1], ones)
 
 
-def test_replicas_and_determinism_of_the_reduction(jp, oracle):
+def test_direct_path_and_chunking(jp, oracle):
+    """The direct kernel (no shared-memory tiles, red.global.add into the image) on a whole workload, and the
+    tiled path with tiny and huge work items."""
     cfg = synth.CONFIGS["cfg2"]
     ev = synth.config_events(cfg, n=50_000)
     ones = np.ones((cfg.n_y, cfg.n_z))
-    want, _, _ = oracle.mlem_iterate(ev, *geom(cfg), ones)
+    want, one, ons = oracle.mlem_iterate(ev, *geom(cfg), ones)
     try:
-        for rep in (1, 3, 16):
-            jp.jpet_set_option("replicas", rep)
-            got, _ = gpu_iterate(jp, ev, cfg, ones)
-            assert jp.jpet_get_option("last_replicas") == rep
-            assert rel_err(got, want) <= TOL_1
+        jp.jpet_set_option("force_direct", 1)
+        got, (ne, ns) = gpu_iterate(jp, ev, cfg, ones)
+        assert jp.jpet_get_option("last_tiled") == 0
+        assert rel_err(got, want) <= TOL_1 and ns == ons and abs(ne - one) <= 1e-5 * one + 2
+        jp.jpet_set_option("force_direct", 0)
+        for chunk in (1, 7, 100_000):
+            jp.jpet_set_option("chunk", chunk)
+            got, (ne, ns) = gpu_iterate(jp, ev, cfg, ones)
+            assert jp.jpet_get_option("last_tiled") == 1
+            assert rel_err(got, want) <= TOL_1 and ns == ons and abs(ne - one) <= 1e-5 * one + 2
     finally:
-        jp.jpet_set_option("replicas", 0)
+        jp.jpet_set_option("force_direct", 0)
+        jp.jpet_set_option("chunk", 0)
