@@ -143,6 +143,7 @@ def main():
     ap.add_argument("--variant", type=int, default=-1)
     ap.add_argument("--chunk", type=int, default=0)
     ap.add_argument("--ctas-per-sm", type=int, default=0)
+    ap.add_argument("--sub-tile-z", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -176,6 +177,8 @@ def main():
         jp.jpet_set_option("variant", args.variant)
     if args.chunk > 0:
         jp.jpet_set_option("chunk", args.chunk)
+    if args.sub_tile_z > 0:
+        jp.jpet_set_option("sub_tile_z", args.sub_tile_z)
     if args.ctas_per_sm > 0:
         jp.jpet_set_option("ctas_per_sm", args.ctas_per_sm)
 

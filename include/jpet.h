@@ -113,6 +113,7 @@ float jpet_get_a3_coef(void);
  *   "force_direct" 1 = skip the shared-memory tiled path: every event goes through the direct kernel
  *                  (w from global memory, red.global.add into the image); 0 = automatic
  *   "chunk"        events per work item of the tiled path; 0 = automatic
+ *   "sub_tile_z"   width in pixels of the image sub-tiles the events are sorted by; 0 = automatic
  *   "ctas_per_sm"  cap on resident CTAs per SM for the persistent grid; 0 = automatic
  *   "time_kernel"  1 = bracket each tiled event-kernel launch with CUDA events on its stream; the duration of the
  *                  last launch is then read with jpet_get_option("last_kernel_ns") (synchronises on that launch)

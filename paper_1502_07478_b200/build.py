@@ -10,7 +10,7 @@ CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libjpet.so")
 SOURCES = [os.path.join(CSRC, "jpet_api.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "mlem_kernels.cuh"), os.path.join(os.path.dirname(_HERE), "include", "jpet.h")]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math",
               "-Xcompiler", "-fPIC", "-shared"]
 
 

@@ -23,6 +23,7 @@ std::atomic<uint64_t> g_launches{0};
 float g_a3_coef = 2.0f;
 int64_t g_opt_force_direct = 0;  // 1 = every event takes the direct (global-memory) path
 int64_t g_opt_chunk = 0;         // events per work item, 0 = automatic
+int64_t g_opt_sz = 0;            // sub-tile width in pixels, 0 = automatic
 int64_t g_opt_time_kernel = 0;   // 1 = bracket the tiled event kernel with CUDA events (bench.py's roofline)
 cudaEvent_t g_tk0 = nullptr, g_tk1 = nullptr;
 bool g_tk_valid = false;
@@ -145,22 +146,22 @@ int ensure_images(int M) {
 
 // ---- event-kernel variants: NW warps per CTA, rows split in NH parts, NR row passes, NJ cached pixels,
 // HS = region row stride (compile time, so every shared-memory access has an immediate offset) ---------------
-struct Variant { int NW, NH, NR, NJ, HS; };
+struct Variant { int NW, NH, NR, NJ, HS, U, CF, MINB; };
 constexpr Variant kVariants[] = {
-    {1, 1, 1, 12, 64},    // 0: <= 32 rows, chords <= 12 px                    (config 1)
-    {2, 1, 1, 20, 64},    // 1: <= 64 rows, chords <= 20 px                    (configs 2, 3)
-    {4, 2, 1, 12, 64},    // 2: <= 64 rows, chords <= 24 px in two halves
-    {4, 1, 1, 36, 128},   // 3: <= 128 rows, chords <= 36 px                   (config 4)
-    {8, 2, 1, 20, 128},   // 4: <= 128 rows, chords <= 40 px in two halves
-    {8, 2, 1, 24, 160},   // 5: <= 128 rows, chords <= 48 px in two halves     (config 5)
-    {4, 1, 1, 44, 160},   // 6: <= 128 rows, chords <= 44 px
-    {1, 1, 2, 20, 64},    // 7: <= 64 rows in two passes of one warp, chords <= 20 px
+    {1, 1, 1, 12, 64, 4, 1, 1},    // 0: <= 32 rows, chords <= 12 px                            (config 1)
+    {2, 1, 1, 20, 64, 4, 1, 10},   // 1: <= 64 rows, chords <= 20 px, <= 96 registers           (configs 2, 3)
+    {4, 2, 1, 12, 64, 4, 1, 1},    // 2: <= 64 rows, chords <= 24 px in two halves
+    {4, 1, 1, 36, 128, 4, 1, 1},   // 3: <= 128 rows, chords <= 36 px
+    {8, 2, 1, 20, 128, 4, 1, 1},   // 4: <= 128 rows, chords <= 40 px in two halves             (config 4)
+    {8, 2, 1, 24, 160, 4, 1, 1},   // 5: <= 128 rows, chords <= 48 px in two halves             (config 5)
+    {4, 1, 1, 44, 160, 4, 1, 1},   // 6: <= 128 rows, chords <= 44 px
+    {1, 1, 2, 20, 64, 4, 1, 1},    // 7: <= 64 rows in two passes of one warp, chords <= 20 px
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
-template <int NW, int NH, int NR, int NJ, int HS>
+template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF, int MINB>
 int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
-    auto kern = jpet::mlem_rows_kernel<NW, NH, NR, NJ, HS>;
+    auto kern = jpet::mlem_rows_kernel<NW, NH, NR, NJ, HS, U, CF, MINB>;
     if (dp.t_max >= 0.f) {     // tiled path
         if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
         static size_t attr_set = 0;
@@ -193,14 +194,14 @@ int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t
 
 int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t st) {
     switch (variant) {
-        case 0: return launch_rows<1, 1, 1, 12, 64>(bs, dp, smem, st);
-        case 1: return launch_rows<2, 1, 1, 20, 64>(bs, dp, smem, st);
-        case 2: return launch_rows<4, 2, 1, 12, 64>(bs, dp, smem, st);
-        case 3: return launch_rows<4, 1, 1, 36, 128>(bs, dp, smem, st);
-        case 4: return launch_rows<8, 2, 1, 20, 128>(bs, dp, smem, st);
-        case 5: return launch_rows<8, 2, 1, 24, 160>(bs, dp, smem, st);
-        case 6: return launch_rows<4, 1, 1, 44, 160>(bs, dp, smem, st);
-        case 7: return launch_rows<1, 1, 2, 20, 64>(bs, dp, smem, st);
+        case 0: return launch_rows<1, 1, 1, 12, 64, 4, true, 1>(bs, dp, smem, st);
+        case 1: return launch_rows<2, 1, 1, 20, 64, 4, true, 10>(bs, dp, smem, st);
+        case 2: return launch_rows<4, 2, 1, 12, 64, 4, true, 1>(bs, dp, smem, st);
+        case 3: return launch_rows<4, 1, 1, 36, 128, 4, true, 1>(bs, dp, smem, st);
+        case 4: return launch_rows<8, 2, 1, 20, 128, 4, true, 1>(bs, dp, smem, st);
+        case 5: return launch_rows<8, 2, 1, 24, 160, 4, true, 1>(bs, dp, smem, st);
+        case 6: return launch_rows<4, 1, 1, 44, 160, 4, true, 1>(bs, dp, smem, st);
+        case 7: return launch_rows<1, 1, 2, 20, 64, 4, true, 1>(bs, dp, smem, st);
         default: return fail(JPET_E_INVAL, "unknown kernel variant %d", variant);
     }
 }
@@ -241,12 +242,12 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     p.t_max = (float)t_max;
     // variant: smallest shape that holds rows_max rows, chord_max pixels per row, and the region's rows
     auto fits = [&](const Variant& c) {
-        return rows_max <= c.NW * 32 / c.NH * c.NR && chord_max <= c.NJ * c.NH && 2 * p.Hy + 4 <= c.HS;
+        return rows_max + 1 <= c.NW * 32 / c.NH * c.NR && chord_max <= c.NJ * c.NH && 2 * p.Hy + 4 <= c.HS;
     };
     int v = -1;
     if (g_opt_variant >= 0) v = (int)g_opt_variant;
     else {
-        const int order[] = {0, 1, 3, 5};
+        const int order[] = {0, 1, 4, 5};
         for (int cand : order)
             if (fits(kVariants[cand])) { v = cand; break; }
         if (v < 0) v = 5;
@@ -254,7 +255,7 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     const bool tiles_ok = 2 * p.Hy + 4 <= kVariants[v].HS;     // else: every event takes the direct path
     p.HS = kVariants[v].HS;
     p.Sy = std::max(1, p.HS - 2 * p.Hy);
-    p.Sz = 16;
+    p.Sz = g_opt_sz > 0 ? (int)g_opt_sz : 8;
     // shared memory: w region + accumulator region; shrink the sub-tile width, then give up tiling
     const size_t budget = 200 * 1024;
     size_t smem = 0;
@@ -267,7 +268,7 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     if (smem > budget || !tiles_ok || p.WZ < kVariants[v].NJ + 4 || g_opt_force_direct) { p.t_max = -1.f; smem = 0; }
     p.nby = (gr.n_y + 2 * p.Hy + p.Sy - 1) / p.Sy;
     p.nbz = (gr.n_z + 2 * p.Hz + p.Sz - 1) / p.Sz;
-    p.chunk = g_opt_chunk > 0 ? (int)g_opt_chunk : 128;
+    p.chunk = g_opt_chunk > 0 ? (int)g_opt_chunk : 64;
     *out = p;
     *variant = v;
     *smem_out = smem;
@@ -683,6 +684,9 @@ int jpet_set_option(const char* name, int64_t value) {
         if (value < 0 || value > 1) return fail(JPET_E_INVAL, "time_kernel must be 0 or 1");
         g_opt_time_kernel = value;
         g_tk_valid = false;
+    } else if (!strcmp(name, "sub_tile_z")) {
+        if (value < 0 || value > 256) return fail(JPET_E_INVAL, "sub_tile_z must be 0 (auto) .. 256");
+        g_opt_sz = value;
     } else if (!strcmp(name, "chunk")) {
         if (value < 0 || value > (1 << 20)) return fail(JPET_E_INVAL, "chunk must be 0 (auto) .. 2^20");
         g_opt_chunk = value;
@@ -702,6 +706,7 @@ int64_t jpet_get_option(const char* name) {
     if (!name) return -1;
     if (!strcmp(name, "force_direct")) return g_opt_force_direct;
     if (!strcmp(name, "chunk")) return g_opt_chunk;
+    if (!strcmp(name, "sub_tile_z")) return g_opt_sz;
     if (!strcmp(name, "time_kernel")) return g_opt_time_kernel;
     if (!strcmp(name, "last_kernel_ns")) {      // duration of the last tiled event-kernel launch (synchronises on it)
         if (!g_tk_valid || cudaEventSynchronize(g_tk1) != cudaSuccess) return -1;

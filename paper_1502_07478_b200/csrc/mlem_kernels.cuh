@@ -86,6 +86,11 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+__device__ __forceinline__ float sqrt_approx(float x) {
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 __device__ __forceinline__ void red_add_f32(float* addr, float v) {
     asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
 }
@@ -145,7 +150,7 @@ __device__ __forceinline__ EventConsts event_setup(float zu, float zd, float dl,
     EventConsts e;
     e.t = (zu - zd) * p.inv2R;                      // tan theta~
     e.sec2 = fmaf(e.t, e.t, 1.f);
-    float cos_t = rsqrtf(e.sec2);
+    float cos_t = rsqrt_approx(e.sec2);
     e.y_t = -0.5f * dl * cos_t;                     // y~
     e.z_t = fmaf(e.y_t, e.t, 0.5f * (zu + zd));     // z~
     e.fy = (e.y_t - p.y0) * p.inv_px;
@@ -156,10 +161,8 @@ __device__ __forceinline__ EventConsts event_setup(float zu, float zd, float dl,
 
 // Rows of the ellipse clipped to [row_lo, row_hi]: returns first row and count.
 __device__ __forceinline__ void event_rows(const EventConsts& e, int row_lo, int row_hi, int& iy_lo, int& nrows) {
-    float flo = fminf(fmaxf(e.fy - e.hy_px, -2.0e6f), 2.0e6f);
-    float fhi = fminf(fmaxf(e.fy + e.hy_px, -2.0e6f), 2.0e6f);
-    int lo = max(row_lo, __float2int_ru(flo));
-    int hi = min(row_hi, __float2int_rd(fhi));
+    int lo = max(row_lo, __float2int_ru(e.fy - e.hy_px));      // cvt saturates; non-finite events are dropped below
+    int hi = min(row_hi, __float2int_rd(e.fy + e.hy_px));
     iy_lo = lo;
     nrows = e.finite ? max(0, hi - lo + 1) : 0;
 }
@@ -184,12 +187,10 @@ __device__ __forceinline__ RowConsts row_setup(const EventConsts& e, int iy, int
     float dy = y - e.y_t;
     float c2 = p.c2k * e.sec2 * dy * dy;
     float rem = 9.f - c2;                                  // row chord: c1 u^2 <= 9 - c2
-    float hw = sqrtf(fmaxf(rem, 0.f) * p.half_sz2);
+    float hw = sqrt_approx(fmaxf(rem, 0.f) * p.half_sz2);
     float zc = fmaf(e.t, dy, e.z_t);                       // u = 0 on the line z = z~ + t dy
-    float flo = fminf(fmaxf((zc - hw - p.z0) * p.inv_px, -2.0e6f), 2.0e6f);
-    float fhi = fminf(fmaxf((zc + hw - p.z0) * p.inv_px, -2.0e6f), 2.0e6f);
-    int lo = max(col_lo, __float2int_ru(flo));
-    int hi = min(col_hi, __float2int_rd(fhi));
+    int lo = max(col_lo, __float2int_ru((zc - hw - p.z0) * p.inv_px));
+    int hi = min(col_hi, __float2int_rd((zc + hw - p.z0) * p.inv_px));
     int len = rem >= 0.f ? max(0, hi - lo + 1) : 0;
     if (NH > 1) {
         int part = (len + NH - 1) / NH;
@@ -375,6 +376,17 @@ __device__ __forceinline__ void smem_fma_if(uint32_t addr, float P, float inv, i
         : "memory");
 }
 
+template <int IMM>
+__device__ __forceinline__ void smem_fma(uint32_t addr, float P, float inv) {
+    asm volatile(
+        "{\n\t.reg .f32 t;\n\t"
+        "ld.shared.f32 t, [%0 + %3];\n\t"
+        "fma.rn.f32 t, %1, %2, t;\n\t"
+        "st.shared.f32 [%0 + %3], t;\n\t}"
+        ::"r"(addr), "f"(P), "f"(inv), "n"(IMM)
+        : "memory");
+}
+
 // Row constants rescaled so that the Gaussian term is -u'^2 with u' = u * sqrt(-c1s) (saves one FMUL per pixel).
 struct RowWalk {
     float u0s, c2s, betas, delta, alphas, eps;   // alphas, eps divided by sqrt(-c1s); u0s multiplied by it
@@ -408,16 +420,30 @@ __device__ __forceinline__ float kernel_value_scaled(const RowWalk& r, float jf,
     return rs * ex2_approx(e2);
 }
 
+// Slot m -> row index, central rows first (c, c+1, c-1, c+2, ...), so that the first warp gets the 32 longest
+// chords and the last one the short caps: warp-uniform loop bounds then fit the ellipse better.  Any 32
+// consecutive slots map to rows that are distinct modulo 32 (shared-memory banks).  -1: no such row.
+__device__ __forceinline__ int centre_first(int m, int nrows) {
+    const int c = nrows >> 1;
+    const int r = (m & 1) ? c + ((m + 1) >> 1) : c - (m >> 1);
+    return (r >= 0 && r < nrows) ? r : -1;
+}
+
+template <bool CF>
+__device__ __forceinline__ int row_of_slot(int m, int nrows) {
+    if (CF) return centre_first(m, nrows);
+    return m < nrows ? m : -1;
+}
+
 // One event on one CTA, tiled path.  w_addr / a_addr: 32-bit shared addresses of the region origins; pixel
 // (iy, iz) lives at base + 4 * ((iz - rz0) * HS + (iy - ry0)).  THREAD <-> ROW (part h of NH).
-template <int NW, int NH, int NR, int NJ, int HS>
+template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF>
 __device__ __forceinline__ void process_event_tiled(float zu, float zd, float dl, const DevParams& p, uint32_t w_addr,
                                                     uint32_t a_addr, int ry0, int rz0, int row_lo, int row_hi, int col_lo,
                                                     int col_hi, float* red_s, unsigned long long& my_evals,
                                                     unsigned long long& my_skipped) {
     constexpr int GT = NW * 32;
     constexpr int RT = GT / NH;                 // threads (rows) per pass
-    constexpr int U = 4;                        // pixels per branch-free block
     constexpr int NB = (NJ + U - 1) / U;
     const int tid = threadIdx.x, lane = tid & 31;
     const int h = tid / RT, k = tid - h * RT;   // row part and row slot of this thread
@@ -428,25 +454,33 @@ __device__ __forceinline__ void process_event_tiled(float zu, float zd, float dl
     event_rows(e, row_lo, row_hi, iy_lo, nrows);
 
     float preg[NR][NB * U];
-    int len[NR], wmax[NR];
+    int len[NR], wmax[NR], wmin[NR];
     uint32_t off[NR];
     float denom = 0.f;
     int cnt = 0;
 #pragma unroll
     for (int i = 0; i < NR; ++i) {
-        const int r = k + i * RT;
+        const int r = row_of_slot<CF>(k + i * RT, nrows);
         RowWalk rc;
         rc.u0s = 0.f; rc.c2s = 0.f; rc.betas = 0.f; rc.delta = 1.f; rc.alphas = 0.f; rc.eps = 0.f; rc.lo = rz0; rc.len = 0;
         int iy = ry0;
-        if (r < nrows) { iy = iy_lo + r; rc = row_walk_setup<NH>(e, iy, h, col_lo, col_hi, p); }
+        if (r >= 0) { iy = iy_lo + r; rc = row_walk_setup<NH>(e, iy, h, col_lo, col_hi, p); }
         len[i] = rc.len;
         off[i] = 4u * (uint32_t)((rc.lo - rz0) * HS + (iy - ry0));
         cnt += rc.len;
         wmax[i] = __reduce_max_sync(0xffffffffu, rc.len);
+        wmin[i] = __reduce_min_sync(0xffffffffu, rc.len);
         const uint32_t wa = w_addr + off[i];
         static_for<0, NB>([&](auto bc) {
             constexpr int jb = decltype(bc)::value * U;
-            if (jb < wmax[i]) {                                  // warp-uniform
+            if (jb + U <= wmin[i]) {                             // warp-uniform: every lane owns these pixels
+                static_for<0, U>([&](auto jc) {
+                    constexpr int j = jb + decltype(jc)::value;
+                    const float P = kernel_value_scaled(rc, (float)j, pxs);
+                    denom = fmaf(P, lds_imm<4 * j * HS>(wa), denom);
+                    preg[i][j] = P;
+                });
+            } else if (jb < wmax[i]) {                           // warp-uniform: ragged end of the rows
                 static_for<0, U>([&](auto jc) {
                     constexpr int j = jb + decltype(jc)::value;
                     float P = kernel_value_scaled(rc, (float)j, pxs);
@@ -464,7 +498,9 @@ __device__ __forceinline__ void process_event_tiled(float zu, float zd, float dl
             denom = fmaf(P, wv, denom);
         }
     }
-    for (int r = k + NR * RT; r < nrows; r += RT) {              // more rows than NR passes (not in tuned configs)
+    for (int m = k + NR * RT; m <= nrows; m += RT) {             // more rows than NR passes (not in tuned configs)
+        const int r = row_of_slot<CF>(m, nrows);
+        if (r < 0) continue;
         RowWalk rc = row_walk_setup<NH>(e, iy_lo + r, h, col_lo, col_hi, p);
         const uint32_t wa = w_addr + 4u * (uint32_t)((rc.lo - rz0) * HS + (iy_lo + r - ry0));
         cnt += rc.len;
@@ -500,7 +536,12 @@ __device__ __forceinline__ void process_event_tiled(float zu, float zd, float dl
         const uint32_t aa = a_addr + off[i];
         static_for<0, NB>([&](auto bc) {
             constexpr int jb = decltype(bc)::value * U;
-            if (jb < wmax[i]) {
+            if (jb + U <= wmin[i]) {
+                static_for<0, U>([&](auto jc) {
+                    constexpr int j = jb + decltype(jc)::value;
+                    smem_fma<4 * j * HS>(aa, preg[i][j], inv);
+                });
+            } else if (jb < wmax[i]) {
                 static_for<0, U>([&](auto jc) {
                     constexpr int j = jb + decltype(jc)::value;
                     smem_fma_if<4 * j * HS, j>(aa, preg[i][j], inv, len[i]);
@@ -508,7 +549,7 @@ __device__ __forceinline__ void process_event_tiled(float zu, float zd, float dl
             }
         });
         if (len[i] > NB * U) {
-            const int r = k + i * RT;
+            const int r = row_of_slot<CF>(k + i * RT, nrows);
             RowWalk rc = row_walk_setup<NH>(e, iy_lo + r, h, col_lo, col_hi, p);
             for (int j = NB * U; j < rc.len; ++j) {
                 float v = kernel_value_scaled(rc, (float)j, pxs) * inv, t;
@@ -518,7 +559,9 @@ __device__ __forceinline__ void process_event_tiled(float zu, float zd, float dl
             }
         }
     }
-    for (int r = k + NR * RT; r < nrows; r += RT) {
+    for (int m = k + NR * RT; m <= nrows; m += RT) {
+        const int r = row_of_slot<CF>(m, nrows);
+        if (r < 0) continue;
         RowWalk rc = row_walk_setup<NH>(e, iy_lo + r, h, col_lo, col_hi, p);
         const uint32_t aa = a_addr + 4u * (uint32_t)((rc.lo - rz0) * HS + (iy_lo + r - ry0));
         for (int j = 0; j < rc.len; ++j) {
@@ -531,8 +574,8 @@ __device__ __forceinline__ void process_event_tiled(float zu, float zd, float dl
 }
 
 // Tiled path: work items (sub-tile, chunk of sorted events), private shared-memory region per CTA.
-template <int NW, int NH, int NR, int NJ, int HS>
-__global__ void __launch_bounds__(NW * 32)
+template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF, int MINB>
+__global__ void __launch_bounds__(NW * 32, MINB)
 mlem_rows_kernel(const float* __restrict__ sorted, const WorkItem* __restrict__ items, int* __restrict__ meta,
                  const __grid_constant__ DevParams p, const float* __restrict__ wT, float* __restrict__ accT,
                  unsigned long long* __restrict__ counters) {
@@ -584,7 +627,7 @@ mlem_rows_kernel(const float* __restrict__ sorted, const WorkItem* __restrict__ 
         for (int q = 0; q < wi.count; ++q) {
             float nzu = 0.f, nzd = 0.f, ndl = 0.f;
             if (q + 1 < wi.count) { nzu = __ldg(ev + 3 * (q + 1)); nzd = __ldg(ev + 3 * (q + 1) + 1); ndl = __ldg(ev + 3 * (q + 1) + 2); }
-            process_event_tiled<NW, NH, NR, NJ, HS>(zu, zd, dl, p, w_addr, a_addr, ry0, rz0, row_lo, row_hi, col_lo, col_hi,
+            process_event_tiled<NW, NH, NR, NJ, HS, U, CF>(zu, zd, dl, p, w_addr, a_addr, ry0, rz0, row_lo, row_hi, col_lo, col_hi,
                                                     red_s[parity], my_evals, my_skipped);
             parity ^= 1;
             zu = nzu; zd = nzd; dl = ndl;

@@ -26,6 +26,7 @@ def jp():
     jp.jpet_set_option("variant", -1)
     jp.jpet_set_option("force_direct", 0)
     jp.jpet_set_option("chunk", 0)
+    jp.jpet_set_option("sub_tile_z", 0)
     jp.jpet_set_a3_coef(2.0)
 
 
