@@ -73,6 +73,49 @@ class ClockSampler(threading.Thread):
                 "reasons": reasons, "samples": len(self.rows)}
 
 
+class Ranks:
+    """One process per GPU (torchrun env: RANK / LOCAL_RANK / WORLD_SIZE / MASTER_*).  Replicas only: no collective
+    on the data path; the only exchanges are the barrier around the timed region and the max over ranks of its time."""
+
+    def __init__(self, backend: str = "nccl", device=None):
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+        self.dist = None
+        self.device = device
+        if self.world > 1:
+            import torch.distributed as dist
+
+            kwargs = {"device_id": device} if (backend == "nccl" and device is not None) else {}
+            dist.init_process_group(backend, **kwargs)
+            self.dist = dist
+
+    def seed(self, base: int) -> int:
+        return base + self.rank                      # each replica draws its own events
+
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+
+    def max(self, x: float) -> float:
+        """Max over ranks of a host float (time of the slowest replica)."""
+        if self.dist is None:
+            return float(x)
+        import torch
+
+        t = torch.tensor([x], dtype=torch.float64, device=self.device if self.device is not None else "cpu")
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def aggregate(self, per_rank_units: float, seconds_local: float) -> float:
+        """Whole-job throughput: units processed by all ranks / time of the slowest rank."""
+        return self.world * per_rank_units / self.max(seconds_local)
+
+    def close(self):
+        if self.dist is not None:
+            self.dist.destroy_process_group()
+
+
 def geom(cfg):
     return (cfg.R, cfg.L, cfg.sigma_z, cfg.sigma_dl, cfg.n_y, cfg.n_z, cfg.pixel)
 
@@ -161,17 +204,12 @@ def main():
 
     import paper_1502_07478_b200 as jp
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    ranks = Ranks("nccl", torch.device("cuda", local_rank))
+    world, rank, dist = ranks.world, ranks.rank, ranks.dist
     jp.binding.load(build_if_missing=False)
     if args.variant >= 0:
         jp.jpet_set_option("variant", args.variant)
@@ -183,7 +221,7 @@ def main():
         jp.jpet_set_option("ctas_per_sm", args.ctas_per_sm)
 
     n_events = args.events or cfg.n_events
-    events = synth.config_events(cfg, n=n_events, seed=cfg.seed + rank)     # replicas: same shape, own seed
+    events = synth.config_events(cfg, n=n_events, seed=ranks.seed(cfg.seed))     # replicas: same shape, own seed
     M = cfg.n_y * cfg.n_z
     g = geom(cfg)
     ev_d = torch.from_numpy(events).cuda()
@@ -193,8 +231,7 @@ def main():
 
     def barrier():
         torch.cuda.synchronize()
-        if dist is not None:
-            dist.barrier()
+        ranks.barrier()
         torch.cuda.synchronize()
 
     # ---- device-resident steps: CUDA events on the launching stream, L2 flushed between steps -------------
@@ -234,11 +271,7 @@ def main():
     step_ms = [a.elapsed_time(d) for a, _, _, d in pairs]
     acc_ms = [b.elapsed_time(c) for _, b, c, _ in pairs]          # binning + event kernels of the step
     kern_ms = kern_ms or acc_ms
-    total_ms = sum(step_ms)
-    if dist is not None:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = ranks.max(sum(step_ms))
     ms_per_step = total_ms / args.steps
     value = world * n_events / (ms_per_step * 1e-3)
 
@@ -256,19 +289,14 @@ def main():
         for _ in range(k_e2e):
             jp.jpet_mlem_iterate_host(ev_h, *g, rho_h, out_h)
             rho_h, out_h = out_h, rho_h
-        dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = ranks.max(time.perf_counter() - t0)
         e2e = {"value": world * n_events * k_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": int(events.nbytes + 4 * M),
                "d2h_bytes_per_step": int(4 * M), "steps": k_e2e, "ms_per_step": dt / k_e2e * 1e3,
                "timing": "host wall clock around the blocking call"}
     clocks = sampler.summary()
 
     if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
+        ranks.close()
         return
 
     # ---- roofline of the dominant kernel (mlem_events_kernel) ---------------------------------------------
@@ -302,8 +330,7 @@ def main():
             "px_per_event": n_evals / max(n_events, 1), "events_skipped": n_skipped,
             "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu_baseline, "clocks": clocks}
     print(json.dumps(line))
-    if dist is not None:
-        dist.destroy_process_group()
+    ranks.close()
 
 
 if __name__ == "__main__":

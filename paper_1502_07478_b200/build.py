@@ -30,5 +30,16 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_microbench() -> str:
+    """Roofline micro-benchmarks (FFMA, MUFU, red.global.add.f32, shared-memory RMW): csrc/microbench.cu -> csrc/microbench."""
+    out = os.path.join(CSRC, "microbench")
+    subprocess.run([nvcc_path(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", out,
+                    os.path.join(CSRC, "microbench.cu")], check=True)
+    return out
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--microbench" in sys.argv:
+        print(build_microbench())
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
