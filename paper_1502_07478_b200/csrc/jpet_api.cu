@@ -146,22 +146,26 @@ int ensure_images(int M) {
 
 // ---- event-kernel variants: NW warps per CTA, rows split in NH parts, NR row passes, NJ cached pixels,
 // HS = region row stride (compile time, so every shared-memory access has an immediate offset) ---------------
-struct Variant { int NW, NH, NR, NJ, HS, U, CF, MINB; };
+struct Variant { int NW, NH, NR, NJ, HS, U, CF, MINB, PK; };
 constexpr Variant kVariants[] = {
-    {1, 1, 1, 12, 64, 4, 1, 1},    // 0: <= 32 rows, chords <= 12 px                            (config 1)
-    {2, 1, 1, 20, 64, 4, 1, 10},   // 1: <= 64 rows, chords <= 20 px, <= 96 registers           (configs 2, 3)
-    {4, 2, 1, 12, 64, 4, 1, 1},    // 2: <= 64 rows, chords <= 24 px in two halves
-    {4, 1, 1, 36, 128, 4, 1, 1},   // 3: <= 128 rows, chords <= 36 px
-    {8, 2, 1, 20, 128, 4, 1, 1},   // 4: <= 128 rows, chords <= 40 px in two halves             (config 4)
-    {8, 2, 1, 24, 160, 4, 1, 1},   // 5: <= 128 rows, chords <= 48 px in two halves             (config 5)
-    {4, 1, 1, 44, 160, 4, 1, 1},   // 6: <= 128 rows, chords <= 44 px
-    {1, 1, 2, 20, 64, 4, 1, 1},    // 7: <= 64 rows in two passes of one warp, chords <= 20 px
+    {1, 1, 1, 12, 64, 4, 1, 1, 0},    // 0: <= 32 rows, chords <= 12 px                            (config 1)
+    {2, 1, 1, 20, 64, 4, 1, 10, 0},   // 1: <= 64 rows, chords <= 20 px, <= 96 registers           (configs 2, 3)
+    {4, 2, 1, 12, 64, 4, 1, 1, 0},    // 2: <= 64 rows, chords <= 24 px in two halves
+    {4, 1, 1, 36, 128, 4, 1, 1, 0},   // 3: <= 128 rows, chords <= 36 px
+    {8, 2, 1, 20, 128, 4, 1, 1, 0},   // 4: <= 128 rows, chords <= 40 px in two halves             (config 4)
+    {8, 2, 1, 24, 160, 4, 1, 1, 0},   // 5: <= 128 rows, chords <= 48 px in two halves
+    {4, 1, 1, 44, 160, 4, 1, 1, 0},   // 6: <= 128 rows, chords <= 44 px                           (config 5)
+    {1, 1, 2, 20, 64, 4, 1, 1, 0},    // 7: <= 64 rows in two passes of one warp, chords <= 20 px
+    {2, 1, 1, 20, 64, 4, 1, 10, 1},   // 8: as 1, packed fp32x2 arithmetic
+    {8, 2, 1, 20, 128, 4, 1, 1, 1},   // 9: as 4, packed
+    {4, 1, 1, 44, 160, 4, 1, 1, 1},   // 10: as 6, packed
+    {1, 1, 1, 12, 64, 4, 1, 1, 1},    // 11: as 0, packed
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
-template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF, int MINB>
+template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF, int MINB, bool PK>
 int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
-    auto kern = jpet::mlem_rows_kernel<NW, NH, NR, NJ, HS, U, CF, MINB>;
+    auto kern = jpet::mlem_rows_kernel<NW, NH, NR, NJ, HS, U, CF, MINB, PK>;
     if (dp.t_max >= 0.f) {     // tiled path
         if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
         static size_t attr_set = 0;
@@ -194,14 +198,18 @@ int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t
 
 int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t st) {
     switch (variant) {
-        case 0: return launch_rows<1, 1, 1, 12, 64, 4, true, 1>(bs, dp, smem, st);
-        case 1: return launch_rows<2, 1, 1, 20, 64, 4, true, 10>(bs, dp, smem, st);
-        case 2: return launch_rows<4, 2, 1, 12, 64, 4, true, 1>(bs, dp, smem, st);
-        case 3: return launch_rows<4, 1, 1, 36, 128, 4, true, 1>(bs, dp, smem, st);
-        case 4: return launch_rows<8, 2, 1, 20, 128, 4, true, 1>(bs, dp, smem, st);
-        case 5: return launch_rows<8, 2, 1, 24, 160, 4, true, 1>(bs, dp, smem, st);
-        case 6: return launch_rows<4, 1, 1, 44, 160, 4, true, 1>(bs, dp, smem, st);
-        case 7: return launch_rows<1, 1, 2, 20, 64, 4, true, 1>(bs, dp, smem, st);
+        case 0: return launch_rows<1, 1, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
+        case 1: return launch_rows<2, 1, 1, 20, 64, 4, true, 10, false>(bs, dp, smem, st);
+        case 2: return launch_rows<4, 2, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
+        case 3: return launch_rows<4, 1, 1, 36, 128, 4, true, 1, false>(bs, dp, smem, st);
+        case 4: return launch_rows<8, 2, 1, 20, 128, 4, true, 1, false>(bs, dp, smem, st);
+        case 5: return launch_rows<8, 2, 1, 24, 160, 4, true, 1, false>(bs, dp, smem, st);
+        case 6: return launch_rows<4, 1, 1, 44, 160, 4, true, 1, false>(bs, dp, smem, st);
+        case 7: return launch_rows<1, 1, 2, 20, 64, 4, true, 1, false>(bs, dp, smem, st);
+        case 8: return launch_rows<2, 1, 1, 20, 64, 4, true, 10, true>(bs, dp, smem, st);
+        case 9: return launch_rows<8, 2, 1, 20, 128, 4, true, 1, true>(bs, dp, smem, st);
+        case 10: return launch_rows<4, 1, 1, 44, 160, 4, true, 1, true>(bs, dp, smem, st);
+        case 11: return launch_rows<1, 1, 1, 12, 64, 4, true, 1, true>(bs, dp, smem, st);
         default: return fail(JPET_E_INVAL, "unknown kernel variant %d", variant);
     }
 }
@@ -247,7 +255,7 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     int v = -1;
     if (g_opt_variant >= 0) v = (int)g_opt_variant;
     else {
-        const int order[] = {0, 1, 4, 5};
+        const int order[] = {0, 8, 9, 10, 5};     // packed fp32x2 forms measured 2-9 % faster on configs 2-5
         for (int cand : order)
             if (fits(kVariants[cand])) { v = cand; break; }
         if (v < 0) v = 5;

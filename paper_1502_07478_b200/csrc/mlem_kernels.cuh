@@ -387,6 +387,37 @@ __device__ __forceinline__ void smem_fma(uint32_t addr, float P, float inv) {
         : "memory");
 }
 
+// Packed fp32x2 arithmetic (sm_100: FFMA2 / FMUL2 / FADD2 - two fp32 operations per issue slot).
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
 // Row constants rescaled so that the Gaussian term is -u'^2 with u' = u * sqrt(-c1s) (saves one FMUL per pixel).
 struct RowWalk {
     float u0s, c2s, betas, delta, alphas, eps;   // alphas, eps divided by sqrt(-c1s); u0s multiplied by it
@@ -437,7 +468,7 @@ __device__ __forceinline__ int row_of_slot(int m, int nrows) {
 
 // One event on one CTA, tiled path.  w_addr / a_addr: 32-bit shared addresses of the region origins; pixel
 // (iy, iz) lives at base + 4 * ((iz - rz0) * HS + (iy - ry0)).  THREAD <-> ROW (part h of NH).
-template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF>
+template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF, bool PK>
 __device__ __forceinline__ void process_event_tiled(float zu, float zd, float dl, const DevParams& p, uint32_t w_addr,
                                                     uint32_t a_addr, int ry0, int rz0, int row_lo, int row_hi, int col_lo,
                                                     int col_hi, float* red_s, unsigned long long& my_evals,
@@ -471,6 +502,7 @@ __device__ __forceinline__ void process_event_tiled(float zu, float zd, float dl
         wmax[i] = __reduce_max_sync(0xffffffffu, rc.len);
         wmin[i] = __reduce_min_sync(0xffffffffu, rc.len);
         const uint32_t wa = w_addr + off[i];
+        if constexpr (!PK) {
         static_for<0, NB>([&](auto bc) {
             constexpr int jb = decltype(bc)::value * U;
             if (jb + U <= wmin[i]) {                             // warp-uniform: every lane owns these pixels
@@ -491,6 +523,50 @@ __device__ __forceinline__ void process_event_tiled(float zu, float zd, float dl
                 });
             }
         });
+        } else {
+        // packed form: two adjacent pixels of the row per fp32x2 operation.  Exponent written as
+        // c2s + (bar - v)(bar + v) = c2s - v^2 + bar^2 so that no packed negation is needed.
+        static_assert(U % 2 == 0, "packed walk needs an even block");
+        const f32x2 EPS2 = pack2(rc.eps, rc.eps), DEL2 = pack2(rc.delta, rc.delta), ALP2 = pack2(rc.alphas, rc.alphas),
+                    BET2 = pack2(rc.betas, rc.betas), C2S2 = pack2(rc.c2s, rc.c2s), STEP2 = pack2(2.f * pxs, 2.f * pxs);
+        f32x2 V2 = pack2(rc.u0s, rc.u0s + pxs), DEN2 = pack2(0.f, 0.f);
+        auto pair_step = [&](auto jc, auto maskc) {
+            constexpr int j = decltype(jc)::value;
+            constexpr bool MASK = decltype(maskc)::value;
+            const f32x2 D2 = fma2(EPS2, V2, DEL2), BA2 = fma2(ALP2, V2, BET2);
+            float d0, d1;
+            unpack2(D2, d0, d1);
+            const f32x2 RS2 = pack2(rsqrt_approx(d0), rsqrt_approx(d1));
+            const f32x2 BAR2 = mul2(BA2, RS2);
+            const f32x2 E2 = fma2(add2(BAR2, V2), sub2(BAR2, V2), C2S2);
+            float e0, e1;
+            unpack2(E2, e0, e1);
+            float x0 = ex2_approx(e0), x1 = ex2_approx(e1);
+            if (MASK) {                                           // 2^e -> 0 for lanes past their span
+                x0 = j < rc.len ? x0 : 0.f;
+                x1 = j + 1 < rc.len ? x1 : 0.f;
+            }
+            const f32x2 P2 = mul2(RS2, pack2(x0, x1));
+            DEN2 = fma2(P2, pack2(lds_imm<4 * j * HS>(wa), lds_imm<4 * (j + 1) * HS>(wa)), DEN2);
+            unpack2(P2, preg[i][j], preg[i][j + 1]);
+            V2 = add2(V2, STEP2);
+        };
+        static_for<0, NB>([&](auto bc) {
+            constexpr int jb = decltype(bc)::value * U;
+            if (jb + U <= wmin[i]) {                             // warp-uniform: every lane owns these pixels
+                static_for<0, U / 2>([&](auto jc) {
+                    pair_step(std::integral_constant<int, jb + 2 * decltype(jc)::value>{}, std::false_type{});
+                });
+            } else if (jb < wmax[i]) {                           // warp-uniform: ragged end of the rows
+                static_for<0, U / 2>([&](auto jc) {
+                    pair_step(std::integral_constant<int, jb + 2 * decltype(jc)::value>{}, std::true_type{});
+                });
+            }
+        });
+        float q0, q1;
+        unpack2(DEN2, q0, q1);
+        denom += q0 + q1;
+        }
         for (int j = NB * U; j < rc.len; ++j) {                  // longer than the register cache (not in tuned configs)
             float P = kernel_value_scaled(rc, (float)j, pxs);
             float wv;
@@ -574,7 +650,7 @@ __device__ __forceinline__ void process_event_tiled(float zu, float zd, float dl
 }
 
 // Tiled path: work items (sub-tile, chunk of sorted events), private shared-memory region per CTA.
-template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF, int MINB>
+template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF, int MINB, bool PK>
 __global__ void __launch_bounds__(NW * 32, MINB)
 mlem_rows_kernel(const float* __restrict__ sorted, const WorkItem* __restrict__ items, int* __restrict__ meta,
                  const __grid_constant__ DevParams p, const float* __restrict__ wT, float* __restrict__ accT,
@@ -627,7 +703,7 @@ mlem_rows_kernel(const float* __restrict__ sorted, const WorkItem* __restrict__ 
         for (int q = 0; q < wi.count; ++q) {
             float nzu = 0.f, nzd = 0.f, ndl = 0.f;
             if (q + 1 < wi.count) { nzu = __ldg(ev + 3 * (q + 1)); nzd = __ldg(ev + 3 * (q + 1) + 1); ndl = __ldg(ev + 3 * (q + 1) + 2); }
-            process_event_tiled<NW, NH, NR, NJ, HS, U, CF>(zu, zd, dl, p, w_addr, a_addr, ry0, rz0, row_lo, row_hi, col_lo, col_hi,
+            process_event_tiled<NW, NH, NR, NJ, HS, U, CF, PK>(zu, zd, dl, p, w_addr, a_addr, ry0, rz0, row_lo, row_hi, col_lo, col_hi,
                                                     red_s[parity], my_evals, my_skipped);
             parity ^= 1;
             zu = nzu; zd = nzd; dl = ndl;
