@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "mlem_kernels.cuh"
+#include "mlem_rows2.cuh"
 
 namespace {
 
@@ -51,7 +52,8 @@ int fail(int code, const char* fmt, ...) {
 
 // One batch of events sorted by sub-tile, with its work-item list (device memory).
 struct BinSet {
-    float* sorted = nullptr;            // [n][3], regular bins first, the direct bin last
+    float* sorted = nullptr;            // [n][stride], regular bins first, the direct bin last
+    int stride = 3;                     // floats per event: 3 = raw triple, 16 = EventRec (second-generation kernel)
     jpet::WorkItem* items = nullptr;
     int* meta = nullptr;                // 0: #items, 1: direct start, 2: direct count, 3: work counter
     int64_t n = 0;
@@ -146,7 +148,9 @@ int ensure_images(int M) {
 
 // ---- event-kernel variants: NW warps per CTA, rows split in NH parts, NR row passes, NJ cached pixels,
 // HS = region row stride (compile time, so every shared-memory access has an immediate offset) ---------------
-struct Variant { int NW, NH, NR, NJ, HS, U, CF, MINB, PK; };
+// Second-generation shapes (mlem_rows2.cuh) have NA > 0: NA blocks of 32 central rows, NH parts per row, NBW = 1
+// adds the warp that takes the cap rows; NW = NA * NH + NBW.
+struct Variant { int NW, NH, NR, NJ, HS, U, CF, MINB, PK, NA, NBW; };
 constexpr Variant kVariants[] = {
     {1, 1, 1, 12, 64, 4, 1, 1, 0},    // 0: <= 32 rows, chords <= 12 px                            (config 1)
     {2, 1, 1, 20, 64, 4, 1, 10, 0},   // 1: <= 64 rows, chords <= 20 px, <= 96 registers           (configs 2, 3)
@@ -160,12 +164,22 @@ constexpr Variant kVariants[] = {
     {8, 2, 1, 20, 128, 4, 1, 1, 1},   // 9: as 4, packed
     {4, 1, 1, 44, 160, 4, 1, 1, 1},   // 10: as 6, packed
     {1, 1, 1, 12, 64, 4, 1, 1, 1},    // 11: as 0, packed
+    {2, 1, 1, 20, 64, 4, 1, 10, 1, 1, 1},    // 12: rows2, 32 central rows + cap warp, chords <= 20      (configs 2, 3)
+    {2, 1, 1, 20, 64, 4, 1, 10, 0, 1, 1},    // 13: as 12, scalar arithmetic
+    {1, 1, 1, 12, 64, 4, 1, 1, 1, 1, 0},     // 14: rows2, <= 32 rows, chords <= 12                       (config 1)
+    {7, 2, 1, 20, 128, 4, 1, 1, 1, 3, 1},    // 15: rows2, 96 central rows in halves + cap warp, chords <= 40 (config 4)
+    {8, 2, 1, 24, 160, 4, 1, 1, 1, 4, 0},    // 16: rows2, <= 128 rows in halves, chords <= 48            (config 5)
+    {8, 2, 1, 20, 128, 4, 1, 1, 1, 4, 0},    // 17: rows2, <= 128 rows in halves, chords <= 40
+    {7, 2, 1, 24, 160, 4, 1, 1, 1, 3, 1},    // 18: rows2, 96 central rows in halves + cap warp, chords <= 48
+    {4, 1, 1, 44, 160, 4, 1, 1, 1, 4, 0},    // 19: rows2, <= 128 rows, chords <= 44
+    {4, 1, 1, 36, 128, 4, 1, 1, 1, 3, 1},    // 20: rows2, 96 central rows + cap warp, chords <= 36
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
 template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF, int MINB, bool PK>
 int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
     auto kern = jpet::mlem_rows_kernel<NW, NH, NR, NJ, HS, U, CF, MINB, PK>;
+    if (bs.stride != 3) return fail(JPET_E_INVAL, "internal: first-generation kernel needs raw event triples");
     if (dp.t_max >= 0.f) {     // tiled path
         if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
         static size_t attr_set = 0;
@@ -190,7 +204,42 @@ int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t
     }
     // direct path for the events of the last bin (all events when no region fits shared memory)
     int dgrid = dp.t_max >= 0.f ? g_ws.sm_count : g_ws.sm_count * 16;
-    jpet::mlem_rows_direct_kernel<<<dgrid, 128, 0, stream>>>(bs.sorted, bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.counters);
+    jpet::mlem_rows_direct_kernel<<<dgrid, 128, 0, stream>>>(bs.sorted, bs.stride, bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.counters);
+    g_launches++;
+    CUDA_TRY(cudaGetLastError());
+    return JPET_OK;
+}
+
+template <int NA, int NH, int NBW, int NJ, int HS, int U, bool PK, int MINB>
+int launch_rows2(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
+    constexpr int NW = NA * NH + NBW;
+    auto kern = jpet::mlem_rows2_kernel<NA, NH, NBW, NJ, HS, U, PK, MINB>;
+    if (bs.stride != 16) return fail(JPET_E_INVAL, "internal: rows2 kernel needs event records");
+    if (dp.t_max >= 0.f) {
+        if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
+        static size_t attr_set = 0;
+        if (smem > 48 * 1024 && smem > attr_set) {
+            CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            attr_set = smem;
+        }
+        int per_sm = 0;
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NW * 32, smem));
+        if (per_sm < 1) return fail(JPET_E_CUDA, "event kernel does not fit on an SM (%zu B of shared memory)", smem);
+        if (g_opt_ctas_per_sm > 0) per_sm = (int)std::min<int64_t>(per_sm, g_opt_ctas_per_sm);
+        int64_t max_items = bs.n / dp.chunk + (int64_t)dp.nby * dp.nbz + 1;
+        int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(max_items, 1));
+        if (g_opt_time_kernel) {
+            if (!g_tk0) { CUDA_TRY(cudaEventCreate(&g_tk0)); CUDA_TRY(cudaEventCreate(&g_tk1)); }
+            CUDA_TRY(cudaEventRecord(g_tk0, stream));
+        }
+        kern<<<grid, NW * 32, smem, stream>>>(reinterpret_cast<const jpet::EventRec*>(bs.sorted), bs.items, bs.meta, dp,
+                                             g_ws.wT, g_ws.accT, g_ws.counters);
+        g_launches++;
+        if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk1, stream)); g_tk_valid = true; }
+        CUDA_TRY(cudaGetLastError());
+    }
+    int dgrid = dp.t_max >= 0.f ? g_ws.sm_count : g_ws.sm_count * 16;
+    jpet::mlem_rows_direct_kernel<<<dgrid, 128, 0, stream>>>(bs.sorted, bs.stride, bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.counters);
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     return JPET_OK;
@@ -210,6 +259,15 @@ int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t sme
         case 9: return launch_rows<8, 2, 1, 20, 128, 4, true, 1, true>(bs, dp, smem, st);
         case 10: return launch_rows<4, 1, 1, 44, 160, 4, true, 1, true>(bs, dp, smem, st);
         case 11: return launch_rows<1, 1, 1, 12, 64, 4, true, 1, true>(bs, dp, smem, st);
+        case 12: return launch_rows2<1, 1, 1, 20, 64, 4, true, 10>(bs, dp, smem, st);
+        case 13: return launch_rows2<1, 1, 1, 20, 64, 4, false, 10>(bs, dp, smem, st);
+        case 14: return launch_rows2<1, 1, 0, 12, 64, 4, true, 1>(bs, dp, smem, st);
+        case 15: return launch_rows2<3, 2, 1, 20, 128, 4, true, 1>(bs, dp, smem, st);
+        case 16: return launch_rows2<4, 2, 0, 24, 160, 4, true, 1>(bs, dp, smem, st);
+        case 17: return launch_rows2<4, 2, 0, 20, 128, 4, true, 1>(bs, dp, smem, st);
+        case 18: return launch_rows2<3, 2, 1, 24, 160, 4, true, 1>(bs, dp, smem, st);
+        case 19: return launch_rows2<4, 1, 0, 44, 160, 4, true, 1>(bs, dp, smem, st);
+        case 20: return launch_rows2<3, 1, 1, 36, 128, 4, true, 1>(bs, dp, smem, st);
         default: return fail(JPET_E_INVAL, "unknown kernel variant %d", variant);
     }
 }
@@ -231,6 +289,8 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     p.c1s = (float)(-LH * 2.0 * iz2);
     p.sq = (float)std::sqrt(LH * 2.0 * iz2);
     p.inv_sq = (float)(1.0 / std::sqrt(LH * 2.0 * iz2));
+    p.pxs = (float)(px * std::sqrt(LH * 2.0 * iz2));
+    p.H0p = (float)(9.0 * 0.5 * (double)sg.sigma_z * sg.sigma_z / (px * px));
     p.c2k = (float)(4.0 * il2);
     p.ak = (float)(-2.0 * iz2);
     p.bk = (float)(2.0 * a3 * il2);
@@ -250,17 +310,19 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     p.t_max = (float)t_max;
     // variant: smallest shape that holds rows_max rows, chord_max pixels per row, and the region's rows
     auto fits = [&](const Variant& c) {
+        if (c.NA > 0) return rows_max + 1 <= 32 * (c.NA + c.NBW) && chord_max + 1 <= c.NJ * c.NH && 2 * p.Hy + 4 <= c.HS;
         return rows_max + 1 <= c.NW * 32 / c.NH * c.NR && chord_max <= c.NJ * c.NH && 2 * p.Hy + 4 <= c.HS;
     };
     int v = -1;
     if (g_opt_variant >= 0) v = (int)g_opt_variant;
     else {
-        const int order[] = {0, 8, 9, 10, 5};     // packed fp32x2 forms measured 2-9 % faster on configs 2-5
+        const int order[] = {14, 12, 15, 16, 0, 8, 9, 10, 5};     // second-generation shapes first
         for (int cand : order)
             if (fits(kVariants[cand])) { v = cand; break; }
         if (v < 0) v = 5;
     }
-    const bool tiles_ok = 2 * p.Hy + 4 <= kVariants[v].HS;     // else: every event takes the direct path
+    // else: every event takes the direct path (the second-generation kernel has no overflow loops)
+    const bool tiles_ok = 2 * p.Hy + 4 <= kVariants[v].HS && (kVariants[v].NA == 0 || fits(kVariants[v]));
     p.HS = kVariants[v].HS;
     p.Sy = std::max(1, p.HS - 2 * p.Hy);
     p.Sz = g_opt_sz > 0 ? (int)g_opt_sz : 8;
@@ -289,13 +351,17 @@ bool same_problem(const jpet_geometry& g, const jpet_grid& gr) {
 
 int grid_for(int64_t M) { return (int)((M + 255) / 256); }
 
+int plan_stride() { return kVariants[g_ws.variant].NA > 0 ? 16 : 3; }
+
 int ensure_binset(BinSet& bs, int64_t n, const DevParams& dp, bool need_sorted) {
     size_t items_cap = (size_t)(n / dp.chunk) + (size_t)dp.nby * dp.nbz + 2;
-    if (need_sorted && (size_t)n > bs.cap_events) {
+    bs.stride = plan_stride();
+    const size_t need_floats = (size_t)bs.stride * (size_t)std::max<int64_t>(n, 1);
+    if (need_sorted && need_floats > bs.cap_events) {          // cap_events counts floats
         if (bs.owns_sorted) cudaFree(bs.sorted);
         bs.sorted = nullptr; bs.cap_events = 0;
-        CUDA_TRY(cudaMalloc(&bs.sorted, sizeof(float) * 3 * (size_t)std::max<int64_t>(n, 1)));
-        bs.cap_events = (size_t)n;
+        CUDA_TRY(cudaMalloc(&bs.sorted, sizeof(float) * need_floats));
+        bs.cap_events = need_floats;
         bs.owns_sorted = true;
     }
     if (items_cap > bs.cap_items) {
@@ -344,7 +410,11 @@ int bin_batch(const float* events, int64_t n, BinSet& bs, const DevParams& dp, c
     jpet::bin_scan_kernel<<<1, 1024, 0, st>>>(counts, cursors, bs.items, bs.meta, nb, dp.chunk);
     g_launches++;
     if (n > 0) {
-        jpet::bin_scatter_kernel<<<blocks, jpet::kBinBlock, hist_bytes, st>>>(events, (int)n, g_ws.bin_of, cursors, bs.sorted, nb + 1, use_smem);
+        if (bs.stride == 16)
+            jpet::bin_scatter_rec_kernel<<<blocks, jpet::kBinBlock, hist_bytes, st>>>(
+                events, (int)n, g_ws.bin_of, cursors, reinterpret_cast<jpet::EventRec*>(bs.sorted), dp, nb + 1, use_smem);
+        else
+            jpet::bin_scatter_kernel<<<blocks, jpet::kBinBlock, hist_bytes, st>>>(events, (int)n, g_ws.bin_of, cursors, bs.sorted, nb + 1, use_smem);
         g_launches++;
     }
     CUDA_TRY(cudaGetLastError());

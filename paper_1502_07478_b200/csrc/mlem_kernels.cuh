@@ -59,6 +59,8 @@ struct DevParams {
     float half_sz2;                    // sigma_z^2 / 2 = 1 / c1
     float c1s;                         // -LH * 2 iz2
     float sq, inv_sq;                  // sqrt(-c1s) and its inverse (u is rescaled so the Gaussian term is -u'^2)
+    float pxs;                         // px * sq: step of u' between neighbouring pixels of a row
+    float H0p;                         // 9 (sigma_z^2 / 2) / px^2: half chord^2 in pixels^2 is H0p + H2p dy^2
     float c2k;                         // 4 il2          (c2 = c2k * sec2 * dy^2)
     float ak;                          // -2 iz2         (alpha = ak sec2 y)
     float bk;                          // 2 k il2        (beta = bk sec2 t y dy)
@@ -729,14 +731,15 @@ mlem_rows_kernel(const float* __restrict__ sorted, const WorkItem* __restrict__ 
 // event when a region does not fit shared memory.  One warp per event, thread <-> row, w read from the global
 // transposed image, back-projection with red.global.add.f32, P recomputed in the second pass.  Simple on purpose.
 __global__ void __launch_bounds__(128)
-mlem_rows_direct_kernel(const float* __restrict__ sorted, const int* __restrict__ meta, const __grid_constant__ DevParams p,
-                        const float* __restrict__ wT, float* __restrict__ accT, unsigned long long* __restrict__ counters) {
+mlem_rows_direct_kernel(const float* __restrict__ sorted, int stride, const int* __restrict__ meta,
+                        const __grid_constant__ DevParams p, const float* __restrict__ wT, float* __restrict__ accT,
+                        unsigned long long* __restrict__ counters) {
     const int lane = threadIdx.x & 31;
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
     const int start = meta[1], count = meta[2];
     unsigned long long my_evals = 0, my_skipped = 0;
     for (int q = warp; q < count; q += n_warps) {
-        const float* ev = sorted + 3 * (size_t)(start + q);
+        const float* ev = sorted + (size_t)stride * (size_t)(start + q);      // raw triple at the head of the slot
         const EventConsts e = event_setup(__ldg(ev), __ldg(ev + 1), __ldg(ev + 2), p);
         int iy_lo, nrows;
         event_rows(e, 0, p.n_y - 1, iy_lo, nrows);
