@@ -483,19 +483,18 @@ int iterate_many(const float* events, int64_t n, const jpet_geometry* g, const j
     const float* cur = rho_start;
     const int64_t n_batches = (n + kMaxBatch - 1) / kMaxBatch;
     const bool keep = n_iter > 1;
-    if (keep) {
-        if ((size_t)n > g_ws.cap_kept_sorted) {
-            cudaFree(g_ws.kept_sorted);
-            g_ws.kept_sorted = nullptr; g_ws.cap_kept_sorted = 0;
-            CUDA_TRY(cudaMalloc(&g_ws.kept_sorted, sizeof(float) * 3 * (size_t)n));
-            g_ws.cap_kept_sorted = (size_t)n;
-        }
-        while ((int64_t)g_ws.kept.size() < n_batches) g_ws.kept.emplace_back();
-    }
+    if (keep) while ((int64_t)g_ws.kept.size() < n_batches) g_ws.kept.emplace_back();
     for (int it = 0; it < n_iter; ++it) {
         float* nxt = (it == n_iter - 1) ? rho_out : (cur == g_ws.rho_a ? g_ws.rho_b : g_ws.rho_a);
-        int rc = do_begin(g, sg, gr, cur, st);
+        int rc = do_begin(g, sg, gr, cur, st);        // fixes the plan (kernel variant, record stride) for this problem
         if (rc) return rc;
+        const size_t stride = (size_t)plan_stride();
+        if (keep && it == 0 && stride * (size_t)n > g_ws.cap_kept_sorted) {      // capacity counts floats
+            cudaFree(g_ws.kept_sorted);
+            g_ws.kept_sorted = nullptr; g_ws.cap_kept_sorted = 0;
+            CUDA_TRY(cudaMalloc(&g_ws.kept_sorted, sizeof(float) * stride * (size_t)n));
+            g_ws.cap_kept_sorted = stride * (size_t)n;
+        }
         if (!keep) {
             if ((rc = do_accumulate(events, n, st))) { g_ws.open = false; return rc; }
         } else {
@@ -504,7 +503,7 @@ int iterate_many(const float* events, int64_t n, const jpet_geometry* g, const j
                 int64_t off = b * kMaxBatch, nb = std::min(kMaxBatch, n - off);
                 if (it == 0) {
                     bs.owns_sorted = false;
-                    bs.sorted = g_ws.kept_sorted + 3 * off;
+                    bs.sorted = g_ws.kept_sorted + stride * (size_t)off;
                     if ((rc = ensure_binset(bs, nb, g_ws.dp, false))) return rc;
                     if ((rc = bin_batch(events + 3 * off, nb, bs, g_ws.dp, st))) return rc;
                 }
