@@ -14,6 +14,8 @@
 
 #include "mlem_kernels.cuh"
 #include "mlem_rows2.cuh"
+#include "mlem_rows3.cuh"
+#include "task_table.h"
 
 namespace {
 
@@ -61,6 +63,11 @@ struct BinSet {
     bool owns_sorted = true;
 };
 
+struct PlanKey {
+    jpet_geometry g; jpet_sigmas sg; jpet_grid gr; float a3;
+    int64_t variant, sz, chunk, force_direct;
+};
+
 struct Workspace {
     // problem the workspace is currently set up for
     jpet_geometry geom{0, 0};
@@ -92,6 +99,11 @@ struct Workspace {
     size_t cap_stage = 0;       // bytes
     cudaStream_t copy_stream = nullptr, compute_stream = nullptr;
     cudaEvent_t ev_copy[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
+    PlanKey plan_key{};
+    bool plan_valid = false;
+    uint32_t* tab = nullptr;    // task table of the third-generation kernel (device copy of tab_host)
+    size_t cap_tab = 0;
+    std::vector<uint32_t> tab_host, tab_uploaded;
     int sm_count = 0;
     int device = -1;
 } g_ws;
@@ -142,7 +154,7 @@ int ensure_images(int M) {
         g_ws.cap_M = M;
         g_ws.s_valid = false;
     }
-    if (!g_ws.counters) CUDA_TRY(cudaMalloc(&g_ws.counters, 2 * sizeof(unsigned long long)));
+    if (!g_ws.counters) CUDA_TRY(cudaMalloc(&g_ws.counters, 4 * sizeof(unsigned long long)));
     return JPET_OK;
 }
 
@@ -174,7 +186,23 @@ constexpr Variant kVariants[] = {
     {4, 1, 1, 44, 160, 4, 1, 1, 1, 4, 0},    // 19: rows2, <= 128 rows, chords <= 44
     {4, 1, 1, 36, 128, 4, 1, 1, 1, 3, 1},    // 20: rows2, 96 central rows + cap warp, chords <= 36
 };
-constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
+constexpr int kNumVariants2 = sizeof(kVariants) / sizeof(kVariants[0]);
+// Third-generation shapes (mlem_rows3.cuh), variant id = kNumVariants2 + index: NWE warps per event, NG event groups
+// per CTA, NJA / NJB pixel capacity of the two pieces a lane walks (NJB = 0: one piece), region row stride HS.
+struct Variant3 { int NWE, NG, NJA, NJB, HS, MINB; };
+constexpr Variant3 kVariants3[] = {
+    {1, 4, 20, 8, 64, 4},      // 21: <= 64 rows, chords <= 20 px, four independent warps per CTA      (configs 2, 3)
+    {1, 4, 12, 0, 64, 4},      // 22: <= 32 rows, chords <= 12 px                                     (config 1)
+    {4, 1, 36, 0, 128, 1},     // 23: <= 128 rows, chords <= 36 px, one row per lane                   (config 4)
+    {4, 1, 44, 0, 128, 1},     // 24: <= 128 rows, chords <= 44 px, one row per lane                   (config 5)
+    {2, 2, 36, 28, 128, 1},    // 25: <= 128 rows on two warps: 64 central rows + caps, chords <= 36
+    {1, 8, 20, 8, 64, 2},      // 26: as 21, eight warps per CTA
+    {1, 2, 20, 8, 64, 8},      // 27: as 21, two warps per CTA
+    {1, 4, 20, 8, 64, 3},      // 28: as 21, at most 3 CTAs per SM (more registers)
+    {1, 4, 20, 8, 64, 2},      // 29: as 21, at most 2 CTAs per SM
+};
+constexpr int kNumVariants3 = sizeof(kVariants3) / sizeof(kVariants3[0]);
+constexpr int kNumVariants = kNumVariants2 + kNumVariants3;
 
 template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF, int MINB, bool PK>
 int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
@@ -183,7 +211,7 @@ int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t
     if (dp.t_max >= 0.f) {     // tiled path
         if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
         static size_t attr_set = 0;
-        if (smem > 48 * 1024 && smem > attr_set) {
+        if (smem > 40 * 1024 && smem > attr_set) {
             CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             attr_set = smem;
         }
@@ -218,7 +246,7 @@ int launch_rows2(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_
     if (dp.t_max >= 0.f) {
         if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
         static size_t attr_set = 0;
-        if (smem > 48 * 1024 && smem > attr_set) {
+        if (smem > 40 * 1024 && smem > attr_set) {
             CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             attr_set = smem;
         }
@@ -245,8 +273,52 @@ int launch_rows2(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_
     return JPET_OK;
 }
 
+template <int NWE, int NG, int NJA, int NJB, int HS, int MINB>
+int launch_rows3(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
+    constexpr int NT = NWE * NG * 32;
+    auto kern = jpet::mlem_rows3_kernel<NWE, NG, NJA, NJB, HS, MINB>;
+    if (bs.stride != 16) return fail(JPET_E_INVAL, "internal: rows3 kernel needs event records");
+    if (dp.t_max >= 0.f) {
+        if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
+        static size_t attr_set = 0;
+        if (smem > 40 * 1024 && smem > attr_set) {
+            CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            attr_set = smem;
+        }
+        int per_sm = 0;
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
+        if (per_sm < 1) return fail(JPET_E_CUDA, "event kernel does not fit on an SM (%zu B of shared memory)", smem);
+        if (g_opt_ctas_per_sm > 0) per_sm = (int)std::min<int64_t>(per_sm, g_opt_ctas_per_sm);
+        int64_t max_items = bs.n / dp.chunk + (int64_t)dp.nby * dp.nbz + 1;
+        int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(max_items, 1));
+        if (g_opt_time_kernel) {
+            if (!g_tk0) { CUDA_TRY(cudaEventCreate(&g_tk0)); CUDA_TRY(cudaEventCreate(&g_tk1)); }
+            CUDA_TRY(cudaEventRecord(g_tk0, stream));
+        }
+        kern<<<grid, NT, smem, stream>>>(reinterpret_cast<const jpet::EventRec*>(bs.sorted), bs.items, bs.meta, dp, g_ws.wT,
+                                         g_ws.accT, g_ws.tab, g_ws.counters);
+        g_launches++;
+        if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk1, stream)); g_tk_valid = true; }
+        CUDA_TRY(cudaGetLastError());
+    }
+    int dgrid = dp.t_max >= 0.f ? g_ws.sm_count : g_ws.sm_count * 16;
+    jpet::mlem_rows_direct_kernel<<<dgrid, 128, 0, stream>>>(bs.sorted, bs.stride, bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.counters);
+    g_launches++;
+    CUDA_TRY(cudaGetLastError());
+    return JPET_OK;
+}
+
 int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t st) {
     switch (variant) {
+        case kNumVariants2 + 0: return launch_rows3<1, 4, 20, 8, 64, 4>(bs, dp, smem, st);
+        case kNumVariants2 + 1: return launch_rows3<1, 4, 12, 0, 64, 4>(bs, dp, smem, st);
+        case kNumVariants2 + 2: return launch_rows3<4, 1, 36, 0, 128, 1>(bs, dp, smem, st);
+        case kNumVariants2 + 3: return launch_rows3<4, 1, 44, 0, 128, 1>(bs, dp, smem, st);
+        case kNumVariants2 + 4: return launch_rows3<2, 2, 36, 28, 128, 1>(bs, dp, smem, st);
+        case kNumVariants2 + 5: return launch_rows3<1, 8, 20, 8, 64, 2>(bs, dp, smem, st);
+        case kNumVariants2 + 6: return launch_rows3<1, 2, 20, 8, 64, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 7: return launch_rows3<1, 4, 20, 8, 64, 3>(bs, dp, smem, st);
+        case kNumVariants2 + 8: return launch_rows3<1, 4, 20, 8, 64, 2>(bs, dp, smem, st);
         case 0: return launch_rows<1, 1, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
         case 1: return launch_rows<2, 1, 1, 20, 64, 4, true, 10, false>(bs, dp, smem, st);
         case 2: return launch_rows<4, 2, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
@@ -275,7 +347,7 @@ int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t sme
 // Constants of the event kernel (computed in double, rounded once), the tiling of the image into
 // sub-tiles + halo regions, and the kernel variant.
 void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& gr, float a3, DevParams* out, int* variant,
-               size_t* smem_out) {
+               size_t* smem_out, std::vector<uint32_t>* tab_out = nullptr) {
     DevParams p{};
     const double LH = 0.72134752044448170368;
     double iz2 = 1.0 / ((double)sg.sigma_z * sg.sigma_z), il2 = 1.0 / ((double)sg.sigma_dl * sg.sigma_dl);
@@ -308,40 +380,64 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     p.Hy = (int)std::ceil(hy) + 1;
     p.Hz = (int)std::ceil(hz) + 1;
     p.t_max = (float)t_max;
+    // ellipse row counts a regular event can have (unclipped): hy_px * cos(theta) for |tan theta| <= t_max, +- rounding
+    const int nr_hi = std::min(255, (int)std::floor(2.0 * hy) + 2);
+    const int nr_lo = std::max(1, (int)std::floor(2.0 * hy / std::sqrt(1.0 + t_max * t_max)) - 1);
     // variant: smallest shape that holds rows_max rows, chord_max pixels per row, and the region's rows
     auto fits = [&](const Variant& c) {
         if (c.NA > 0) return rows_max + 1 <= 32 * (c.NA + c.NBW) && chord_max + 1 <= c.NJ * c.NH && 2 * p.Hy + 4 <= c.HS;
         return rows_max + 1 <= c.NW * 32 / c.NH * c.NR && chord_max <= c.NJ * c.NH && 2 * p.Hy + 4 <= c.HS;
     };
+    std::vector<uint32_t> tab;
+    auto fits3 = [&](const Variant3& c) {
+        return 2 * p.Hy + 4 <= c.HS && jpet_host::build_task_table(nr_lo, nr_hi, (double)p.H0p, c.NWE, c.NJA, c.NJB, &tab);
+    };
     int v = -1;
     if (g_opt_variant >= 0) v = (int)g_opt_variant;
     else {
-        const int order[] = {14, 12, 15, 16, 0, 8, 9, 10, 5};     // second-generation shapes first
+        const int order3[] = {1, 0, 2, 3};                          // third-generation shapes first
+        for (int cand : order3)
+            if (fits3(kVariants3[cand])) { v = kNumVariants2 + cand; break; }
+        const int order[] = {14, 12, 15, 16, 0, 8, 9, 10, 5};
         for (int cand : order)
-            if (fits(kVariants[cand])) { v = cand; break; }
+            if (v < 0 && fits(kVariants[cand])) { v = cand; break; }
         if (v < 0) v = 5;
     }
-    // else: every event takes the direct path (the second-generation kernel has no overflow loops)
-    const bool tiles_ok = 2 * p.Hy + 4 <= kVariants[v].HS && (kVariants[v].NA == 0 || fits(kVariants[v]));
-    p.HS = kVariants[v].HS;
+    const bool gen3 = v >= kNumVariants2;
+    // else: every event takes the direct path (the later generations have no overflow loops)
+    bool tiles_ok;
+    int v_HS, v_NJ, n_regions = 2;
+    if (gen3) {
+        const Variant3& c = kVariants3[v - kNumVariants2];
+        tiles_ok = fits3(c);
+        v_HS = c.HS; v_NJ = c.NJA; n_regions = 1 + c.NG;
+        p.nr_min = nr_lo; p.nr_max = nr_hi;
+    } else {
+        tiles_ok = 2 * p.Hy + 4 <= kVariants[v].HS && (kVariants[v].NA == 0 || fits(kVariants[v]));
+        v_HS = kVariants[v].HS; v_NJ = kVariants[v].NJ;
+        p.nr_min = 0; p.nr_max = 0;
+        tab.clear();
+    }
+    p.HS = v_HS;
     p.Sy = std::max(1, p.HS - 2 * p.Hy);
     p.Sz = g_opt_sz > 0 ? (int)g_opt_sz : 8;
-    // shared memory: w region + accumulator region; shrink the sub-tile width, then give up tiling
-    const size_t budget = 200 * 1024;
+    // shared memory: w region + accumulator region(s) (+ task table); shrink the sub-tile width, then give up tiling
+    const size_t budget = 200 * 1024, tab_bytes = tab.size() * sizeof(uint32_t);
     size_t smem = 0;
     for (;;) {
         p.WZ = p.Sz + 2 * p.Hz;
-        smem = 2 * sizeof(float) * (size_t)p.HS * p.WZ;
+        smem = n_regions * sizeof(float) * (size_t)p.HS * p.WZ + tab_bytes;
         if (smem <= budget / 2 || p.Sz <= 4) break;
         p.Sz /= 2;
     }
-    if (smem > budget || !tiles_ok || p.WZ < kVariants[v].NJ + 4 || g_opt_force_direct) { p.t_max = -1.f; smem = 0; }
+    if (smem > budget || !tiles_ok || p.WZ < v_NJ + 4 || g_opt_force_direct) { p.t_max = -1.f; smem = 0; p.nr_min = p.nr_max = 0; tab.clear(); }
     p.nby = (gr.n_y + 2 * p.Hy + p.Sy - 1) / p.Sy;
     p.nbz = (gr.n_z + 2 * p.Hz + p.Sz - 1) / p.Sz;
-    p.chunk = g_opt_chunk > 0 ? (int)g_opt_chunk : 64;
+    p.chunk = g_opt_chunk > 0 ? (int)g_opt_chunk : (gen3 ? 32 * kVariants3[v - kNumVariants2].NG : 64);
     *out = p;
     *variant = v;
     *smem_out = smem;
+    if (tab_out) tab_out->swap(tab);
 }
 
 bool same_problem(const jpet_geometry& g, const jpet_grid& gr) {
@@ -351,7 +447,7 @@ bool same_problem(const jpet_geometry& g, const jpet_grid& gr) {
 
 int grid_for(int64_t M) { return (int)((M + 255) / 256); }
 
-int plan_stride() { return kVariants[g_ws.variant].NA > 0 ? 16 : 3; }
+int plan_stride() { return (g_ws.variant >= kNumVariants2 || kVariants[g_ws.variant].NA > 0) ? 16 : 3; }
 
 int ensure_binset(BinSet& bs, int64_t n, const DevParams& dp, bool need_sorted) {
     size_t items_cap = (size_t)(n / dp.chunk) + (size_t)dp.nby * dp.nbz + 2;
@@ -442,8 +538,26 @@ int do_begin(const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr,
         g_ws.geom = *g; g_ws.grid = *gr; g_ws.s_valid = true;
     }
     g_ws.sig = *sg; g_ws.M = M;
-    make_plan(*g, *sg, *gr, g_a3_coef, &g_ws.dp, &g_ws.variant, &g_ws.smem);
+    {   // the plan depends only on these inputs: rebuild it (and the task table) when one of them changes
+        const PlanKey key{*g, *sg, *gr, g_a3_coef, g_opt_variant, g_opt_sz, g_opt_chunk, g_opt_force_direct};
+        if (!g_ws.plan_valid || memcmp(&key, &g_ws.plan_key, sizeof key) != 0) {
+            make_plan(*g, *sg, *gr, g_a3_coef, &g_ws.dp, &g_ws.variant, &g_ws.smem, &g_ws.tab_host);
+            g_ws.plan_key = key;
+            g_ws.plan_valid = true;
+        }
+    }
     if (g_ws.variant < 0 || g_ws.variant >= kNumVariants) return fail(JPET_E_INVAL, "unknown kernel variant");
+    if (!g_ws.tab_host.empty() && g_ws.tab_host != g_ws.tab_uploaded) {        // task table of the third-generation kernel
+        if (g_ws.tab_host.size() > g_ws.cap_tab) {
+            cudaFree(g_ws.tab);
+            g_ws.tab = nullptr; g_ws.cap_tab = 0;
+            CUDA_TRY(cudaMalloc(&g_ws.tab, sizeof(uint32_t) * g_ws.tab_host.size()));
+            g_ws.cap_tab = g_ws.tab_host.size();
+        }
+        g_ws.tab_uploaded = g_ws.tab_host;      // the copy below reads tab_uploaded, which stays put until the next change
+        CUDA_TRY(cudaMemcpyAsync(g_ws.tab, g_ws.tab_uploaded.data(), sizeof(uint32_t) * g_ws.tab_uploaded.size(),
+                                 cudaMemcpyHostToDevice, st));
+    }
     jpet::prepass_kernel<<<grid_for(M), 256, 0, st>>>(g_ws.s, rho_in, g_ws.wT, g_ws.accT, gr->n_y, gr->n_z, g_ws.counters);
     g_launches++;
     CUDA_TRY(cudaGetLastError());
@@ -796,6 +910,11 @@ int64_t jpet_get_option(const char* name) {
     if (!strcmp(name, "last_variant")) return g_ws.variant;
     if (!strcmp(name, "last_smem_bytes")) return (int64_t)g_ws.smem;
     if (!strcmp(name, "last_tiled")) return g_ws.dp.t_max >= 0.f;
+    if (!strcmp(name, "last_overflow")) {       // pieces that exceeded their slot (0 by construction; synchronises the device)
+        unsigned long long h = 0;
+        if (!g_ws.counters || cudaMemcpy(&h, g_ws.counters + 2, sizeof h, cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+        return (int64_t)h;
+    }
     return -1;
 }
 
@@ -804,6 +923,7 @@ uint64_t jpet_launch_count(void) { return g_launches.load(); }
 void jpet_release(void) {
     cudaFree(g_ws.s); cudaFree(g_ws.wT); cudaFree(g_ws.accT); cudaFree(g_ws.rho_a); cudaFree(g_ws.rho_b);
     cudaFree(g_ws.counters); cudaFree(g_ws.stage); cudaFree(g_ws.bin_of); cudaFree(g_ws.counts); cudaFree(g_ws.kept_sorted);
+    cudaFree(g_ws.tab);
     free_binset(g_ws.scratch);
     for (auto& bs : g_ws.kept) free_binset(bs);
     for (int i = 0; i < 2; ++i) {

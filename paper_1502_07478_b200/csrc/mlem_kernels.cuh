@@ -74,6 +74,8 @@ struct DevParams {
     int nby, nbz;                      // bins cover pixel indices [-Hy, n_y + Hy) x [-Hz, n_z + Hz)
     float t_max;                       // events with |tan theta~| above this go to the direct (global) path
     int chunk;                         // events per work item
+    int nr_min, nr_max;                // third-generation kernel: ellipse row counts covered by its task table;
+                                       // nr_max > 0 makes the records carry the UNCLIPPED row range of the ellipse
 };
 
 struct WorkItem { int bin, start, count; };
@@ -123,7 +125,7 @@ __global__ void prepass_kernel(const float* __restrict__ s, const float* __restr
         wT[i] = s[src] * rho_in[src];
         accT[i] = 0.f;
     }
-    if (i < 2) counters[i] = 0ull;
+    if (i < 4) counters[i] = 0ull;
 }
 
 __global__ void finalise_kernel(const float* __restrict__ s, const float* rho_in, const float* __restrict__ accT,
@@ -234,6 +236,10 @@ __device__ __forceinline__ int event_bin(float zu, float zd, float dl, const Dev
     float fz = (e.z_t - p.z0) * p.inv_px;
     bool regular = e.finite && fabsf(e.t) <= p.t_max && e.fy >= (float)(1 - p.Hy) && e.fy < (float)(p.n_y + p.Hy - 1) &&
                    fz >= (float)(1 - p.Hz) && fz < (float)(p.n_z + p.Hz - 1);
+    if (p.nr_max > 0) {                // the row count of the whole ellipse must be one the task table knows
+        const int nr = __float2int_rd(e.fy + e.hy_px) - __float2int_ru(e.fy - e.hy_px) + 1;
+        regular = regular && nr >= p.nr_min && nr <= p.nr_max;
+    }
     if (!regular) return p.nby * p.nbz;
     int iyc = __float2int_rd(e.fy + 0.5f), izc = __float2int_rd(fz + 0.5f);
     int by = (iyc + p.Hy) / p.Sy, bz = (izc + p.Hz) / p.Sz;

@@ -60,7 +60,8 @@ __device__ __forceinline__ EventRec make_event_rec(float zu, float zd, float dl,
     r.Z0 = (e.z_t - p.z0) * p.inv_px;
     r.T1 = t * p.inv_px;
     int iy_lo, nrows;
-    event_rows(e, 0, p.n_y - 1, iy_lo, nrows);
+    if (p.nr_max > 0) event_rows(e, -(1 << 24), 1 << 24, iy_lo, nrows);     // whole ellipse (mlem_rows3.cuh clips per row)
+    else event_rows(e, 0, p.n_y - 1, iy_lo, nrows);
     r.iy_lo = iy_lo;
     r.nrows = nrows;
     return r;

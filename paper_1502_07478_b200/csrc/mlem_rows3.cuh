@@ -1,0 +1,337 @@
+// mlem_rows3.cuh - third-generation event kernel of the list-mode MLEM hot path (sm_100a).
+//
+// Same mathematics, the same sorted 64-byte event records and the same tiling as mlem_rows2_kernel (events sorted
+// by image sub-tile, w = s*rho region and private accumulator regions in shared memory, LANE <-> ELLIPSE ROW,
+// kernel values cached in registers between the denominator pass and the back-projection pass).  ncu on the
+// second generation showed the bound to be issue slots spent outside the per-pixel arithmetic: 772 warp
+// instructions per config-2 event of which about 320 are the two pixel passes; the rest is the lane -> row map,
+// row set-up repeated by two warps, the CTA barrier of the denominator and region staging.  Changes:
+//
+//   * an event is handled by a GROUP of NWE warps (1 for ellipses of up to 64 rows), several groups per CTA
+//     share one staged w region and own one accumulator region each; with NWE = 1 the event loop has no
+//     barrier at all (the denominator is a warp shuffle reduction);
+//   * every lane owns up to two PIECES of ellipse rows per event: piece A, a whole row of the central block
+//     (capacity NJA pixels), and piece B, a row or a half / quarter of a row of the caps (capacity NJB).  Which
+//     (row, part) a lane takes is read from a table indexed by the number of rows of the ellipse, built on
+//     the host from the ellipse geometry (task_table.h) and kept in shared memory - no index arithmetic;
+//   * the row constants of the two pieces are evaluated together in packed fp32x2 arithmetic;
+//   * pixel walks are nested (each block of pixels is entered only if the previous one was), pairs of pixels
+//     per fp32x2 operation, warp-uniform bounds from redux; the ragged ends of the rows are masked per pair.
+//
+// Citations are /root/reference/PAPER.md lines.  Nothing here is shared with oracle/.
+#pragma once
+#include "mlem_rows2.cuh"
+
+namespace jpet {
+
+// Table entry: bits 0-7 row (relative to the first row of the unclipped ellipse), 8-9 part, 10-11 log2(parts),
+// bit 15 valid.  Layout: [n_rows - nr_min][slot (A, B)][lane of the group].
+constexpr uint32_t kTaskValid = 1u << 15;
+
+__device__ __forceinline__ f32x2 bc2(float x) { return pack2(x, x); }
+
+struct Piece {
+    RowWalk rc;          // rc.lo / rc.len: first column and pixel count of the piece
+    uint32_t off;        // byte offset of its first pixel inside a region
+};
+
+// Span of one piece: row iy (valid or not), half chord^2 hw2 [px^2], chord centre zcp [px]; part `part` of 2^sh.
+template <int CAP, int HS>
+__device__ __forceinline__ void piece_span(uint32_t te, int iy, float hw2, float zcp, float pxs, const DevParams& p, int ry0,
+                                           int rz0, int col_lo, int col_hi, Piece& pc, int& overflow) {
+    const int part = (te >> 8) & 3, sh = (te >> 10) & 3;
+    const bool valid = (te & kTaskValid) && (unsigned)iy < (unsigned)p.n_y && hw2 >= 0.f;
+    const float hw = sqrt_approx(fmaxf(hw2, 0.f));
+    int lo = max(col_lo, __float2int_ru(zcp - hw));
+    const int hi = min(col_hi, __float2int_rd(zcp + hw));
+    int len = valid ? max(0, hi - lo + 1) : 0;
+    const int plen = (len + (1 << sh) - 1) >> sh;
+    const int first = min(len, part * plen);
+    len = min(len - first, plen);
+    lo += first;
+    overflow |= len > CAP;
+    len = min(len, CAP);                       // never taken: the table guarantees the capacity (task_table.h)
+    if (len == 0) { lo = rz0; iy = ry0; pc.rc.delta = 1.f; pc.rc.eps = 0.f; }     // idle lanes stay inside the region
+    pc.rc.u0s = ((float)lo - zcp) * pxs;
+    pc.rc.lo = lo;
+    pc.rc.len = len;
+    pc.off = 4u * (uint32_t)((lo - rz0) * HS + (iy - ry0));
+}
+
+// Row constants of pieces A and B (polynomials in dy, see mlem_rows2.cuh) in packed arithmetic, then their spans.
+template <int NJA, int NJB, int HS>
+__device__ __forceinline__ void pieces_setup(uint32_t teA, uint32_t teB, const float4 r0, const float4 r1, const float4 r2,
+                                             const float4 r3, const DevParams& p, int ry0, int rz0, int col_lo, int col_hi,
+                                             Piece& A, Piece& B, int& overflow) {
+    const int iy0 = __float_as_int(r3.z);
+    const int iyA = iy0 + (int)(teA & 0xffu), iyB = iy0 + (int)(teB & 0xffu);
+    if constexpr (NJB > 0) {
+        const f32x2 DY = fma2(pack2((float)iyA, (float)iyB), bc2(p.px), bc2(r0.x));
+        const f32x2 DY2 = mul2(DY, DY);
+        const f32x2 C2S = mul2(bc2(r0.y), DY2);
+        const f32x2 BET = mul2(DY, fma2(bc2(r0.w), DY, bc2(r0.z)));
+        const f32x2 ALP = fma2(bc2(r1.y), DY, bc2(r1.x));
+        const f32x2 EPS = fma2(bc2(r1.w), DY, bc2(r1.z));
+        const f32x2 DEL = fma2(DY, fma2(bc2(r2.z), DY, bc2(r2.y)), bc2(r2.x));
+        const f32x2 HW2 = fma2(bc2(r2.w), DY2, bc2(p.H0p));
+        const f32x2 ZCP = fma2(bc2(r3.y), DY, bc2(r3.x));
+        float hwA, hwB, zcA, zcB;
+        unpack2(C2S, A.rc.c2s, B.rc.c2s);
+        unpack2(BET, A.rc.betas, B.rc.betas);
+        unpack2(ALP, A.rc.alphas, B.rc.alphas);
+        unpack2(EPS, A.rc.eps, B.rc.eps);
+        unpack2(DEL, A.rc.delta, B.rc.delta);
+        unpack2(HW2, hwA, hwB);
+        unpack2(ZCP, zcA, zcB);
+        piece_span<NJA, HS>(teA, iyA, hwA, zcA, p.pxs, p, ry0, rz0, col_lo, col_hi, A, overflow);
+        piece_span<NJB, HS>(teB, iyB, hwB, zcB, p.pxs, p, ry0, rz0, col_lo, col_hi, B, overflow);
+    } else {
+        const float dy = fmaf((float)iyA, p.px, r0.x);
+        const float dy2 = dy * dy;
+        A.rc.c2s = r0.y * dy2;
+        A.rc.betas = dy * fmaf(r0.w, dy, r0.z);
+        A.rc.alphas = fmaf(r1.y, dy, r1.x);
+        A.rc.eps = fmaf(r1.w, dy, r1.z);
+        A.rc.delta = fmaf(dy, fmaf(r2.z, dy, r2.y), r2.x);
+        piece_span<NJA, HS>(teA, iyA, fmaf(r2.w, dy2, p.H0p), fmaf(r3.y, dy, r3.x), p.pxs, p, ry0, rz0, col_lo, col_hi, A, overflow);
+    }
+}
+
+// State of one pixel walk (pass 1): packed row constants, running u' pair and denominator pair.
+struct Walk {
+    f32x2 EPS2, DEL2, ALP2, BET2, C2S2, STEP2, V2, DEN2;
+    uint32_t wa;
+    int len;
+};
+
+// Two adjacent pixels j, j+1 of the piece: Eq. 7 (up to the constant K) and the denominator term.
+template <int J, int HS, bool MASK>
+__device__ __forceinline__ void walk_pair(Walk& s, float& p0, float& p1) {
+    const f32x2 D2 = fma2(s.EPS2, s.V2, s.DEL2), BA2 = fma2(s.ALP2, s.V2, s.BET2);
+    float d0, d1;
+    unpack2(D2, d0, d1);
+    const f32x2 RS2 = pack2(rsqrt_approx(d0), rsqrt_approx(d1));
+    const f32x2 BAR2 = mul2(BA2, RS2);
+    const f32x2 E2 = fma2(add2(BAR2, s.V2), sub2(BAR2, s.V2), s.C2S2);     // c2s - v^2 + bar^2
+    float e0, e1;
+    unpack2(E2, e0, e1);
+    float x0 = ex2_approx(e0), x1 = ex2_approx(e1);
+    if (MASK) {
+        x0 = J < s.len ? x0 : 0.f;
+        x1 = J + 1 < s.len ? x1 : 0.f;
+    }
+    const f32x2 P2 = mul2(RS2, pack2(x0, x1));
+    s.DEN2 = fma2(P2, pack2(lds_imm<4 * J * HS>(s.wa), lds_imm<4 * (J + 1) * HS>(s.wa)), s.DEN2);
+    unpack2(P2, p0, p1);
+    s.V2 = add2(s.V2, s.STEP2);
+}
+
+// Pixel walks are cut into blocks of BW pixels entered through ONE switch on the number of blocks the warp needs
+// (highest block first, falling through to block 0): no compare-and-branch between blocks - ncu showed each such
+// pair to cost the 4-warp schedulers about as much as the block's own arithmetic - and every block is one basic
+// block of BW / 2 independent pixel pairs for the scheduler to interleave.  All pairs are masked by the lane's own
+// pixel count.
+constexpr int kBW = 8;
+
+template <int JB, int NJ, int HS>
+__device__ __forceinline__ void walk_block(Walk& s, float u0s, float pxs, float (&preg)[NJ]) {
+    const float vb = fmaf((float)JB, pxs, u0s);
+    s.V2 = pack2(vb, vb + pxs);
+    static_for<0, kBW / 2>([&](auto kc) {
+        constexpr int J = JB + 2 * decltype(kc)::value;
+        if constexpr (J < NJ) walk_pair<J, HS, true>(s, preg[J], preg[J + 1]);
+    });
+}
+
+template <int NJ, int HS>
+__device__ __forceinline__ float piece_pass1(const Piece& pc, uint32_t w_addr, float pxs, int nblk, float (&preg)[NJ]) {
+    static_assert(NJ % 2 == 0 && NJ <= 6 * kBW, "pixel capacity must be even and at most 48");
+    constexpr int NB = (NJ + kBW - 1) / kBW;
+    Walk s;
+    s.EPS2 = bc2(pc.rc.eps); s.DEL2 = bc2(pc.rc.delta); s.ALP2 = bc2(pc.rc.alphas); s.BET2 = bc2(pc.rc.betas);
+    s.C2S2 = bc2(pc.rc.c2s); s.STEP2 = bc2(2.f * pxs);
+    s.DEN2 = pack2(0.f, 0.f);
+    s.wa = w_addr + pc.off;
+    s.len = pc.rc.len;
+    const float u0s = pc.rc.u0s;
+    switch (nblk) {
+        default:
+        case 6: if constexpr (NB > 5) walk_block<5 * kBW, NJ, HS>(s, u0s, pxs, preg); [[fallthrough]];
+        case 5: if constexpr (NB > 4) walk_block<4 * kBW, NJ, HS>(s, u0s, pxs, preg); [[fallthrough]];
+        case 4: if constexpr (NB > 3) walk_block<3 * kBW, NJ, HS>(s, u0s, pxs, preg); [[fallthrough]];
+        case 3: if constexpr (NB > 2) walk_block<2 * kBW, NJ, HS>(s, u0s, pxs, preg); [[fallthrough]];
+        case 2: if constexpr (NB > 1) walk_block<1 * kBW, NJ, HS>(s, u0s, pxs, preg); [[fallthrough]];
+        case 1: walk_block<0, NJ, HS>(s, u0s, pxs, preg); [[fallthrough]];
+        case 0: break;
+    }
+    float q0, q1;
+    unpack2(s.DEN2, q0, q1);
+    return q0 + q1;
+}
+
+// Pass 2: acc += P * inv over the same pixels (private region, one owner lane per pixel: plain read-modify-write).
+template <int JB, int NJ, int HS>
+__device__ __forceinline__ void scatter_block(uint32_t aa, const float (&preg)[NJ], float inv, int len) {
+    static_for<0, kBW>([&](auto kc) {
+        constexpr int J = JB + decltype(kc)::value;
+        if constexpr (J < NJ) smem_fma_if<4 * J * HS, J>(aa, preg[J], inv, len);
+    });
+}
+
+template <int NJ, int HS>
+__device__ __forceinline__ void piece_pass2(uint32_t aa, const float (&preg)[NJ], float inv, int len, int nblk) {
+    constexpr int NB = (NJ + kBW - 1) / kBW;
+    switch (nblk) {
+        default:
+        case 6: if constexpr (NB > 5) scatter_block<5 * kBW, NJ, HS>(aa, preg, inv, len); [[fallthrough]];
+        case 5: if constexpr (NB > 4) scatter_block<4 * kBW, NJ, HS>(aa, preg, inv, len); [[fallthrough]];
+        case 4: if constexpr (NB > 3) scatter_block<3 * kBW, NJ, HS>(aa, preg, inv, len); [[fallthrough]];
+        case 3: if constexpr (NB > 2) scatter_block<2 * kBW, NJ, HS>(aa, preg, inv, len); [[fallthrough]];
+        case 2: if constexpr (NB > 1) scatter_block<1 * kBW, NJ, HS>(aa, preg, inv, len); [[fallthrough]];
+        case 1: scatter_block<0, NJ, HS>(aa, preg, inv, len); [[fallthrough]];
+        case 0: break;
+    }
+}
+
+__device__ __forceinline__ void prefetch_l1(const void* ptr) {          // one 64-byte record = half a line
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(ptr));
+}
+
+__device__ __forceinline__ void named_barrier(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// One event on one group of NWE warps.  tab_n: table rows of this event's row count ([slot][lane of the group]).
+template <int NWE, int NJA, int NJB, int HS>
+__device__ __forceinline__ void process_event_rows3(const float4 r0, const float4 r1, const float4 r2, const float4 r3,
+                                                    const DevParams& p, const uint32_t* tab_n, uint32_t w_addr, uint32_t a_addr,
+                                                    int ry0, int rz0, int col_lo, int col_hi, float* red_s, int group, int glane,
+                                                    int& my_evals, int& my_skipped, int& overflow) {
+    constexpr int GL = NWE * 32;
+    const uint32_t teA = tab_n[glane];
+    const uint32_t teB = NJB > 0 ? tab_n[GL + glane] : 0u;
+    Piece A, B;
+    pieces_setup<NJA, NJB, HS>(teA, teB, r0, r1, r2, r3, p, ry0, rz0, col_lo, col_hi, A, B, overflow);
+    const int nbA = (__reduce_max_sync(0xffffffffu, A.rc.len) + kBW - 1) / kBW;
+    float pregA[NJA];
+    float denom = piece_pass1<NJA, HS>(A, w_addr, p.pxs, nbA, pregA);
+    my_evals += A.rc.len;
+    constexpr int NJB1 = NJB > 0 ? NJB : 2;
+    float pregB[NJB1];
+    int nbB = 0;
+    if constexpr (NJB > 0) {
+        nbB = (__reduce_max_sync(0xffffffffu, B.rc.len) + kBW - 1) / kBW;
+        denom += piece_pass1<NJB, HS>(B, w_addr, p.pxs, nbB, pregB);
+        my_evals += B.rc.len;
+    }
+    // ---- denominator: sum over the group -----------------------------------------------------------------------
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) denom += __shfl_xor_sync(0xffffffffu, denom, d);
+    if constexpr (NWE > 1) {
+        if ((glane & 31) == 0) red_s[glane >> 5] = denom;
+        named_barrier(1 + group, GL);
+        denom = 0.f;
+#pragma unroll
+        for (int q = 0; q < NWE; ++q) denom += red_s[q];
+    }
+    const bool ok = (denom > 0.f) && (denom < 3.0e38f);
+    if (!ok) { if (glane == 0) my_skipped += 1; return; }
+    const float inv = 1.f / denom;
+    piece_pass2<NJA, HS>(a_addr + A.off, pregA, inv, A.rc.len, nbA);
+    if constexpr (NJB > 0) piece_pass2<NJB, HS>(a_addr + B.off, pregB, inv, B.rc.len, nbB);
+}
+
+// CTA = NG groups of NWE warps.  Work item = (sub-tile, chunk of sorted events): the CTA stages w once, group g
+// takes events g, g + NG, ... of the chunk into its own accumulator region and flushes it with red.global.add.
+template <int NWE, int NG, int NJA, int NJB, int HS, int MINB>
+__global__ void __launch_bounds__(NWE * NG * 32, MINB)
+mlem_rows3_kernel(const EventRec* __restrict__ sorted, const WorkItem* __restrict__ items, int* __restrict__ meta,
+                  const __grid_constant__ DevParams p, const float* __restrict__ wT, float* __restrict__ accT,
+                  const uint32_t* __restrict__ tab, unsigned long long* __restrict__ counters) {
+    constexpr int GT = NWE * NG * 32, GL = NWE * 32;
+    extern __shared__ __align__(16) float smem[];
+    const int WZ = p.WZ, RS = HS * WZ;
+    const int tid = threadIdx.x, group = tid / GL, glane = tid - group * GL;
+    float* w_s = smem;
+    float* acc_s = smem + RS * (1 + group);
+    uint32_t* tab_s = reinterpret_cast<uint32_t*>(smem + RS * (1 + NG));
+    const uint32_t w_addr = (uint32_t)__cvta_generic_to_shared(w_s);
+    const uint32_t a_addr = (uint32_t)__cvta_generic_to_shared(acc_s);
+    __shared__ float red_s[NG][2][NWE];
+    __shared__ int item_s[2];
+    constexpr int NSLOT = NJB > 0 ? 2 : 1;
+    const int n_tab = (p.nr_max - p.nr_min + 1) * NSLOT * GL;
+    for (int i = tid; i < n_tab; i += GT) tab_s[i] = __ldg(tab + i);
+    const int n_items = meta[0];
+    int my_evals = 0, my_skipped = 0, overflow = 0;
+    unsigned long long tot_evals = 0;
+    int parity = 0, ip = 0;
+
+    while (true) {
+        if (tid == 0) item_s[ip] = atomicAdd(meta + 3, 1);
+        __syncthreads();                                   // also: every group is done with the previous w region
+        const int item = item_s[ip];
+        ip ^= 1;
+        if (item >= n_items) break;
+        const WorkItem wi = items[item];
+        const int by = wi.bin / p.nbz, bz = wi.bin - by * p.nbz;
+        const int ry0 = by * p.Sy - 2 * p.Hy, rz0 = bz * p.Sz - 2 * p.Hz;        // region origin (pixel indices)
+        const int row_lo = max(0, ry0), row_hi = min(p.n_y - 1, ry0 + HS - 1);
+        const int col_lo = max(0, rz0), col_hi = min(p.n_z - 1, rz0 + WZ - 1);
+        const float4* rec = reinterpret_cast<const float4*>(sorted + wi.start);
+        if (group < wi.count) prefetch_l1(rec + 4 * group);
+        for (int i0 = tid; i0 < RS; i0 += 4 * GT) {        // stage w: several loads in flight per thread
+            float v[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int i = i0 + q * GT;
+                const int c = i / HS, r = i - c * HS;
+                const int iz = rz0 + c, iy = ry0 + r;
+                v[q] = 0.f;
+                if (i < RS && iz >= col_lo && iz <= col_hi && iy >= row_lo && iy <= row_hi) v[q] = __ldg(wT + (size_t)iz * p.n_y + iy);
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int i = i0 + q * GT;
+                if (i < RS) w_s[i] = v[q];
+            }
+        }
+        for (int i = 4 * glane; i < RS; i += 4 * GL) *reinterpret_cast<float4*>(acc_s + i) = make_float4(0.f, 0.f, 0.f, 0.f);
+        __syncthreads();
+        for (int q = group; q < wi.count; q += NG) {
+            const float4* e = rec + 4 * q;
+            const float4 r0 = __ldg(e), r1 = __ldg(e + 1), r2 = __ldg(e + 2), r3 = __ldg(e + 3);
+            if (q + NG < wi.count) prefetch_l1(e + 4 * NG);      // next record into L1 while this event is walked
+            const int nrows = __float_as_int(r3.w);
+            const uint32_t* tab_n = tab_s + (nrows - p.nr_min) * (NSLOT * GL);
+            process_event_rows3<NWE, NJA, NJB, HS>(r0, r1, r2, r3, p, tab_n, w_addr, a_addr, ry0, rz0, col_lo, col_hi,
+                                                   red_s[group][parity], group, glane, my_evals, my_skipped, overflow);
+            parity ^= 1;
+        }
+        tot_evals += (unsigned long long)my_evals;
+        my_evals = 0;
+        if constexpr (NWE > 1) named_barrier(1 + group, GL); else __syncwarp();
+        // flush the group's region into the global transposed accumulator
+        for (int i = 4 * glane; i < RS; i += 4 * GL) {
+            const float4 v = *reinterpret_cast<const float4*>(acc_s + i);
+            const int c = i / HS, r = i - c * HS;
+            const int iz = rz0 + c, iy = ry0 + r;
+            if (iz < col_lo || iz > col_hi) continue;
+            float* dst = accT + (size_t)iz * p.n_y + iy;
+            if (v.x != 0.f && iy >= row_lo && iy <= row_hi) red_add_f32(dst, v.x);
+            if (v.y != 0.f && iy + 1 >= row_lo && iy + 1 <= row_hi) red_add_f32(dst + 1, v.y);
+            if (v.z != 0.f && iy + 2 >= row_lo && iy + 2 <= row_hi) red_add_f32(dst + 2, v.z);
+            if (v.w != 0.f && iy + 3 >= row_lo && iy + 3 <= row_hi) red_add_f32(dst + 3, v.w);
+        }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        tot_evals += __shfl_xor_sync(0xffffffffu, tot_evals, d);
+        overflow |= __shfl_xor_sync(0xffffffffu, overflow, d);
+    }
+    if ((tid & 31) == 0 && tot_evals) atomicAdd(counters + 0, tot_evals);
+    if (glane == 0 && my_skipped) atomicAdd(counters + 1, (unsigned long long)my_skipped);
+    if ((tid & 31) == 0 && overflow) atomicAdd(counters + 2, 1ull);
+}
+
+}  // namespace jpet
