@@ -279,41 +279,46 @@ bin_count_kernel(const float* __restrict__ events, int n, const __grid_constant_
     }
 }
 
-// One block: exclusive prefix of counts -> starts (and cursors), work items for the regular bins.
+// One block: exclusive prefix of counts -> starts (and cursors), work items for the regular bins.  Full items
+// (chunk events) come first in the list, the partly filled last item of every bin after them, so that the persistent
+// event kernel ends on small items.
 // meta[0] = number of items, meta[1] = start of the direct bin, meta[2] = its count, meta[3] = work counter (zeroed)
 __global__ void bin_scan_kernel(const int* __restrict__ counts, int* __restrict__ cursors, WorkItem* __restrict__ items,
                                 int* __restrict__ meta, int nb, int chunk) {
-    __shared__ int s_ev[1024], s_it[1024];
+    __shared__ int s_ev[1024], s_it[1024], s_pt[1024];
     const int tid = threadIdx.x, T = blockDim.x;
     const int per = (nb + 1 + T - 1) / T;                  // bins per thread, contiguous
     const int b0 = tid * per, b1 = min(nb + 1, b0 + per);
-    int ev = 0, it = 0;
+    int ev = 0, it = 0, pt = 0;
     for (int b = b0; b < b1; ++b) {
         int c = counts[b];
         ev += c;
-        if (b < nb) it += (c + chunk - 1) / chunk;
+        if (b < nb) { it += c / chunk; pt += (c % chunk) != 0; }
     }
-    s_ev[tid] = ev; s_it[tid] = it;
+    s_ev[tid] = ev; s_it[tid] = it; s_pt[tid] = pt;
     __syncthreads();
     for (int d = 1; d < T; d <<= 1) {                      // Hillis-Steele inclusive scan
-        int a = tid >= d ? s_ev[tid - d] : 0, c = tid >= d ? s_it[tid - d] : 0;
+        int a = tid >= d ? s_ev[tid - d] : 0, c = tid >= d ? s_it[tid - d] : 0, e = tid >= d ? s_pt[tid - d] : 0;
         __syncthreads();
-        s_ev[tid] += a; s_it[tid] += c;
+        s_ev[tid] += a; s_it[tid] += c; s_pt[tid] += e;
         __syncthreads();
     }
-    int ev_off = s_ev[tid] - ev, it_off = s_it[tid] - it;
+    const int n_full = s_it[T - 1];
+    int ev_off = s_ev[tid] - ev, it_off = s_it[tid] - it, pt_off = n_full + s_pt[tid] - pt;
     for (int b = b0; b < b1; ++b) {
         int c = counts[b];
         cursors[b] = ev_off;
         if (b < nb) {
-            for (int k = 0; k < c; k += chunk) items[it_off++] = WorkItem{b, ev_off + k, min(chunk, c - k)};
+            int k = 0;
+            for (; k + chunk <= c; k += chunk) items[it_off++] = WorkItem{b, ev_off + k, chunk};
+            if (k < c) items[pt_off++] = WorkItem{b, ev_off + k, c - k};
         } else {
             meta[1] = ev_off;
             meta[2] = c;
         }
         ev_off += c;
     }
-    if (tid == T - 1) { meta[0] = s_it[tid]; meta[3] = 0; }
+    if (tid == T - 1) { meta[0] = s_it[tid] + s_pt[tid]; meta[3] = 0; }
 }
 
 // Scatter into bin order: ranks inside the block from a shared-memory histogram, one global cursor atomic per

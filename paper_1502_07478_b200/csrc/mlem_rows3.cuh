@@ -24,8 +24,9 @@
 
 namespace jpet {
 
-// Table entry: bits 0-7 row (relative to the first row of the unclipped ellipse), 8-9 part, 10-11 log2(parts),
-// bit 15 valid.  Layout: [n_rows - nr_min][slot (A, B)][lane of the group].
+// Table: one 32-bit word per (row count of the ellipse, lane of the group): piece A in bits 0-15, piece B in bits
+// 16-31.  A 16-bit entry: bits 0-7 row (relative to the first row of the unclipped ellipse), 8-9 part,
+// 10-11 log2(parts), bit 15 valid.  Slot A only ever holds whole rows.
 constexpr uint32_t kTaskValid = 1u << 15;
 
 __device__ __forceinline__ f32x2 bc2(float x) { return pack2(x, x); }
@@ -36,19 +37,21 @@ struct Piece {
 };
 
 // Span of one piece: row iy (valid or not), half chord^2 hw2 [px^2], chord centre zcp [px]; part `part` of 2^sh.
-template <int CAP, int HS>
+template <int CAP, int HS, bool SPLIT>
 __device__ __forceinline__ void piece_span(uint32_t te, int iy, float hw2, float zcp, float pxs, const DevParams& p, int ry0,
                                            int rz0, int col_lo, int col_hi, Piece& pc, int& overflow) {
-    const int part = (te >> 8) & 3, sh = (te >> 10) & 3;
     const bool valid = (te & kTaskValid) && (unsigned)iy < (unsigned)p.n_y && hw2 >= 0.f;
     const float hw = sqrt_approx(fmaxf(hw2, 0.f));
     int lo = max(col_lo, __float2int_ru(zcp - hw));
     const int hi = min(col_hi, __float2int_rd(zcp + hw));
     int len = valid ? max(0, hi - lo + 1) : 0;
-    const int plen = (len + (1 << sh) - 1) >> sh;
-    const int first = min(len, part * plen);
-    len = min(len - first, plen);
-    lo += first;
+    if constexpr (SPLIT) {
+        const int part = (te >> 8) & 3, sh = (te >> 10) & 3;
+        const int plen = (len + (1 << sh) - 1) >> sh;
+        const int first = min(len, part * plen);
+        len = min(len - first, plen);
+        lo += first;
+    }
     overflow |= len > CAP;
     len = min(len, CAP);                       // never taken: the table guarantees the capacity (task_table.h)
     if (len == 0) { lo = rz0; iy = ry0; pc.rc.delta = 1.f; pc.rc.eps = 0.f; }     // idle lanes stay inside the region
@@ -60,10 +63,11 @@ __device__ __forceinline__ void piece_span(uint32_t te, int iy, float hw2, float
 
 // Row constants of pieces A and B (polynomials in dy, see mlem_rows2.cuh) in packed arithmetic, then their spans.
 template <int NJA, int NJB, int HS>
-__device__ __forceinline__ void pieces_setup(uint32_t teA, uint32_t teB, const float4 r0, const float4 r1, const float4 r2,
+__device__ __forceinline__ void pieces_setup(uint32_t te, const float4 r0, const float4 r1, const float4 r2,
                                              const float4 r3, const DevParams& p, int ry0, int rz0, int col_lo, int col_hi,
                                              Piece& A, Piece& B, int& overflow) {
     const int iy0 = __float_as_int(r3.z);
+    const uint32_t teA = te, teB = te >> 16;
     const int iyA = iy0 + (int)(teA & 0xffu), iyB = iy0 + (int)(teB & 0xffu);
     if constexpr (NJB > 0) {
         const f32x2 DY = fma2(pack2((float)iyA, (float)iyB), bc2(p.px), bc2(r0.x));
@@ -83,8 +87,8 @@ __device__ __forceinline__ void pieces_setup(uint32_t teA, uint32_t teB, const f
         unpack2(DEL, A.rc.delta, B.rc.delta);
         unpack2(HW2, hwA, hwB);
         unpack2(ZCP, zcA, zcB);
-        piece_span<NJA, HS>(teA, iyA, hwA, zcA, p.pxs, p, ry0, rz0, col_lo, col_hi, A, overflow);
-        piece_span<NJB, HS>(teB, iyB, hwB, zcB, p.pxs, p, ry0, rz0, col_lo, col_hi, B, overflow);
+        piece_span<NJA, HS, false>(teA, iyA, hwA, zcA, p.pxs, p, ry0, rz0, col_lo, col_hi, A, overflow);
+        piece_span<NJB, HS, true>(teB, iyB, hwB, zcB, p.pxs, p, ry0, rz0, col_lo, col_hi, B, overflow);
     } else {
         const float dy = fmaf((float)iyA, p.px, r0.x);
         const float dy2 = dy * dy;
@@ -93,7 +97,7 @@ __device__ __forceinline__ void pieces_setup(uint32_t teA, uint32_t teB, const f
         A.rc.alphas = fmaf(r1.y, dy, r1.x);
         A.rc.eps = fmaf(r1.w, dy, r1.z);
         A.rc.delta = fmaf(dy, fmaf(r2.z, dy, r2.y), r2.x);
-        piece_span<NJA, HS>(teA, iyA, fmaf(r2.w, dy2, p.H0p), fmaf(r3.y, dy, r3.x), p.pxs, p, ry0, rz0, col_lo, col_hi, A, overflow);
+        piece_span<NJA, HS, false>(teA, iyA, fmaf(r2.w, dy2, p.H0p), fmaf(r3.y, dy, r3.x), p.pxs, p, ry0, rz0, col_lo, col_hi, A, overflow);
     }
 }
 
@@ -193,25 +197,33 @@ __device__ __forceinline__ void piece_pass2(uint32_t aa, const float (&preg)[NJ]
     }
 }
 
-__device__ __forceinline__ void prefetch_l1(const void* ptr) {          // one 64-byte record = half a line
-    asm volatile("prefetch.global.L1 [%0];" ::"l"(ptr));
+// Event records travel global -> shared with cp.async into a two-slot ring per warp, one event ahead: no registers
+// are held across an event and the record is there when the warp comes back for it (an L1 prefetch hint was not:
+// ncu showed 11 % of the samples waiting on the record's first use).
+__device__ __forceinline__ void cp_async16(uint32_t saddr, const void* gptr) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ float4 lds128(uint32_t saddr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(saddr));
+    return v;
 }
 
 __device__ __forceinline__ void named_barrier(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-// One event on one group of NWE warps.  tab_n: table rows of this event's row count ([slot][lane of the group]).
+// One event on one group of NWE warps.  tab_n: table row of this event's row count ([lane of the group]).
 template <int NWE, int NJA, int NJB, int HS>
 __device__ __forceinline__ void process_event_rows3(const float4 r0, const float4 r1, const float4 r2, const float4 r3,
                                                     const DevParams& p, const uint32_t* tab_n, uint32_t w_addr, uint32_t a_addr,
                                                     int ry0, int rz0, int col_lo, int col_hi, float* red_s, int group, int glane,
                                                     int& my_evals, int& my_skipped, int& overflow) {
     constexpr int GL = NWE * 32;
-    const uint32_t teA = tab_n[glane];
-    const uint32_t teB = NJB > 0 ? tab_n[GL + glane] : 0u;
     Piece A, B;
-    pieces_setup<NJA, NJB, HS>(teA, teB, r0, r1, r2, r3, p, ry0, rz0, col_lo, col_hi, A, B, overflow);
+    pieces_setup<NJA, NJB, HS>(tab_n[glane], r0, r1, r2, r3, p, ry0, rz0, col_lo, col_hi, A, B, overflow);
     const int nbA = (__reduce_max_sync(0xffffffffu, A.rc.len) + kBW - 1) / kBW;
     float pregA[NJA];
     float denom = piece_pass1<NJA, HS>(A, w_addr, p.pxs, nbA, pregA);
@@ -259,8 +271,10 @@ mlem_rows3_kernel(const EventRec* __restrict__ sorted, const WorkItem* __restric
     const uint32_t a_addr = (uint32_t)__cvta_generic_to_shared(acc_s);
     __shared__ float red_s[NG][2][NWE];
     __shared__ int item_s[2];
-    constexpr int NSLOT = NJB > 0 ? 2 : 1;
-    const int n_tab = (p.nr_max - p.nr_min + 1) * NSLOT * GL;
+    __shared__ __align__(16) float rec_s[NWE * NG][2][16];
+    const int lane = tid & 31;
+    const uint32_t rec_addr = (uint32_t)__cvta_generic_to_shared(&rec_s[tid >> 5][0][0]);
+    const int n_tab = (p.nr_max - p.nr_min + 1) * GL;
     for (int i = tid; i < n_tab; i += GT) tab_s[i] = __ldg(tab + i);
     const int n_items = meta[0];
     int my_evals = 0, my_skipped = 0, overflow = 0;
@@ -279,7 +293,8 @@ mlem_rows3_kernel(const EventRec* __restrict__ sorted, const WorkItem* __restric
         const int row_lo = max(0, ry0), row_hi = min(p.n_y - 1, ry0 + HS - 1);
         const int col_lo = max(0, rz0), col_hi = min(p.n_z - 1, rz0 + WZ - 1);
         const float4* rec = reinterpret_cast<const float4*>(sorted + wi.start);
-        if (group < wi.count) prefetch_l1(rec + 4 * group);
+        if (group < wi.count && lane < 4) cp_async16(rec_addr + 16 * lane, rec + 4 * group + lane);      // slot 0
+        cp_async_commit();
         for (int i0 = tid; i0 < RS; i0 += 4 * GT) {        // stage w: several loads in flight per thread
             float v[4];
 #pragma unroll
@@ -298,12 +313,17 @@ mlem_rows3_kernel(const EventRec* __restrict__ sorted, const WorkItem* __restric
         }
         for (int i = 4 * glane; i < RS; i += 4 * GL) *reinterpret_cast<float4*>(acc_s + i) = make_float4(0.f, 0.f, 0.f, 0.f);
         __syncthreads();
+        uint32_t slot = 0;
         for (int q = group; q < wi.count; q += NG) {
-            const float4* e = rec + 4 * q;
-            const float4 r0 = __ldg(e), r1 = __ldg(e + 1), r2 = __ldg(e + 2), r3 = __ldg(e + 3);
-            if (q + NG < wi.count) prefetch_l1(e + 4 * NG);      // next record into L1 while this event is walked
+            cp_async_wait_all();
+            __syncwarp();
+            const uint32_t ra = rec_addr + slot;
+            const float4 r0 = lds128(ra), r1 = lds128(ra + 16), r2 = lds128(ra + 32), r3 = lds128(ra + 48);
+            slot ^= 64u;
+            if (q + NG < wi.count && lane < 4) cp_async16(rec_addr + slot + 16 * lane, rec + 4 * (q + NG) + lane);
+            cp_async_commit();
             const int nrows = __float_as_int(r3.w);
-            const uint32_t* tab_n = tab_s + (nrows - p.nr_min) * (NSLOT * GL);
+            const uint32_t* tab_n = tab_s + (nrows - p.nr_min) * GL;
             process_event_rows3<NWE, NJA, NJB, HS>(r0, r1, r2, r3, p, tab_n, w_addr, a_addr, ry0, rz0, col_lo, col_hi,
                                                    red_s[group][parity], group, glane, my_evals, my_skipped, overflow);
             parity ^= 1;

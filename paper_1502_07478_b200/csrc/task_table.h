@@ -34,14 +34,16 @@ inline int row_len_max(int n, int r, double H0p) {
     return (int)std::floor(2.0 * std::sqrt(best) + 1e-3) + 1;
 }
 
-// Builds the table [n - nr_min][slot][lane], lanes = 32 * nwe.  cap_b == 0: slot A only.  Returns false if some
-// n in [nr_min, nr_max] does not fit the shape (too many rows, a chord longer than a slot).
+// Builds the table [n - nr_min][lane], lanes = 32 * nwe: slot A in bits 0-15 of a word, slot B in bits 16-31.
+// cap_b == 0: slot A only.  Returns false if some n in [nr_min, nr_max] does not fit the shape (too many rows, a
+// chord longer than a slot).
 inline bool build_task_table(int nr_min, int nr_max, double H0p, int nwe, int cap_a, int cap_b, std::vector<uint32_t>* out) {
-    const int lanes = 32 * nwe, nslot = cap_b > 0 ? 2 : 1;
-    out->assign((size_t)(nr_max - nr_min + 1) * nslot * lanes, 0u);
+    const int lanes = 32 * nwe;
+    out->assign((size_t)(nr_max - nr_min + 1) * lanes, 0u);
+    std::vector<uint32_t> A(lanes), B(lanes);
     for (int n = nr_min; n <= nr_max; ++n) {
-        uint32_t* A = out->data() + (size_t)(n - nr_min) * nslot * lanes;
-        uint32_t* B = A + lanes;
+        std::fill(A.begin(), A.end(), 0u);
+        std::fill(B.begin(), B.end(), 0u);
         if (n > 255) return false;
         const int na = std::min(n, lanes);
         const int a0 = (n - na + 1) / 2;                       // central block [a0, a0 + na)
@@ -89,6 +91,8 @@ inline bool build_task_table(int nr_min, int nr_max, double H0p, int nwe, int ca
                 }
             }
         }
+        uint32_t* W = out->data() + (size_t)(n - nr_min) * lanes;
+        for (int q = 0; q < lanes; ++q) W[q] = A[q] | (B[q] << 16);
     }
     return true;
 }
