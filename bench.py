@@ -308,7 +308,7 @@ def main():
     peak_evals = n_sm * 8.0 * sm_mhz_peak * 1e6
     kern_s = statistics.mean(kern_ms) * 1e-3
     achieved = n_evals / kern_s
-    roofline = {"bound": "alu", "kernel": "mlem_rows_kernel", "achieved": achieved / 1e9, "peak": peak_evals / 1e9,
+    roofline = {"bound": "alu", "kernel": "mlem_rows3_kernel", "achieved": achieved / 1e9, "peak": peak_evals / 1e9,
                 "unit": "Geval/s", "frac": achieved / peak_evals, "traffic": None,
                 "peak_source": f"{n_sm} SMs x 16 MUFU/clk / 2 MUFU per eval x {sm_mhz_peak:.0f} MHz ({peak_kind} sm_max_mhz)",
                 "kernel_ms": kern_s * 1e3, "kernel_share_of_step": statistics.mean(kern_ms) / statistics.mean(step_ms),

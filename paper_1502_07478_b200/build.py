@@ -9,7 +9,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libjpet.so")
 SOURCES = [os.path.join(CSRC, "jpet_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "mlem_kernels.cuh"), os.path.join(CSRC, "mlem_rows2.cuh"), os.path.join(os.path.dirname(_HERE), "include", "jpet.h")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("mlem_kernels.cuh", "mlem_rows2.cuh", "mlem_rows3.cuh", "task_table.h")] + [
+    os.path.join(os.path.dirname(_HERE), "include", "jpet.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math",
               "-Xcompiler", "-fPIC", "-shared"]
 

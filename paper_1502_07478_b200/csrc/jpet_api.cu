@@ -28,9 +28,10 @@ int64_t g_opt_force_direct = 0;  // 1 = every event takes the direct (global-mem
 int64_t g_opt_chunk = 0;         // events per work item, 0 = automatic
 int64_t g_opt_sz = 0;            // sub-tile width in pixels, 0 = automatic
 int64_t g_opt_time_kernel = 0;   // 1 = bracket the tiled event kernel with CUDA events (bench.py's roofline)
-cudaEvent_t g_tk0 = nullptr, g_tk1 = nullptr;
-bool g_tk_valid = false;
+std::vector<cudaEvent_t> g_tk;    // event pairs around the tiled event kernel launches since the last begin
+size_t g_tk_used = 0;
 int64_t g_opt_variant = -1;      // -1 = automatic
+int64_t g_opt_poly_off = 0;      // 1 = never pick a polynomial-exponent variant automatically
 int64_t g_opt_ctas_per_sm = 0;   // 0 = automatic
 constexpr int64_t kMaxBatch = 10000000;          // events per launch (BASELINE config 5: 10M-event batches)
 constexpr int64_t kStageBytes = 4ll << 30;       // device staging budget of the host-buffer calls
@@ -189,18 +190,43 @@ constexpr Variant kVariants[] = {
 constexpr int kNumVariants2 = sizeof(kVariants) / sizeof(kVariants[0]);
 // Third-generation shapes (mlem_rows3.cuh), variant id = kNumVariants2 + index: NWE warps per event, NG event groups
 // per CTA, NJA / NJB pixel capacity of the two pieces a lane walks (NJB = 0: one piece), region row stride HS.
-struct Variant3 { int NWE, NG, NJA, NJB, HS, MINB; };
+// DEG: 0 = closed form (rsqrt + ex2 per pixel), 4 / 5 = exponent as a polynomial in u (one ex2 per pixel; make_plan
+// bounds the truncation error and picks the degree); BW: pixels per block of the walks.
+struct Variant3 { int NWE, NG, NJA, NJB, HS, MINB, DEG, BW; };
 constexpr Variant3 kVariants3[] = {
-    {1, 4, 20, 8, 64, 4},      // 21: <= 64 rows, chords <= 20 px, four independent warps per CTA      (configs 2, 3)
-    {1, 4, 12, 0, 64, 4},      // 22: <= 32 rows, chords <= 12 px                                     (config 1)
-    {4, 1, 36, 0, 128, 1},     // 23: <= 128 rows, chords <= 36 px, one row per lane                   (config 4)
-    {4, 1, 44, 0, 128, 1},     // 24: <= 128 rows, chords <= 44 px, one row per lane                   (config 5)
-    {2, 2, 36, 28, 128, 1},    // 25: <= 128 rows on two warps: 64 central rows + caps, chords <= 36
-    {1, 8, 20, 8, 64, 2},      // 26: as 21, eight warps per CTA
-    {1, 2, 20, 8, 64, 8},      // 27: as 21, two warps per CTA
-    {1, 4, 20, 8, 64, 3},      // 28: as 21, at most 3 CTAs per SM (more registers)
-    {1, 4, 20, 8, 64, 2},      // 29: as 21, at most 2 CTAs per SM
+    {1, 4, 20, 8, 64, 4, 0, 8},      // 21: <= 64 rows, chords <= 20 px, four independent warps per CTA      (configs 2, 3)
+    {1, 4, 12, 0, 64, 4, 0, 8},      // 22: <= 32 rows, chords <= 12 px                                     (config 1)
+    {4, 1, 36, 0, 128, 1, 0, 8},     // 23: <= 128 rows, chords <= 36 px, one row per lane                   (config 4)
+    {4, 1, 44, 0, 128, 1, 0, 8},     // 24: <= 128 rows, chords <= 44 px, one row per lane                   (config 5)
+    {2, 2, 36, 28, 128, 1, 0, 8},    // 25: <= 128 rows on two warps: 64 central rows + caps, chords <= 36
+    {1, 8, 20, 8, 64, 2, 0, 8},      // 26: as 21, eight warps per CTA
+    {1, 2, 20, 8, 64, 8, 0, 8},      // 27: as 21, two warps per CTA
+    {1, 4, 20, 8, 64, 3, 0, 8},      // 28: as 21, at most 3 CTAs per SM (more registers)
+    {1, 4, 20, 8, 64, 2, 0, 8},      // 29: as 21, at most 2 CTAs per SM
+    {1, 4, 20, 8, 64, 4, 4, 4},      // 30: as 21, polynomial exponent of degree 4, blocks of 4          (configs 2, 3)
+    {1, 4, 12, 0, 64, 4, 4, 4},      // 31: as 22, degree 4                                              (config 1)
+    {4, 1, 36, 0, 128, 1, 5, 8},     // 32: as 23, degree 5                                              (config 4)
+    {4, 1, 44, 0, 128, 1, 4, 8},     // 33: as 24, degree 4                                              (config 5)
+    {1, 4, 20, 8, 64, 4, 5, 4},      // 34: as 30, degree 5
+    {1, 4, 12, 0, 64, 4, 5, 4},      // 35: as 31, degree 5
+    {4, 1, 36, 0, 128, 1, 4, 8},     // 36: as 32, degree 4
+    {4, 1, 44, 0, 128, 1, 5, 8},     // 37: as 33, degree 5
+    {1, 4, 20, 8, 64, 4, 4, 8},      // 38: as 30, blocks of 8
+    {1, 4, 20, 8, 64, 4, 0, 4},      // 39: as 21, blocks of 4
+    {1, 4, 12, 0, 64, 4, 4, 8},      // 40: as 31, blocks of 8
+    {1, 4, 12, 0, 64, 4, 5, 8},      // 41: as 40, degree 5
+    {1, 4, 20, 8, 64, 4, 5, 8},      // 42: as 38, degree 5
+    {4, 4, 36, 0, 128, 1, 5, 8},     // 43: as 32, four event groups per CTA (one CTA of 16 warps per SM)
+    {4, 4, 44, 0, 128, 1, 4, 8},     // 44: as 33, four event groups per CTA
+    {4, 3, 36, 0, 128, 1, 5, 8},     // 45: as 32, three event groups per CTA
+    {4, 3, 44, 0, 128, 1, 4, 8},     // 46: as 33, three event groups per CTA
+    {4, 4, 36, 0, 128, 1, 0, 8},     // 47: as 43, closed form
+    {4, 4, 44, 0, 128, 1, 0, 8},     // 48: as 44, closed form
+    {4, 4, 36, 0, 128, 1, 4, 8},     // 49: as 43, degree 4
+    {4, 4, 44, 0, 128, 1, 5, 8},     // 50: as 44, degree 5
 };
+// shapes in order of size: closed-form / degree-4 / degree-5 instances of each
+constexpr int kShape3[4][3] = {{1, 19, 20}, {0, 17, 21}, {26, 28, 22}, {27, 23, 29}};
 constexpr int kNumVariants3 = sizeof(kVariants3) / sizeof(kVariants3[0]);
 constexpr int kNumVariants = kNumVariants2 + kNumVariants3;
 
@@ -222,12 +248,15 @@ int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t
         int64_t max_items = bs.n / dp.chunk + (int64_t)dp.nby * dp.nbz + 1;
         int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(max_items, 1));
         if (g_opt_time_kernel) {
-            if (!g_tk0) { CUDA_TRY(cudaEventCreate(&g_tk0)); CUDA_TRY(cudaEventCreate(&g_tk1)); }
-            CUDA_TRY(cudaEventRecord(g_tk0, stream));
+            if (g_tk_used + 2 > g_tk.size()) {
+                g_tk.resize(g_tk_used + 2, nullptr);
+                CUDA_TRY(cudaEventCreate(&g_tk[g_tk_used])); CUDA_TRY(cudaEventCreate(&g_tk[g_tk_used + 1]));
+            }
+            CUDA_TRY(cudaEventRecord(g_tk[g_tk_used], stream));
         }
         kern<<<grid, NW * 32, smem, stream>>>(bs.sorted, bs.items, bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.counters);
         g_launches++;
-        if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk1, stream)); g_tk_valid = true; }
+        if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk[g_tk_used + 1], stream)); g_tk_used += 2; }
         CUDA_TRY(cudaGetLastError());
     }
     // direct path for the events of the last bin (all events when no region fits shared memory)
@@ -257,13 +286,16 @@ int launch_rows2(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_
         int64_t max_items = bs.n / dp.chunk + (int64_t)dp.nby * dp.nbz + 1;
         int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(max_items, 1));
         if (g_opt_time_kernel) {
-            if (!g_tk0) { CUDA_TRY(cudaEventCreate(&g_tk0)); CUDA_TRY(cudaEventCreate(&g_tk1)); }
-            CUDA_TRY(cudaEventRecord(g_tk0, stream));
+            if (g_tk_used + 2 > g_tk.size()) {
+                g_tk.resize(g_tk_used + 2, nullptr);
+                CUDA_TRY(cudaEventCreate(&g_tk[g_tk_used])); CUDA_TRY(cudaEventCreate(&g_tk[g_tk_used + 1]));
+            }
+            CUDA_TRY(cudaEventRecord(g_tk[g_tk_used], stream));
         }
         kern<<<grid, NW * 32, smem, stream>>>(reinterpret_cast<const jpet::EventRec*>(bs.sorted), bs.items, bs.meta, dp,
                                              g_ws.wT, g_ws.accT, g_ws.counters);
         g_launches++;
-        if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk1, stream)); g_tk_valid = true; }
+        if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk[g_tk_used + 1], stream)); g_tk_used += 2; }
         CUDA_TRY(cudaGetLastError());
     }
     int dgrid = dp.t_max >= 0.f ? g_ws.sm_count : g_ws.sm_count * 16;
@@ -273,10 +305,10 @@ int launch_rows2(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_
     return JPET_OK;
 }
 
-template <int NWE, int NG, int NJA, int NJB, int HS, int MINB>
+template <int NWE, int NG, int NJA, int NJB, int HS, int MINB, int DEG, int BW>
 int launch_rows3(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
     constexpr int NT = NWE * NG * 32;
-    auto kern = jpet::mlem_rows3_kernel<NWE, NG, NJA, NJB, HS, MINB>;
+    auto kern = jpet::mlem_rows3_kernel<NWE, NG, NJA, NJB, HS, MINB, DEG, BW>;
     if (bs.stride != 16) return fail(JPET_E_INVAL, "internal: rows3 kernel needs event records");
     if (dp.t_max >= 0.f) {
         if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
@@ -292,13 +324,16 @@ int launch_rows3(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_
         int64_t max_items = bs.n / dp.chunk + (int64_t)dp.nby * dp.nbz + 1;
         int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(max_items, 1));
         if (g_opt_time_kernel) {
-            if (!g_tk0) { CUDA_TRY(cudaEventCreate(&g_tk0)); CUDA_TRY(cudaEventCreate(&g_tk1)); }
-            CUDA_TRY(cudaEventRecord(g_tk0, stream));
+            if (g_tk_used + 2 > g_tk.size()) {
+                g_tk.resize(g_tk_used + 2, nullptr);
+                CUDA_TRY(cudaEventCreate(&g_tk[g_tk_used])); CUDA_TRY(cudaEventCreate(&g_tk[g_tk_used + 1]));
+            }
+            CUDA_TRY(cudaEventRecord(g_tk[g_tk_used], stream));
         }
         kern<<<grid, NT, smem, stream>>>(reinterpret_cast<const jpet::EventRec*>(bs.sorted), bs.items, bs.meta, dp, g_ws.wT,
                                          g_ws.accT, g_ws.tab, g_ws.counters);
         g_launches++;
-        if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk1, stream)); g_tk_valid = true; }
+        if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk[g_tk_used + 1], stream)); g_tk_used += 2; }
         CUDA_TRY(cudaGetLastError());
     }
     int dgrid = dp.t_max >= 0.f ? g_ws.sm_count : g_ws.sm_count * 16;
@@ -310,15 +345,36 @@ int launch_rows3(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_
 
 int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t st) {
     switch (variant) {
-        case kNumVariants2 + 0: return launch_rows3<1, 4, 20, 8, 64, 4>(bs, dp, smem, st);
-        case kNumVariants2 + 1: return launch_rows3<1, 4, 12, 0, 64, 4>(bs, dp, smem, st);
-        case kNumVariants2 + 2: return launch_rows3<4, 1, 36, 0, 128, 1>(bs, dp, smem, st);
-        case kNumVariants2 + 3: return launch_rows3<4, 1, 44, 0, 128, 1>(bs, dp, smem, st);
-        case kNumVariants2 + 4: return launch_rows3<2, 2, 36, 28, 128, 1>(bs, dp, smem, st);
-        case kNumVariants2 + 5: return launch_rows3<1, 8, 20, 8, 64, 2>(bs, dp, smem, st);
-        case kNumVariants2 + 6: return launch_rows3<1, 2, 20, 8, 64, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 7: return launch_rows3<1, 4, 20, 8, 64, 3>(bs, dp, smem, st);
-        case kNumVariants2 + 8: return launch_rows3<1, 4, 20, 8, 64, 2>(bs, dp, smem, st);
+        case kNumVariants2 + 0: return launch_rows3<1, 4, 20, 8, 64, 4, 0, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 1: return launch_rows3<1, 4, 12, 0, 64, 4, 0, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 2: return launch_rows3<4, 1, 36, 0, 128, 1, 0, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 3: return launch_rows3<4, 1, 44, 0, 128, 1, 0, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 4: return launch_rows3<2, 2, 36, 28, 128, 1, 0, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 5: return launch_rows3<1, 8, 20, 8, 64, 2, 0, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 6: return launch_rows3<1, 2, 20, 8, 64, 8, 0, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 7: return launch_rows3<1, 4, 20, 8, 64, 3, 0, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 8: return launch_rows3<1, 4, 20, 8, 64, 2, 0, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 9: return launch_rows3<1, 4, 20, 8, 64, 4, 4, 4>(bs, dp, smem, st);
+        case kNumVariants2 + 10: return launch_rows3<1, 4, 12, 0, 64, 4, 4, 4>(bs, dp, smem, st);
+        case kNumVariants2 + 11: return launch_rows3<4, 1, 36, 0, 128, 1, 5, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 12: return launch_rows3<4, 1, 44, 0, 128, 1, 4, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 13: return launch_rows3<1, 4, 20, 8, 64, 4, 5, 4>(bs, dp, smem, st);
+        case kNumVariants2 + 14: return launch_rows3<1, 4, 12, 0, 64, 4, 5, 4>(bs, dp, smem, st);
+        case kNumVariants2 + 15: return launch_rows3<4, 1, 36, 0, 128, 1, 4, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 16: return launch_rows3<4, 1, 44, 0, 128, 1, 5, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 17: return launch_rows3<1, 4, 20, 8, 64, 4, 4, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 18: return launch_rows3<1, 4, 20, 8, 64, 4, 0, 4>(bs, dp, smem, st);
+        case kNumVariants2 + 19: return launch_rows3<1, 4, 12, 0, 64, 4, 4, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 20: return launch_rows3<1, 4, 12, 0, 64, 4, 5, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 21: return launch_rows3<1, 4, 20, 8, 64, 4, 5, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 22: return launch_rows3<4, 4, 36, 0, 128, 1, 5, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 23: return launch_rows3<4, 4, 44, 0, 128, 1, 4, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 24: return launch_rows3<4, 3, 36, 0, 128, 1, 5, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 25: return launch_rows3<4, 3, 44, 0, 128, 1, 4, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 26: return launch_rows3<4, 4, 36, 0, 128, 1, 0, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 27: return launch_rows3<4, 4, 44, 0, 128, 1, 0, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 28: return launch_rows3<4, 4, 36, 0, 128, 1, 4, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 29: return launch_rows3<4, 4, 44, 0, 128, 1, 5, 8>(bs, dp, smem, st);
         case 0: return launch_rows<1, 1, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
         case 1: return launch_rows<2, 1, 1, 20, 64, 4, true, 10, false>(bs, dp, smem, st);
         case 2: return launch_rows<4, 2, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
@@ -395,9 +451,17 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     int v = -1;
     if (g_opt_variant >= 0) v = (int)g_opt_variant;
     else {
-        const int order3[] = {1, 0, 2, 3};                          // third-generation shapes first
-        for (int cand : order3)
-            if (fits3(kVariants3[cand])) { v = kNumVariants2 + cand; break; }
+        // third-generation shapes first; degree of the exponent polynomial from the truncation bound (mlem_rows3.cuh,
+        // poly_coeffs2): |x| = |eps u / delta| <= xb, ba^2 / D <= eb inside the ellipse and the image
+        const double y_max = 0.5 * gr.n_y * px, u_max = 3.0 * sg.sigma_z / std::sqrt(2.0), R2 = (double)g.R * g.R;
+        const double xb = 2.0 * (t_max / (1.0 + t_max * t_max)) * y_max * u_max / (R2 + y_max * y_max) / 0.95;
+        const double eb = 1.1 * 9.0 * y_max * y_max / (R2 + y_max * y_max);
+        auto trunc_err = [&](int deg) {      // log2 units
+            return 1.4427 * (0.5 * eb * std::pow(xb, deg - 1) / (1.0 - xb) + 0.5 * std::pow(xb, deg + 1) / (deg + 1));
+        };
+        const int deg_sel = g_opt_poly_off ? 0 : (trunc_err(4) <= 2e-5 ? 1 : (trunc_err(5) <= 2e-5 ? 2 : 0));
+        for (int sh = 0; sh < 4 && v < 0; ++sh)
+            if (fits3(kVariants3[kShape3[sh][deg_sel]])) v = kNumVariants2 + kShape3[sh][deg_sel];
         const int order[] = {14, 12, 15, 16, 0, 8, 9, 10, 5};
         for (int cand : order)
             if (v < 0 && fits(kVariants[cand])) { v = cand; break; }
@@ -420,15 +484,23 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     }
     p.HS = v_HS;
     p.Sy = std::max(1, p.HS - 2 * p.Hy);
-    p.Sz = g_opt_sz > 0 ? (int)g_opt_sz : 8;
-    // shared memory: w region + accumulator region(s) (+ task table); shrink the sub-tile width, then give up tiling
-    const size_t budget = 200 * 1024, tab_bytes = tab.size() * sizeof(uint32_t);
+    // shared memory: w region + accumulator region(s) (+ task table).  The sub-tile width Sz (8 or 4 columns) is the
+    // one that lets most warps live on an SM (228 KB per SM, 1 KB reserved per CTA, 227 KB per CTA); 8 on a tie.
+    const size_t budget = 225 * 1024, sm_bytes = 228 * 1024, tab_bytes = tab.size() * sizeof(uint32_t);
+    const int cta_warps = gen3 ? kVariants3[v - kNumVariants2].NWE * kVariants3[v - kNumVariants2].NG : kVariants[v].NW;
     size_t smem = 0;
-    for (;;) {
+    {
+        int best_sz = 4;
+        size_t best_warps = 0;
+        for (int sz : {8, 4}) {
+            if (g_opt_sz > 0) sz = (int)g_opt_sz;
+            const size_t need = n_regions * sizeof(float) * (size_t)p.HS * (sz + 2 * p.Hz) + tab_bytes;
+            const size_t ctas = need <= budget ? std::min<size_t>(sm_bytes / (need + 2048), 2048 / (32 * cta_warps)) : 0;
+            if (ctas * cta_warps > best_warps) { best_warps = ctas * cta_warps; best_sz = sz; }
+        }
+        p.Sz = best_sz;
         p.WZ = p.Sz + 2 * p.Hz;
         smem = n_regions * sizeof(float) * (size_t)p.HS * p.WZ + tab_bytes;
-        if (smem <= budget / 2 || p.Sz <= 4) break;
-        p.Sz /= 2;
     }
     if (smem > budget || !tiles_ok || p.WZ < v_NJ + 4 || g_opt_force_direct) { p.t_max = -1.f; smem = 0; p.nr_min = p.nr_max = 0; tab.clear(); }
     p.nby = (gr.n_y + 2 * p.Hy + p.Sy - 1) / p.Sy;
@@ -539,7 +611,7 @@ int do_begin(const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr,
     }
     g_ws.sig = *sg; g_ws.M = M;
     {   // the plan depends only on these inputs: rebuild it (and the task table) when one of them changes
-        const PlanKey key{*g, *sg, *gr, g_a3_coef, g_opt_variant, g_opt_sz, g_opt_chunk, g_opt_force_direct};
+        const PlanKey key{*g, *sg, *gr, g_a3_coef, g_opt_variant, g_opt_sz, g_opt_chunk, g_opt_force_direct + 2 * g_opt_poly_off};
         if (!g_ws.plan_valid || memcmp(&key, &g_ws.plan_key, sizeof key) != 0) {
             make_plan(*g, *sg, *gr, g_a3_coef, &g_ws.dp, &g_ws.variant, &g_ws.smem, &g_ws.tab_host);
             g_ws.plan_key = key;
@@ -558,6 +630,7 @@ int do_begin(const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr,
         CUDA_TRY(cudaMemcpyAsync(g_ws.tab, g_ws.tab_uploaded.data(), sizeof(uint32_t) * g_ws.tab_uploaded.size(),
                                  cudaMemcpyHostToDevice, st));
     }
+    g_tk_used = 0;                 // last_kernel_ns covers the event-kernel launches of one iteration
     jpet::prepass_kernel<<<grid_for(M), 256, 0, st>>>(g_ws.s, rho_in, g_ws.wT, g_ws.accT, gr->n_y, gr->n_z, g_ws.counters);
     g_launches++;
     CUDA_TRY(cudaGetLastError());
@@ -874,7 +947,7 @@ int jpet_set_option(const char* name, int64_t value) {
     } else if (!strcmp(name, "time_kernel")) {
         if (value < 0 || value > 1) return fail(JPET_E_INVAL, "time_kernel must be 0 or 1");
         g_opt_time_kernel = value;
-        g_tk_valid = false;
+        g_tk_used = 0;
     } else if (!strcmp(name, "sub_tile_z")) {
         if (value < 0 || value > 256) return fail(JPET_E_INVAL, "sub_tile_z must be 0 (auto) .. 256");
         g_opt_sz = value;
@@ -884,6 +957,8 @@ int jpet_set_option(const char* name, int64_t value) {
     } else if (!strcmp(name, "variant")) {
         if (value < -1 || value >= kNumVariants) return fail(JPET_E_INVAL, "variant must be -1 (auto) .. %d", kNumVariants - 1);
         g_opt_variant = value;
+    } else if (!strcmp(name, "poly_off")) {
+        g_opt_poly_off = value != 0;
     } else if (!strcmp(name, "ctas_per_sm")) {
         if (value < 0 || value > 32) return fail(JPET_E_INVAL, "ctas_per_sm must be 0 (auto) .. 32");
         g_opt_ctas_per_sm = value;
@@ -899,13 +974,19 @@ int64_t jpet_get_option(const char* name) {
     if (!strcmp(name, "chunk")) return g_opt_chunk;
     if (!strcmp(name, "sub_tile_z")) return g_opt_sz;
     if (!strcmp(name, "time_kernel")) return g_opt_time_kernel;
-    if (!strcmp(name, "last_kernel_ns")) {      // duration of the last tiled event-kernel launch (synchronises on it)
-        if (!g_tk_valid || cudaEventSynchronize(g_tk1) != cudaSuccess) return -1;
-        float ms = 0.f;
-        if (cudaEventElapsedTime(&ms, g_tk0, g_tk1) != cudaSuccess) return -1;
-        return (int64_t)((double)ms * 1e6);
+    if (!strcmp(name, "last_kernel_ns")) {      // summed duration of the tiled event-kernel launches of the last iteration
+        if (g_tk_used == 0) return -1;          // (one launch per batch of events; synchronises on the last one)
+        double total = 0.0;
+        for (size_t i = 0; i + 1 < g_tk_used; i += 2) {
+            float ms = 0.f;
+            if (cudaEventSynchronize(g_tk[i + 1]) != cudaSuccess || cudaEventElapsedTime(&ms, g_tk[i], g_tk[i + 1]) != cudaSuccess) return -1;
+            total += ms;
+        }
+        return (int64_t)(total * 1e6);
     }
+    if (!strcmp(name, "last_kernel_launches")) return (int64_t)(g_tk_used / 2);
     if (!strcmp(name, "variant")) return g_opt_variant;
+    if (!strcmp(name, "poly_off")) return g_opt_poly_off;
     if (!strcmp(name, "ctas_per_sm")) return g_opt_ctas_per_sm;
     if (!strcmp(name, "last_variant")) return g_ws.variant;
     if (!strcmp(name, "last_smem_bytes")) return (int64_t)g_ws.smem;

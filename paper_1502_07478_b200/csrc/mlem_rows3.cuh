@@ -34,7 +34,53 @@ __device__ __forceinline__ f32x2 bc2(float x) { return pack2(x, x); }
 struct Piece {
     RowWalk rc;          // rc.lo / rc.len: first column and pixel count of the piece
     uint32_t off;        // byte offset of its first pixel inside a region
+    float c[6];          // DEG > 0: log2 P = c[0] + c[1] v + ... + c[DEG] v^DEG along the piece (see poly_coeffs2)
 };
+
+__device__ __forceinline__ float rcp_approx(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float lg2_approx(float x) {
+    float y;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// One MUFU per kernel value instead of two.  Along a row (v = scaled u, mlem_kernels.cuh) Eq. 7 reads
+//     log2 P = c2s - v^2 + ba(v)^2 / D(v) - 1/2 log2 D(v),     ba = alphas v + betas,   D = delta + eps v,
+// and x = eps v / delta is small inside the 3-sigma ellipse: |x| <= 2 |t| |y| |u| / (sec^2 (R^2 + y^2)), a few
+// per cent at most (the host plan bounds it and picks DEG, or falls back to DEG = 0, the closed form).  With
+// kappa = eps / delta, 1 / D = (1 - x + x^2 - ...) / delta and ln D = ln delta + x - x^2/2 + x^3/3 - ..., so
+//     ba^2 / D = sum_n e_n v^n,   e_0 = beta^2 / delta,  e_1 = 2 alpha beta / delta - kappa e_0,
+//                                 e_2 = alpha^2 / delta - kappa e_1,  e_n = -kappa e_(n-1)  (n >= 3),
+//     -1/2 log2 D = -1/2 log2 delta - LH (kappa v - kappa^2 v^2 / 2 + kappa^3 v^3 / 3 - ...),   LH = log2(e) / 2.
+// The series is cut after v^DEG; the neglected terms are bounded by (ba^2/D) |x|^(DEG-1) + |x|^(DEG+1).
+// Two pieces (A in the low half, B in the high half) at a time.
+template <int DEG>
+__device__ __forceinline__ void poly_coeffs2(f32x2 C2S, f32x2 BET, f32x2 ALP, f32x2 EPS, f32x2 DEL, f32x2 (&C)[6]) {
+    float d0, d1;
+    unpack2(DEL, d0, d1);
+    const f32x2 G = pack2(rcp_approx(d0), rcp_approx(d1));
+    const f32x2 L2 = pack2(lg2_approx(d0), lg2_approx(d1));
+    const f32x2 NK = mul2(mul2(EPS, G), bc2(-1.f));                   // -kappa
+    const f32x2 GB = mul2(G, BET), GA = mul2(G, ALP);
+    f32x2 E[6], K[6];
+    E[0] = mul2(GB, BET);
+    E[1] = fma2(NK, E[0], mul2(add2(GB, GB), ALP));
+    E[2] = fma2(NK, E[1], mul2(GA, ALP));
+    K[1] = NK;                                                          // K[n] = (-kappa)^n
+#pragma unroll
+    for (int n = 2; n <= DEG; ++n) K[n] = mul2(K[n - 1], NK);
+#pragma unroll
+    for (int n = 3; n <= DEG; ++n) E[n] = mul2(NK, E[n - 1]);
+    C[0] = fma2(L2, bc2(-0.5f), add2(C2S, E[0]));
+    C[1] = fma2(K[1], bc2(kLH), E[1]);                                  // -LH kappa
+    C[2] = fma2(K[2], bc2(0.5f * kLH), add2(E[2], bc2(-1.f)));          // +LH kappa^2 / 2, and the Gaussian -v^2
+#pragma unroll
+    for (int n = 3; n <= DEG; ++n) C[n] = fma2(K[n], bc2(kLH / (float)n), E[n]);      // (-1)^n LH kappa^n / n
+}
 
 // Span of one piece: row iy (valid or not), half chord^2 hw2 [px^2], chord centre zcp [px]; part `part` of 2^sh.
 template <int CAP, int HS, bool SPLIT>
@@ -62,7 +108,7 @@ __device__ __forceinline__ void piece_span(uint32_t te, int iy, float hw2, float
 }
 
 // Row constants of pieces A and B (polynomials in dy, see mlem_rows2.cuh) in packed arithmetic, then their spans.
-template <int NJA, int NJB, int HS>
+template <int NJA, int NJB, int HS, int DEG>
 __device__ __forceinline__ void pieces_setup(uint32_t te, const float4 r0, const float4 r1, const float4 r2,
                                              const float4 r3, const DevParams& p, int ry0, int rz0, int col_lo, int col_hi,
                                              Piece& A, Piece& B, int& overflow) {
@@ -87,6 +133,12 @@ __device__ __forceinline__ void pieces_setup(uint32_t te, const float4 r0, const
         unpack2(DEL, A.rc.delta, B.rc.delta);
         unpack2(HW2, hwA, hwB);
         unpack2(ZCP, zcA, zcB);
+        if constexpr (DEG > 0) {
+            f32x2 C[6];
+            poly_coeffs2<DEG>(C2S, BET, ALP, EPS, DEL, C);
+#pragma unroll
+            for (int n = 0; n <= DEG; ++n) unpack2(C[n], A.c[n], B.c[n]);
+        }
         piece_span<NJA, HS, false>(teA, iyA, hwA, zcA, p.pxs, p, ry0, rz0, col_lo, col_hi, A, overflow);
         piece_span<NJB, HS, true>(teB, iyB, hwB, zcB, p.pxs, p, ry0, rz0, col_lo, col_hi, B, overflow);
     } else {
@@ -97,6 +149,13 @@ __device__ __forceinline__ void pieces_setup(uint32_t te, const float4 r0, const
         A.rc.alphas = fmaf(r1.y, dy, r1.x);
         A.rc.eps = fmaf(r1.w, dy, r1.z);
         A.rc.delta = fmaf(dy, fmaf(r2.z, dy, r2.y), r2.x);
+        if constexpr (DEG > 0) {
+            f32x2 C[6];
+            poly_coeffs2<DEG>(bc2(A.rc.c2s), bc2(A.rc.betas), bc2(A.rc.alphas), bc2(A.rc.eps), bc2(A.rc.delta), C);
+            float dummy;
+#pragma unroll
+            for (int n = 0; n <= DEG; ++n) unpack2(C[n], A.c[n], dummy);
+        }
         piece_span<NJA, HS, false>(teA, iyA, fmaf(r2.w, dy2, p.H0p), fmaf(r3.y, dy, r3.x), p.pxs, p, ry0, rz0, col_lo, col_hi, A, overflow);
     }
 }
@@ -104,13 +163,31 @@ __device__ __forceinline__ void pieces_setup(uint32_t te, const float4 r0, const
 // State of one pixel walk (pass 1): packed row constants, running u' pair and denominator pair.
 struct Walk {
     f32x2 EPS2, DEL2, ALP2, BET2, C2S2, STEP2, V2, DEN2;
+    f32x2 C[6];          // DEG > 0: broadcast polynomial coefficients (EPS2 ... C2S2 unused)
     uint32_t wa;
     int len;
 };
 
 // Two adjacent pixels j, j+1 of the piece: Eq. 7 (up to the constant K) and the denominator term.
-template <int J, int HS, bool MASK>
+template <int J, int HS, bool MASK, int DEG>
 __device__ __forceinline__ void walk_pair(Walk& s, float& p0, float& p1) {
+    if constexpr (DEG > 0) {
+        f32x2 E2 = fma2(s.C[DEG], s.V2, s.C[DEG - 1]);
+#pragma unroll
+        for (int n = DEG - 2; n >= 0; --n) E2 = fma2(E2, s.V2, s.C[n]);
+        float e0, e1;
+        unpack2(E2, e0, e1);
+        float x0 = ex2_approx(e0), x1 = ex2_approx(e1);
+        if (MASK) {
+            x0 = J < s.len ? x0 : 0.f;
+            x1 = J + 1 < s.len ? x1 : 0.f;
+        }
+        s.DEN2 = fma2(pack2(x0, x1), pack2(lds_imm<4 * J * HS>(s.wa), lds_imm<4 * (J + 1) * HS>(s.wa)), s.DEN2);
+        p0 = x0;
+        p1 = x1;
+        s.V2 = add2(s.V2, s.STEP2);
+        return;
+    }
     const f32x2 D2 = fma2(s.EPS2, s.V2, s.DEL2), BA2 = fma2(s.ALP2, s.V2, s.BET2);
     float d0, d1;
     unpack2(D2, d0, d1);
@@ -135,66 +212,107 @@ __device__ __forceinline__ void walk_pair(Walk& s, float& p0, float& p1) {
 // pair to cost the 4-warp schedulers about as much as the block's own arithmetic - and every block is one basic
 // block of BW / 2 independent pixel pairs for the scheduler to interleave.  All pairs are masked by the lane's own
 // pixel count.
-constexpr int kBW = 8;
+// BW (template parameter): pixels per block, 4 or 8.
 
-template <int JB, int NJ, int HS>
+template <int JB, int NJ, int HS, int DEG, int BW>
 __device__ __forceinline__ void walk_block(Walk& s, float u0s, float pxs, float (&preg)[NJ]) {
     const float vb = fmaf((float)JB, pxs, u0s);
     s.V2 = pack2(vb, vb + pxs);
-    static_for<0, kBW / 2>([&](auto kc) {
+    static_for<0, BW / 2>([&](auto kc) {
         constexpr int J = JB + 2 * decltype(kc)::value;
-        if constexpr (J < NJ) walk_pair<J, HS, true>(s, preg[J], preg[J + 1]);
+        if constexpr (J < NJ) walk_pair<J, HS, true, DEG>(s, preg[J], preg[J + 1]);
     });
 }
 
-template <int NJ, int HS>
+#define JPET_BLOCK_CASES(CALL)                                                 \
+    switch (nblk) {                                                            \
+        default:                                                               \
+        case 12: if constexpr (NB > 11) { CALL(11); } [[fallthrough]];         \
+        case 11: if constexpr (NB > 10) { CALL(10); } [[fallthrough]];         \
+        case 10: if constexpr (NB > 9) { CALL(9); } [[fallthrough]];           \
+        case 9: if constexpr (NB > 8) { CALL(8); } [[fallthrough]];            \
+        case 8: if constexpr (NB > 7) { CALL(7); } [[fallthrough]];            \
+        case 7: if constexpr (NB > 6) { CALL(6); } [[fallthrough]];            \
+        case 6: if constexpr (NB > 5) { CALL(5); } [[fallthrough]];            \
+        case 5: if constexpr (NB > 4) { CALL(4); } [[fallthrough]];            \
+        case 4: if constexpr (NB > 3) { CALL(3); } [[fallthrough]];            \
+        case 3: if constexpr (NB > 2) { CALL(2); } [[fallthrough]];            \
+        case 2: if constexpr (NB > 1) { CALL(1); } [[fallthrough]];            \
+        case 1: { CALL(0); } [[fallthrough]];                                  \
+        case 0: break;                                                         \
+    }
+
+template <int NJ, int HS, int DEG, int BW>
 __device__ __forceinline__ float piece_pass1(const Piece& pc, uint32_t w_addr, float pxs, int nblk, float (&preg)[NJ]) {
-    static_assert(NJ % 2 == 0 && NJ <= 6 * kBW, "pixel capacity must be even and at most 48");
-    constexpr int NB = (NJ + kBW - 1) / kBW;
+    static_assert(NJ % 2 == 0 && NJ <= 12 * BW && (BW == 4 || BW == 8), "pixel capacity must be even and at most 12 blocks");
+    constexpr int NB = (NJ + BW - 1) / BW;
     Walk s;
-    s.EPS2 = bc2(pc.rc.eps); s.DEL2 = bc2(pc.rc.delta); s.ALP2 = bc2(pc.rc.alphas); s.BET2 = bc2(pc.rc.betas);
-    s.C2S2 = bc2(pc.rc.c2s); s.STEP2 = bc2(2.f * pxs);
+    if constexpr (DEG > 0) {
+#pragma unroll
+        for (int n = 0; n <= DEG; ++n) s.C[n] = bc2(pc.c[n]);
+    } else {
+        s.EPS2 = bc2(pc.rc.eps); s.DEL2 = bc2(pc.rc.delta); s.ALP2 = bc2(pc.rc.alphas); s.BET2 = bc2(pc.rc.betas);
+        s.C2S2 = bc2(pc.rc.c2s);
+    }
+    s.STEP2 = bc2(2.f * pxs);
     s.DEN2 = pack2(0.f, 0.f);
     s.wa = w_addr + pc.off;
     s.len = pc.rc.len;
     const float u0s = pc.rc.u0s;
-    switch (nblk) {
-        default:
-        case 6: if constexpr (NB > 5) walk_block<5 * kBW, NJ, HS>(s, u0s, pxs, preg); [[fallthrough]];
-        case 5: if constexpr (NB > 4) walk_block<4 * kBW, NJ, HS>(s, u0s, pxs, preg); [[fallthrough]];
-        case 4: if constexpr (NB > 3) walk_block<3 * kBW, NJ, HS>(s, u0s, pxs, preg); [[fallthrough]];
-        case 3: if constexpr (NB > 2) walk_block<2 * kBW, NJ, HS>(s, u0s, pxs, preg); [[fallthrough]];
-        case 2: if constexpr (NB > 1) walk_block<1 * kBW, NJ, HS>(s, u0s, pxs, preg); [[fallthrough]];
-        case 1: walk_block<0, NJ, HS>(s, u0s, pxs, preg); [[fallthrough]];
-        case 0: break;
-    }
+#define JPET_WALK(B) walk_block<(B) * BW, NJ, HS, DEG, BW>(s, u0s, pxs, preg)
+    JPET_BLOCK_CASES(JPET_WALK)
+#undef JPET_WALK
     float q0, q1;
     unpack2(s.DEN2, q0, q1);
     return q0 + q1;
 }
 
+// acc[addr + IMM + k STRIDE] += P_k * inv for k = 0..3, lanes with len > J + k: four loads in flight, then the four
+// multiply-adds, then the stores (one asm block so that the loads are not serialised behind the previous store).
+template <int IMM, int STRIDE, int J>
+__device__ __forceinline__ void smem_fma_if4(uint32_t addr, float P0, float P1, float P2, float P3, float inv, int len) {
+    asm volatile(
+        "{\n\t.reg .pred p0, p1, p2, p3;\n\t.reg .f32 t0, t1, t2, t3;\n\t"
+        "setp.gt.s32 p0, %6, %7;\n\t"
+        "setp.gt.s32 p1, %6, %8;\n\t"
+        "setp.gt.s32 p2, %6, %9;\n\t"
+        "setp.gt.s32 p3, %6, %10;\n\t"
+        "@p0 ld.shared.f32 t0, [%0 + %11];\n\t"
+        "@p1 ld.shared.f32 t1, [%0 + %12];\n\t"
+        "@p2 ld.shared.f32 t2, [%0 + %13];\n\t"
+        "@p3 ld.shared.f32 t3, [%0 + %14];\n\t"
+        "@p0 fma.rn.f32 t0, %1, %5, t0;\n\t"
+        "@p1 fma.rn.f32 t1, %2, %5, t1;\n\t"
+        "@p2 fma.rn.f32 t2, %3, %5, t2;\n\t"
+        "@p3 fma.rn.f32 t3, %4, %5, t3;\n\t"
+        "@p0 st.shared.f32 [%0 + %11], t0;\n\t"
+        "@p1 st.shared.f32 [%0 + %12], t1;\n\t"
+        "@p2 st.shared.f32 [%0 + %13], t2;\n\t"
+        "@p3 st.shared.f32 [%0 + %14], t3;\n\t}"
+        ::"r"(addr), "f"(P0), "f"(P1), "f"(P2), "f"(P3), "f"(inv), "r"(len), "n"(J), "n"(J + 1), "n"(J + 2), "n"(J + 3),
+          "n"(IMM), "n"(IMM + STRIDE), "n"(IMM + 2 * STRIDE), "n"(IMM + 3 * STRIDE)
+        : "memory");
+}
+
 // Pass 2: acc += P * inv over the same pixels (private region, one owner lane per pixel: plain read-modify-write).
-template <int JB, int NJ, int HS>
+template <int JB, int NJ, int HS, int BW>
 __device__ __forceinline__ void scatter_block(uint32_t aa, const float (&preg)[NJ], float inv, int len) {
-    static_for<0, kBW>([&](auto kc) {
-        constexpr int J = JB + decltype(kc)::value;
-        if constexpr (J < NJ) smem_fma_if<4 * J * HS, J>(aa, preg[J], inv, len);
+    static_for<0, BW / 4>([&](auto kc) {
+        constexpr int J = JB + 4 * decltype(kc)::value;
+        if constexpr (J + 3 < NJ) smem_fma_if4<4 * J * HS, 4 * HS, J>(aa, preg[J], preg[J + 1], preg[J + 2], preg[J + 3], inv, len);
+        else static_for<0, 4>([&](auto qc) {
+            constexpr int Q = J + decltype(qc)::value;
+            if constexpr (Q < NJ) smem_fma_if<4 * Q * HS, Q>(aa, preg[Q], inv, len);
+        });
     });
 }
 
-template <int NJ, int HS>
+template <int NJ, int HS, int BW>
 __device__ __forceinline__ void piece_pass2(uint32_t aa, const float (&preg)[NJ], float inv, int len, int nblk) {
-    constexpr int NB = (NJ + kBW - 1) / kBW;
-    switch (nblk) {
-        default:
-        case 6: if constexpr (NB > 5) scatter_block<5 * kBW, NJ, HS>(aa, preg, inv, len); [[fallthrough]];
-        case 5: if constexpr (NB > 4) scatter_block<4 * kBW, NJ, HS>(aa, preg, inv, len); [[fallthrough]];
-        case 4: if constexpr (NB > 3) scatter_block<3 * kBW, NJ, HS>(aa, preg, inv, len); [[fallthrough]];
-        case 3: if constexpr (NB > 2) scatter_block<2 * kBW, NJ, HS>(aa, preg, inv, len); [[fallthrough]];
-        case 2: if constexpr (NB > 1) scatter_block<1 * kBW, NJ, HS>(aa, preg, inv, len); [[fallthrough]];
-        case 1: scatter_block<0, NJ, HS>(aa, preg, inv, len); [[fallthrough]];
-        case 0: break;
-    }
+    constexpr int NB = (NJ + BW - 1) / BW;
+#define JPET_SCATTER(B) scatter_block<(B) * BW, NJ, HS, BW>(aa, preg, inv, len)
+    JPET_BLOCK_CASES(JPET_SCATTER)
+#undef JPET_SCATTER
 }
 
 // Event records travel global -> shared with cp.async into a two-slot ring per warp, one event ahead: no registers
@@ -216,24 +334,24 @@ __device__ __forceinline__ void named_barrier(int id, int nthreads) {
 }
 
 // One event on one group of NWE warps.  tab_n: table row of this event's row count ([lane of the group]).
-template <int NWE, int NJA, int NJB, int HS>
+template <int NWE, int NJA, int NJB, int HS, int DEG, int BW>
 __device__ __forceinline__ void process_event_rows3(const float4 r0, const float4 r1, const float4 r2, const float4 r3,
                                                     const DevParams& p, const uint32_t* tab_n, uint32_t w_addr, uint32_t a_addr,
                                                     int ry0, int rz0, int col_lo, int col_hi, float* red_s, int group, int glane,
                                                     int& my_evals, int& my_skipped, int& overflow) {
     constexpr int GL = NWE * 32;
     Piece A, B;
-    pieces_setup<NJA, NJB, HS>(tab_n[glane], r0, r1, r2, r3, p, ry0, rz0, col_lo, col_hi, A, B, overflow);
-    const int nbA = (__reduce_max_sync(0xffffffffu, A.rc.len) + kBW - 1) / kBW;
+    pieces_setup<NJA, NJB, HS, DEG>(tab_n[glane], r0, r1, r2, r3, p, ry0, rz0, col_lo, col_hi, A, B, overflow);
+    const int nbA = (__reduce_max_sync(0xffffffffu, A.rc.len) + BW - 1) / BW;
     float pregA[NJA];
-    float denom = piece_pass1<NJA, HS>(A, w_addr, p.pxs, nbA, pregA);
+    float denom = piece_pass1<NJA, HS, DEG, BW>(A, w_addr, p.pxs, nbA, pregA);
     my_evals += A.rc.len;
     constexpr int NJB1 = NJB > 0 ? NJB : 2;
     float pregB[NJB1];
     int nbB = 0;
     if constexpr (NJB > 0) {
-        nbB = (__reduce_max_sync(0xffffffffu, B.rc.len) + kBW - 1) / kBW;
-        denom += piece_pass1<NJB, HS>(B, w_addr, p.pxs, nbB, pregB);
+        nbB = (__reduce_max_sync(0xffffffffu, B.rc.len) + BW - 1) / BW;
+        denom += piece_pass1<NJB, HS, DEG, BW>(B, w_addr, p.pxs, nbB, pregB);
         my_evals += B.rc.len;
     }
     // ---- denominator: sum over the group -----------------------------------------------------------------------
@@ -249,13 +367,13 @@ __device__ __forceinline__ void process_event_rows3(const float4 r0, const float
     const bool ok = (denom > 0.f) && (denom < 3.0e38f);
     if (!ok) { if (glane == 0) my_skipped += 1; return; }
     const float inv = 1.f / denom;
-    piece_pass2<NJA, HS>(a_addr + A.off, pregA, inv, A.rc.len, nbA);
-    if constexpr (NJB > 0) piece_pass2<NJB, HS>(a_addr + B.off, pregB, inv, B.rc.len, nbB);
+    piece_pass2<NJA, HS, BW>(a_addr + A.off, pregA, inv, A.rc.len, nbA);
+    if constexpr (NJB > 0) piece_pass2<NJB, HS, BW>(a_addr + B.off, pregB, inv, B.rc.len, nbB);
 }
 
 // CTA = NG groups of NWE warps.  Work item = (sub-tile, chunk of sorted events): the CTA stages w once, group g
 // takes events g, g + NG, ... of the chunk into its own accumulator region and flushes it with red.global.add.
-template <int NWE, int NG, int NJA, int NJB, int HS, int MINB>
+template <int NWE, int NG, int NJA, int NJB, int HS, int MINB, int DEG, int BW>
 __global__ void __launch_bounds__(NWE * NG * 32, MINB)
 mlem_rows3_kernel(const EventRec* __restrict__ sorted, const WorkItem* __restrict__ items, int* __restrict__ meta,
                   const __grid_constant__ DevParams p, const float* __restrict__ wT, float* __restrict__ accT,
@@ -324,7 +442,7 @@ mlem_rows3_kernel(const EventRec* __restrict__ sorted, const WorkItem* __restric
             cp_async_commit();
             const int nrows = __float_as_int(r3.w);
             const uint32_t* tab_n = tab_s + (nrows - p.nr_min) * GL;
-            process_event_rows3<NWE, NJA, NJB, HS>(r0, r1, r2, r3, p, tab_n, w_addr, a_addr, ry0, rz0, col_lo, col_hi,
+            process_event_rows3<NWE, NJA, NJB, HS, DEG, BW>(r0, r1, r2, r3, p, tab_n, w_addr, a_addr, ry0, rz0, col_lo, col_hi,
                                                    red_s[group][parity], group, glane, my_evals, my_skipped, overflow);
             parity ^= 1;
         }

@@ -106,7 +106,7 @@ def test_cfg1_ten_iterations(jp, oracle):
     assert rel_err(got, want) <= TOL_10
 
 
-@pytest.mark.parametrize("variant", list(range(28)))
+@pytest.mark.parametrize("variant", list(range(51)))
 @pytest.mark.parametrize("name,n", [("cfg1", 7777), ("cfg2", 30011), ("cfg4", 5003)])
 def test_every_kernel_variant(jp, oracle, variant, name, n):
     """Each event-kernel shape (warps per CTA, row parts, row passes, cached pixels) on small, medium and large
@@ -220,7 +220,7 @@ def test_cfg5_streamed_batches(jp, oracle):
     jp.jpet_mlem_end(rho, split)
     ne, ns = jp.jpet_get_counters()
     want, one, ons = oracle.mlem_iterate(ev, *geom(cfg), np.ones((cfg.n_y, cfg.n_z)))
-    assert float((split - whole).abs().max() / whole.max()) <= 2e-6
+    assert float((split - whole).abs().max() / whole.max()) <= 1e-5    # fp32 sums in another order (R20)
     assert rel_err(split.cpu().numpy().astype(np.float64).reshape(cfg.n_y, cfg.n_z), want) <= TOL_1
     assert ns == ons and abs(ne - one) <= 1e-5 * one
     # columns with |z| > L/2 have s = 0 -> rho_out = 0 there (R13)
