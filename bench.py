@@ -267,6 +267,7 @@ def main():
             kern_ms.append(ns * 1e-6)
     barrier()
     launches = jp.jpet_launch_count() - launches0
+    kernel_launches = jp.jpet_get_option("last_kernel_launches")     # event-kernel launches per step (one per batch)
     jp.jpet_set_option("time_kernel", 0)
     step_ms = [a.elapsed_time(d) for a, _, _, d in pairs]
     acc_ms = [b.elapsed_time(c) for _, b, c, _ in pairs]          # binning + event kernels of the step
@@ -312,7 +313,7 @@ def main():
                 "unit": "Geval/s", "frac": achieved / peak_evals, "traffic": None,
                 "peak_source": f"{n_sm} SMs x 16 MUFU/clk / 2 MUFU per eval x {sm_mhz_peak:.0f} MHz ({peak_kind} sm_max_mhz)",
                 "kernel_ms": kern_s * 1e3, "kernel_share_of_step": statistics.mean(kern_ms) / statistics.mean(step_ms),
-                "binning_plus_kernels_ms": statistics.mean(acc_ms),
+                "binning_plus_kernels_ms": statistics.mean(acc_ms), "kernel_launches_per_step": kernel_launches,
                 "hbm_gbs_algorithmic": (events.nbytes + 8 * M) / kern_s / 1e9, "hbm_peak_gbs": peaks.get("hbm_gbs")}
 
     cpu_baseline = None
