@@ -505,7 +505,11 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     if (smem > budget || !tiles_ok || p.WZ < v_NJ + 4 || g_opt_force_direct) { p.t_max = -1.f; smem = 0; p.nr_min = p.nr_max = 0; tab.clear(); }
     p.nby = (gr.n_y + 2 * p.Hy + p.Sy - 1) / p.Sy;
     p.nbz = (gr.n_z + 2 * p.Hz + p.Sz - 1) / p.Sz;
-    p.chunk = g_opt_chunk > 0 ? (int)g_opt_chunk : (gen3 ? 64 * kVariants3[v - kNumVariants2].NG : 64);
+    // events per work item (one staging of w and one flush of the accumulator regions per item): measured optimum on B200
+    // 128 events per group for the one-warp groups (config 2: 0.740 -> 0.734 ms), 256 for the four-warp groups
+    // (configs 4, 5: +5-8 %)
+    p.chunk = g_opt_chunk > 0 ? (int)g_opt_chunk
+                              : (gen3 ? (kVariants3[v - kNumVariants2].NWE > 1 ? 256 : 128) * kVariants3[v - kNumVariants2].NG : 64);
     *out = p;
     *variant = v;
     *smem_out = smem;

@@ -214,14 +214,57 @@ __device__ __forceinline__ void walk_pair(Walk& s, float& p0, float& p1) {
 // pixel count.
 // BW (template parameter): pixels per block, 4 or 8.
 
+// DEG > 0: the pairs of a block in LOCKSTEP - all u' pairs, then one Horner step for every pair, ..., then the ex2, the
+// masks and the denominator terms (two accumulators).  ptxas keeps source order: written pair after pair it issued the
+// four dependent FFMA2 of a Horner chain back to back (4-cycle waits, the largest stall of the kernel in ncu).
+template <int JB, int NJ, int HS, int DEG, int BW>
+__device__ __forceinline__ void walk_block_lockstep(Walk& s, float u0s, float pxs, float (&preg)[NJ]) {
+    constexpr int NPAIR = (NJ - JB < BW ? NJ - JB : BW) / 2;
+    const float vb = fmaf((float)JB, pxs, u0s);
+    f32x2 V[NPAIR], E[NPAIR];
+    float x[2 * NPAIR];
+    V[0] = pack2(vb, vb + pxs);
+#pragma unroll
+    for (int k = 1; k < NPAIR; ++k) V[k] = add2(V[k - 1], s.STEP2);
+#pragma unroll
+    for (int k = 0; k < NPAIR; ++k) E[k] = fma2(s.C[DEG], V[k], s.C[DEG - 1]);
+#pragma unroll
+    for (int n = DEG - 2; n >= 0; --n) {
+#pragma unroll
+        for (int k = 0; k < NPAIR; ++k) E[k] = fma2(E[k], V[k], s.C[n]);
+    }
+#pragma unroll
+    for (int k = 0; k < NPAIR; ++k) {
+        float e0, e1;
+        unpack2(E[k], e0, e1);
+        x[2 * k] = ex2_approx(e0);
+        x[2 * k + 1] = ex2_approx(e1);
+    }
+    f32x2 DENB = pack2(0.f, 0.f);
+    static_for<0, NPAIR>([&](auto kc) {
+        constexpr int K = decltype(kc)::value, J = JB + 2 * K;
+        const float x0 = J < s.len ? x[2 * K] : 0.f, x1 = J + 1 < s.len ? x[2 * K + 1] : 0.f;
+        const f32x2 W2 = pack2(lds_imm<4 * J * HS>(s.wa), lds_imm<4 * (J + 1) * HS>(s.wa));
+        if constexpr (K & 1) DENB = fma2(pack2(x0, x1), W2, DENB);
+        else s.DEN2 = fma2(pack2(x0, x1), W2, s.DEN2);
+        preg[J] = x0;
+        preg[J + 1] = x1;
+    });
+    if constexpr (NPAIR > 1) s.DEN2 = add2(s.DEN2, DENB);
+}
+
 template <int JB, int NJ, int HS, int DEG, int BW>
 __device__ __forceinline__ void walk_block(Walk& s, float u0s, float pxs, float (&preg)[NJ]) {
-    const float vb = fmaf((float)JB, pxs, u0s);
-    s.V2 = pack2(vb, vb + pxs);
-    static_for<0, BW / 2>([&](auto kc) {
-        constexpr int J = JB + 2 * decltype(kc)::value;
-        if constexpr (J < NJ) walk_pair<J, HS, true, DEG>(s, preg[J], preg[J + 1]);
-    });
+    if constexpr (DEG > 0) {
+        if constexpr (JB < NJ) walk_block_lockstep<JB, NJ, HS, DEG, BW>(s, u0s, pxs, preg);
+    } else {
+        const float vb = fmaf((float)JB, pxs, u0s);
+        s.V2 = pack2(vb, vb + pxs);
+        static_for<0, BW / 2>([&](auto kc) {
+            constexpr int J = JB + 2 * decltype(kc)::value;
+            if constexpr (J < NJ) walk_pair<J, HS, true, DEG>(s, preg[J], preg[J + 1]);
+        });
+    }
 }
 
 #define JPET_BLOCK_CASES(CALL)                                                 \

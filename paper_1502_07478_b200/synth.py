@@ -85,6 +85,14 @@ CONFIGS = {
                    (_E(0, -90, 12, 12, 0, 4.0), _E(-50, 70, 18, 18, 0, 3.0), _E(60, 20, 45, 25, -20, 0.0),
                     _E(-60, -20, 55, 30, 20, 2.0), _E(0, 0, 150, 200, 0, 1.0), _E(0, 0, 165, 215, 0, 2.0)),
                    batch=10_000_000),
+    # The paper's own set-up: Fig. 4 geometry R = 130 mm, L = 300 mm, 4 x 4 mm pixels
+    # and the phantom of Table 2 (rows (x, y, a, b, phi, rho), centre (x, y),
+    # half-axes a, b, rotated by phi counter-clockwise, topmost row wins; x is the coordinate along the strips = z,
+    # reading R21), sigma_z = 10 mm, sigma_dl = 40 mm.  The paper does not print the number of events
+    # or the grid of Fig. 4; 64 x 80 pixels cover |y| < R and |z| <= L/2 + 8 mm, 2 x 10^6 events, 10 iterations.
+    "fig4": Config("fig4", 130.0, 300.0, 64, 80, 4.0, 2_000_000, 10, 10.0, 40.0,
+                   (_E(0, 0, 60, 30, 0, 0.3), _E(-62, 50, 33, 10, -40, 0.3), _E(-63, -50, 33, 20, 45, 0.5),
+                    _E(65, 60, 14, 13, 0, 0.5), _E(55, 35, 12, 12, 0, 0.7), _E(0, 0, 110, 120, 0, 0.1))),
 }
 
 

@@ -163,3 +163,22 @@ def test_mlem_sharpens_towards_phantom(oracle):
     body = rec[(truth == 1.0) & ((Y**2 + Z**2) > 50**2)].mean()
     empty = rec[(np.abs(Y) > 130) & (truth == 0)].mean()
     assert hot > 2.0 * body > 10.0 * empty
+
+
+def test_paper_shaped_workload_fig4(oracle):
+    """Fig. 4 geometry with the Table 2 phantom.  The phantom is
+    transcribed with x = z (reading R21): each ellipse's centre carries its own density unless a row above covers
+    it; Eq. 3 conserves counts on this geometry as well (strips at R = 130 mm, |tan theta| up to 1.2)."""
+    cfg = synth.CONFIGS["fig4"]
+    table2 = [(0, 0, 0.3), (50, -62, 0.3), (-50, -63, 0.5), (60, 65, 0.5), (35, 55, 0.7)]        # (x, y, rho)
+    for x, y, rho in table2:
+        assert synth.phantom_intensity(cfg.phantom, np.array([float(y)]), np.array([float(x)]))[0] == rho
+    assert synth.phantom_intensity(cfg.phantom, np.array([0.0]), np.array([100.0]))[0] == 0.1    # background, a = 120 along x
+    assert synth.phantom_intensity(cfg.phantom, np.array([115.0]), np.array([0.0]))[0] == 0.0    # b = 110 along y
+    ev = synth.config_events(cfg, n=20000)
+    assert np.all(np.abs(ev[:, :2]) < cfg.L / 2 + 6 * cfg.sigma_z)
+    g = (cfg.R, cfg.L, cfg.sigma_z, cfg.sigma_dl, cfg.n_y, cfg.n_z, cfg.pixel)
+    out, n_evals, n_skipped = oracle.mlem_iterate(ev, *g, np.ones((cfg.n_y, cfg.n_z)))
+    s = oracle.sensitivity_image(cfg.R, cfg.L, cfg.n_y, cfg.n_z, cfg.pixel)
+    assert abs(float((s * out).sum()) - (len(ev) - n_skipped)) <= 1e-8 * len(ev)
+    assert 150 < n_evals / len(ev) < 260           # 9 pi sigma_z sigma_dl cos(theta) / (2 sqrt 2 pixel^2) <= 250

@@ -151,6 +151,26 @@ def test_large_configs_on_a_prefix(jp, oracle, name, n):
     assert ns == ons and abs(ne - one) <= 1e-5 * one
 
 
+def test_paper_shaped_workload_fig4(jp, oracle):
+    """the paper's own set-up - Fig. 4 geometry (R = 130, L = 300, 4 mm pixels) and the
+    Table 2 phantom.  Strips this close make |tan theta~| reach 1.5 and the truncation bound of the
+    polynomial exponent fails, so the plan must fall back to the closed form (rsqrt + ex2)."""
+    cfg = synth.CONFIGS["fig4"]
+    ev = synth.config_events(cfg, n=500_000)
+    ones = np.ones((cfg.n_y, cfg.n_z))
+    got, (ne, ns) = gpu_iterate(jp, ev, cfg, ones)
+    assert jp.jpet_get_option("last_tiled") == 1 and jp.jpet_get_option("last_variant") in (21, 22)   # closed-form shapes
+    want, one, ons = oracle.mlem_iterate(ev, *geom(cfg), ones)
+    assert rel_err(got, want) <= TOL_1
+    assert ns == ons and abs(ne - one) <= 1e-5 * one
+    got10, _ = gpu_iterate(jp, ev, cfg, ones, n_iter=cfg.n_iter)
+    want10, _, _ = oracle.reconstruct(ev, *geom(cfg), cfg.n_iter)
+    assert rel_err(got10, want10) <= TOL_10
+    # the reconstruction resolves the phantom: brightest insert (rho = 0.7 at (y, z) = (55, 35)) above the background
+    iy, iz = int(round(55 / cfg.pixel + (cfg.n_y - 1) / 2)), int(round(35 / cfg.pixel + (cfg.n_z - 1) / 2))
+    assert got10[iy, iz] > 2.0 * got10[cfg.n_y // 2, 8 + 2]          # background ellipse near z = -120 mm
+
+
 @pytest.mark.parametrize("name", ["cfg3", "cfg4"])
 def test_full_size_properties(jp, oracle, name):
     """10^7 events (too many for the oracle in a test): properties that hold at any size -
