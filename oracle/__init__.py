@@ -57,8 +57,22 @@ def _load():
     lib.jo_reconstruct.argtypes = [p, i64, d, d, d, d, i, i, d, d, p, p, i, i, p, p]
     lib.jo_num_threads.restype = i
     lib.jo_num_threads.argtypes = []
+    lib.jo_set_gamma.restype = None
+    lib.jo_set_gamma.argtypes = [d]
+    lib.jo_get_gamma.restype = d
+    lib.jo_get_gamma.argtypes = []
     _lib = lib
     return lib
+
+
+def set_gamma(gamma: float) -> None:
+    """Off-diagonal coefficient gamma of C^-1 (Eq. 12); 0 = the paper's diagonal case (default).
+    Process-wide: set it back to 0 after use."""
+    _load().jo_set_gamma(float(gamma))
+
+
+def get_gamma() -> float:
+    return float(_load().jo_get_gamma())
 
 
 def num_threads() -> int:

@@ -73,7 +73,16 @@ void jo_sensitivity_image(double R, double L, int n_y, int n_z, double pixel, do
             s[(size_t)iy * n_z + iz] = jo_sensitivity(jo_pixel_y(iy, n_y, pixel), jo_pixel_z(iz, n_z, pixel), R, L);
 }
 
-/* ---- b C^-1 b (first line of B.3), diagonal C (R6) -------------------------------------- */
+/* ---- Eq. 12: the off-diagonal coefficient gamma of C^-1 --------------
+ * The paper prints the general form and then sets gamma = 0; 0 is the default here too.
+ * A process-wide setting, like the a3 coefficient of the tests: set it before an iteration, not during one. */
+static double jo_gamma = 0.0;
+void jo_set_gamma(double gamma) { jo_gamma = gamma; }
+double jo_get_gamma(void) { return jo_gamma; }
+
+/* ---- b C^-1 b (first line of B.3) ------------------------------------------------------
+ * b = (u, u, -2 dy / cos) has equal first and second components (Eq. 10), so the gamma terms of Eq. 12,
+ * 2 gamma (b1 - b2) b3, vanish: B.3 and the 3-sigma ellipse do not depend on gamma.                      */
 double jo_bCb(double dy, double dz, double tan_t, double sigma_z, double sigma_dl)
 {
     double cos2 = 1.0 / (1.0 + tan_t * tan_t);
@@ -82,8 +91,8 @@ double jo_bCb(double dy, double dz, double tan_t, double sigma_z, double sigma_d
 }
 
 /* ---- Eq. 7-12: reconstruction kernel P(e~ | pixel at (y, z)) ----------------------
- * Vectors o, a, b are Eq. 8, 9, 10 written out; C^-1 = diag(1/sz^2, 1/sz^2, 1/sdl^2) (Eq. 12, gamma=0,
- * PAPER.md:124).  a3_coef multiplies the third component of a: 2 gives a = d e/d theta (default, R5),
+ * Vectors o, a, b are Eq. 8, 9, 10 written out; C^-1 is the matrix of Eq. 12 with gamma = jo_gamma (0 unless
+ * set: the paper's diagonal case).  a3_coef multiplies the third component of a: 2 gives a = d e/d theta (default, R5),
  * 1 gives Eq. 9 exactly as printed.  Prefactor: det^(1/2) of the INVERSE covariance over 2 pi^2 (R4).
  * No truncation here: the 3-sigma rule is applied by the caller.                                        */
 double jo_kernel(double y, double z, double tan_t, double y_t, double z_t,
@@ -93,7 +102,10 @@ double jo_kernel(double y, double z, double tan_t, double y_t, double z_t,
     double dz = z - z_t;
     double icos = sqrt(1.0 + tan_t * tan_t);   /* cos^-1(theta~) */
     double icos2 = icos * icos;                /* cos^-2(theta~) */
-    double Cinv[3] = { 1.0 / (sigma_z * sigma_z), 1.0 / (sigma_z * sigma_z), 1.0 / (sigma_dl * sigma_dl) };
+    const double g = jo_gamma;
+    double Cinv[3][3] = { { 1.0 / (sigma_z * sigma_z), 0.0, g },                     /* Eq. 12 */
+                          { 0.0, 1.0 / (sigma_z * sigma_z), -g },
+                          { g, -g, 1.0 / (sigma_dl * sigma_dl) } };
 
     double o[3], a[3], b[3];
     o[0] = -(dy + y_t - R) * tan_t * icos2;                       /* Eq. 8 */
@@ -107,15 +119,20 @@ double jo_kernel(double y, double z, double tan_t, double y_t, double z_t,
     b[2] = -2.0 * dy * icos;
 
     double aCa = 0.0, oCb = 0.0, bCb = 0.0, bCa = 0.0;
-    for (int k = 0; k < 3; ++k) {
-        aCa += a[k] * Cinv[k] * a[k];
-        oCb += o[k] * Cinv[k] * b[k];
-        bCb += b[k] * Cinv[k] * b[k];
-        bCa += b[k] * Cinv[k] * a[k];
-    }
+    for (int k = 0; k < 3; ++k)
+        for (int l = 0; l < 3; ++l) {
+            aCa += a[k] * Cinv[k][l] * a[l];
+            oCb += o[k] * Cinv[k][l] * b[l];
+            bCb += b[k] * Cinv[k][l] * b[l];
+            bCa += b[k] * Cinv[k][l] * a[l];
+        }
     double D = aCa + 2.0 * oCb;
     if (!(D > 0.0)) return 0.0;                                   /* R17 */
-    double sqrt_det_Cinv = sqrt(Cinv[0] * Cinv[1] * Cinv[2]);
+    double det_Cinv = Cinv[0][0] * (Cinv[1][1] * Cinv[2][2] - Cinv[1][2] * Cinv[2][1])
+                    - Cinv[0][1] * (Cinv[1][0] * Cinv[2][2] - Cinv[1][2] * Cinv[2][0])
+                    + Cinv[0][2] * (Cinv[1][0] * Cinv[2][1] - Cinv[1][1] * Cinv[2][0]);
+    if (!(det_Cinv > 0.0)) return 0.0;                             /* gamma too large: C^-1 not positive definite */
+    double sqrt_det_Cinv = sqrt(det_Cinv);
     return sqrt_det_Cinv / (2.0 * JO_PI * JO_PI * sqrt(D)) * exp(-0.5 * (bCb - bCa * bCa / D));   /* Eq. 7 */
 }
 

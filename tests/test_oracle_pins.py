@@ -39,7 +39,12 @@ def exact_theta_integral(ev, y, z, sz, sdl, R=R, n=200001):
     return float(np.sum(0.5 * (f[1:] + f[:-1]) * np.diff(th)) / math.pi)
 
 
-def laplace_from_forward_model(ev, y, z, sz, sdl, R=R):
+def cinv_eq12(sz, sdl, gamma=0.0):
+    """Eq. 12 as printed (PAPER.md:122)."""
+    return np.array([[1 / sz**2, 0.0, gamma], [0.0, 1 / sz**2, -gamma], [gamma, -gamma, 1 / sdl**2]])
+
+
+def laplace_from_forward_model(ev, y, z, sz, sdl, R=R, gamma=0.0):
     """Second-order saddle-point value of the theta integral, built ONLY from the forward model:
     expand e(theta) = e(theta~) + a d + o d^2 with a, o from central differences (no Eq. 8-10 typed in),
     keep terms to d^2 in the exponent and do the Gaussian integral over d analytically."""
@@ -51,7 +56,7 @@ def laplace_from_forward_model(ev, y, z, sz, sdl, R=R):
     a = (-ep2 + 8 * ep - 8 * em + em2) / (12 * h)                       # d e / d theta, O(h^4)
     o = 0.5 * (-ep2 + 16 * ep - 30 * e0 + 16 * em - em2) / (12 * h * h)  # 1/2 d2 e / d theta2, O(h^4)
     b = e0 - np.asarray(ev, float)
-    Cinv = np.diag([1 / sz**2, 1 / sz**2, 1 / sdl**2])
+    Cinv = cinv_eq12(sz, sdl, gamma)
     D = a @ Cinv @ a + 2.0 * (o @ Cinv @ b)
     expo = -0.5 * (b @ Cinv @ b - (b @ Cinv @ a) ** 2 / D)
     norm = math.sqrt(np.linalg.det(Cinv)) / (2.0 * math.pi) ** 1.5       # Gaussian density prefactor
@@ -208,6 +213,35 @@ def test_kernel_is_the_saddle_point_of_the_forward_model(oracle):
             worst = max(worst, abs(got / want - 1.0))
             # the printed third component of a (k=1) is distinguishable at this precision for off-axis pixels
     assert worst < 2e-7, worst
+
+
+def test_kernel_with_gamma_is_the_saddle_point_of_the_forward_model(oracle):
+    """Eq. 7 with the general C^-1 of Eq. 12 (gamma != 0) against the same forward-model Laplace value
+    with the full 3x3 matrix; a gamma term with the wrong sign, on the wrong pair of components or dropped from one of
+    the three quadratic forms fails.  b C^-1 b (B.3, the 3-sigma ellipse) does not depend on gamma: b1 = b2."""
+    rng = np.random.default_rng(17)
+    try:
+        for sz, sdl in [(10, 40), (5, 20), (20, 80)]:
+            for frac in (0.3, -0.3, 0.6):
+                gamma = frac / (math.sqrt(2.0) * sz * sdl)          # positive definite for |frac| < 1
+                oracle.set_gamma(gamma)
+                assert oracle.get_gamma() == gamma
+                worst, moved = 0.0, 0.0
+                for _ in range(60):
+                    ev = forward(rng.uniform(-220, 220), rng.uniform(-150, 150), rng.uniform(-0.5, 0.5))
+                    ev = ev + rng.normal(size=3) * np.array([sz, sz, sdl])
+                    tan_t, y_t, z_t = oracle.eq2(*ev, R)
+                    y, z = y_t + rng.uniform(-1.4, 1.4) * sdl, z_t + rng.uniform(-2, 2) * sz
+                    want = laplace_from_forward_model(ev, y, z, sz, sdl, gamma=gamma)
+                    got = oracle.kernel(y, z, tan_t, y_t, z_t, R, sz, sdl, 2.0)
+                    worst = max(worst, abs(got / want - 1.0))
+                    moved = max(moved, abs(laplace_from_forward_model(ev, y, z, sz, sdl) / want - 1.0))
+                    b = forward(y, z, math.atan(tan_t)) - ev
+                    assert abs(b @ cinv_eq12(sz, sdl, gamma) @ b - oracle.bCb(y - y_t, z - z_t, tan_t, sz, sdl)) < 1e-8
+                assert worst < 2e-7, (sz, sdl, frac, worst)
+                assert moved > 1e-2          # gamma changes the kernel by far more than the pin's resolution
+    finally:
+        oracle.set_gamma(0.0)
 
 
 def test_kernel_k1_differs_from_k2_measurably(oracle):
