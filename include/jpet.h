@@ -108,6 +108,15 @@ int jpet_count_evals(const float *events_dev, int64_t n, const jpet_geometry *ge
 int jpet_set_a3_coef(float k);
 float jpet_get_a3_coef(void);
 
+/* Off-diagonal coefficient gamma of the inverse correlation matrix, Eq. 12:
+ *   C^-1 = [[1/sigma_z^2, 0, gamma], [0, 1/sigma_z^2, -gamma], [gamma, -gamma, 1/sigma_dl^2]]   [1/mm^2].
+ * 0 (default) is the diagonal matrix the paper works with.  Process-wide, takes effect at the next
+ * begin / iterate / reconstruct call; those return JPET_E_INVAL when |gamma| > 0.5 / (sqrt(2) sigma_z sigma_dl)
+ * (the matrix must stay positive definite and Eq. 7's D positive).  The 3-sigma ellipse does not depend on gamma
+ * (b1 = b2 in Eq. 10).  The set call returns JPET_E_INVAL for a non-finite value. */
+int jpet_set_gamma(float gamma);
+float jpet_get_gamma(void);
+
 /* Tuning knobs (do not change results beyond fp32 summation order).  name/value pairs:
  *   "variant"      event-kernel shape id; -1 = automatic
  *   "force_direct" 1 = skip the shared-memory tiled path: every event goes through the direct kernel

@@ -9,6 +9,7 @@ from .binding import (  # noqa: F401
     jpet_count_evals,
     jpet_get_a3_coef,
     jpet_get_counters,
+    jpet_get_gamma,
     jpet_get_option,
     jpet_last_error,
     jpet_launch_count,
@@ -22,5 +23,6 @@ from .binding import (  # noqa: F401
     jpet_release,
     jpet_sensitivity,
     jpet_set_a3_coef,
+    jpet_set_gamma,
     jpet_set_option,
 )

@@ -15,7 +15,7 @@ JPET_OK, JPET_E_INVAL, JPET_E_CUDA = 0, -1, -2
 EXPORTS = (
     "jpet_sensitivity", "jpet_mlem_iterate", "jpet_reconstruct", "jpet_mlem_begin", "jpet_mlem_accumulate",
     "jpet_mlem_end", "jpet_mlem_iterate_host", "jpet_reconstruct_host", "jpet_get_counters", "jpet_count_evals",
-    "jpet_set_a3_coef", "jpet_get_a3_coef", "jpet_set_option", "jpet_get_option", "jpet_launch_count",
+    "jpet_set_a3_coef", "jpet_get_a3_coef", "jpet_set_gamma", "jpet_get_gamma", "jpet_set_option", "jpet_get_option", "jpet_launch_count",
     "jpet_release", "jpet_last_error", "jpet_abi_version",
 )
 
@@ -71,6 +71,8 @@ def load(build_if_missing: bool = True) -> ctypes.CDLL:
         "jpet_count_evals": (ctypes.c_int, [p, i64, G, S, Gr, u64p, u64p, p]),
         "jpet_set_a3_coef": (ctypes.c_int, [ctypes.c_float]),
         "jpet_get_a3_coef": (ctypes.c_float, []),
+        "jpet_set_gamma": (ctypes.c_int, [ctypes.c_float]),
+        "jpet_get_gamma": (ctypes.c_float, []),
         "jpet_set_option": (ctypes.c_int, [ctypes.c_char_p, i64]),
         "jpet_get_option": (i64, [ctypes.c_char_p]),
         "jpet_launch_count": (ctypes.c_uint64, []),
@@ -207,6 +209,14 @@ def jpet_set_a3_coef(k: float) -> None:
 
 def jpet_get_a3_coef() -> float:
     return float(load().jpet_get_a3_coef())
+
+
+def jpet_set_gamma(gamma: float) -> None:
+    _check(load().jpet_set_gamma(float(gamma)))
+
+
+def jpet_get_gamma() -> float:
+    return float(load().jpet_get_gamma())
 
 
 def jpet_set_option(name: str, value: int) -> None:

@@ -24,6 +24,7 @@ using jpet::DevParams;
 thread_local std::string g_err;
 std::atomic<uint64_t> g_launches{0};
 float g_a3_coef = 2.0f;
+float g_gamma = 0.0f;             // off-diagonal coefficient of C^-1 (Eq. 12); 0 = the paper's diagonal case
 int64_t g_opt_force_direct = 0;  // 1 = every event takes the direct (global-memory) path
 int64_t g_opt_chunk = 0;         // events per work item, 0 = automatic
 int64_t g_opt_sz = 0;            // sub-tile width in pixels, 0 = automatic
@@ -65,7 +66,7 @@ struct BinSet {
 };
 
 struct PlanKey {
-    jpet_geometry g; jpet_sigmas sg; jpet_grid gr; float a3;
+    jpet_geometry g; jpet_sigmas sg; jpet_grid gr; float a3, gamma;
     int64_t variant, sz, chunk, force_direct;
 };
 
@@ -125,6 +126,10 @@ int validate(const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr)
         // (bound derived in DESIGN.md "Domain"); we ask for a factor 2 of margin.
         double ratio = (1.07 * sg->sigma_z + 1.8 * (double)sg->sigma_z * sg->sigma_z / sg->sigma_dl) / g->R;
         if (ratio > 0.5) return fail(JPET_E_INVAL, "sigmas too large against R: Eq. 7's square root could go non-positive");
+        // Eq. 12 is positive definite for gamma^2 < 1 / (2 sigma_z^2 sigma_dl^2); half of that keeps D > 0 as well
+        // (a.C^-1.a changes by at most 2 |gamma| k y sigma_z^2 sin(theta) / R of itself)
+        if (std::fabs((double)g_gamma) * std::sqrt(2.0) * sg->sigma_z * sg->sigma_dl > 0.5)
+            return fail(JPET_E_INVAL, "|gamma| must be at most 0.5 / (sqrt(2) sigma_z sigma_dl) (Eq. 12 positive definite, D > 0)");
         if (3.0 * sg->sigma_dl / gr->pixel > 60000.0 || 4.3 * sg->sigma_z / gr->pixel > 60000.0)
             return fail(JPET_E_INVAL, "ellipse spans too many pixels");
     }
@@ -402,8 +407,8 @@ int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t sme
 
 // Constants of the event kernel (computed in double, rounded once), the tiling of the image into
 // sub-tiles + halo regions, and the kernel variant.
-void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& gr, float a3, DevParams* out, int* variant,
-               size_t* smem_out, std::vector<uint32_t>* tab_out = nullptr) {
+void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& gr, float a3, float gamma, DevParams* out,
+               int* variant, size_t* smem_out, std::vector<uint32_t>* tab_out = nullptr) {
     DevParams p{};
     const double LH = 0.72134752044448170368;
     double iz2 = 1.0 / ((double)sg.sigma_z * sg.sigma_z), il2 = 1.0 / ((double)sg.sigma_dl * sg.sigma_dl);
@@ -425,6 +430,8 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     p.d1k = (float)(2.0 * iz2);
     p.d2k = (float)((double)a3 * a3 * il2);
     p.d3k = (float)(4.0 * il2);
+    p.gB = (float)(4.0 * (double)gamma * g.R);
+    p.gD0 = (float)(4.0 * (double)gamma * g.R * a3);
     // ellipse extents in pixels: half height 1.5 sigma_dl cos(theta), half width 3 sqrt(sz^2/2 + sdl^2 sin^2/4) (App. B)
     double t_max = ((double)g.L + 8.0 * sg.sigma_z) / (2.0 * g.R);
     double sin2 = t_max * t_max / (1.0 + t_max * t_max);
@@ -454,8 +461,12 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
         // third-generation shapes first; degree of the exponent polynomial from the truncation bound (mlem_rows3.cuh,
         // poly_coeffs2): |x| = |eps u / delta| <= xb, ba^2 / D <= eb inside the ellipse and the image
         const double y_max = 0.5 * gr.n_y * px, u_max = 3.0 * sg.sigma_z / std::sqrt(2.0), R2 = (double)g.R * g.R;
-        const double xb = 2.0 * (t_max / (1.0 + t_max * t_max)) * y_max * u_max / (R2 + y_max * y_max) / 0.95;
-        const double eb = 1.1 * 9.0 * y_max * y_max / (R2 + y_max * y_max);
+        // gamma (Eq. 12): delta changes by at most g_rel of itself, |b.C^-1.a| / sqrt(D) grows by at most g_ba
+        const double ag = std::fabs((double)gamma);
+        const double g_rel = 2.0 * ag * std::fabs((double)a3) * y_max * sg.sigma_z * sg.sigma_z * (t_max / std::sqrt(1.0 + t_max * t_max)) / g.R;
+        const double g_ba = 6.0 / std::sqrt(2.0) * ag * sg.sigma_z * sg.sigma_dl;
+        const double xb = 2.0 * (t_max / (1.0 + t_max * t_max)) * y_max * u_max / (R2 + y_max * y_max) / (0.95 - g_rel);
+        const double eb = 1.1 * std::pow(3.0 * y_max / std::sqrt(R2 + y_max * y_max) + g_ba, 2.0);
         auto trunc_err = [&](int deg) {      // log2 units
             return 1.4427 * (0.5 * eb * std::pow(xb, deg - 1) / (1.0 - xb) + 0.5 * std::pow(xb, deg + 1) / (deg + 1));
         };
@@ -615,9 +626,9 @@ int do_begin(const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr,
     }
     g_ws.sig = *sg; g_ws.M = M;
     {   // the plan depends only on these inputs: rebuild it (and the task table) when one of them changes
-        const PlanKey key{*g, *sg, *gr, g_a3_coef, g_opt_variant, g_opt_sz, g_opt_chunk, g_opt_force_direct + 2 * g_opt_poly_off};
+        const PlanKey key{*g, *sg, *gr, g_a3_coef, g_gamma, g_opt_variant, g_opt_sz, g_opt_chunk, g_opt_force_direct + 2 * g_opt_poly_off};
         if (!g_ws.plan_valid || memcmp(&key, &g_ws.plan_key, sizeof key) != 0) {
-            make_plan(*g, *sg, *gr, g_a3_coef, &g_ws.dp, &g_ws.variant, &g_ws.smem, &g_ws.tab_host);
+            make_plan(*g, *sg, *gr, g_a3_coef, g_gamma, &g_ws.dp, &g_ws.variant, &g_ws.smem, &g_ws.tab_host);
             g_ws.plan_key = key;
             g_ws.plan_valid = true;
         }
@@ -917,7 +928,7 @@ int jpet_count_evals(const float* events_dev, int64_t n, const jpet_geometry* ge
     DevParams dp;
     int variant = 0;
     size_t smem = 0;
-    make_plan(*geometry, *sigmas, *grid, g_a3_coef, &dp, &variant, &smem);
+    make_plan(*geometry, *sigmas, *grid, g_a3_coef, g_gamma, &dp, &variant, &smem);
     if (n > 0) {
         int blocks = (int)std::min<int64_t>((n + 255) / 256, (int64_t)g_ws.sm_count * 8);
         jpet::count_evals_kernel<<<blocks, 256, 0, st>>>(events_dev, (long long)n, dp, d);
@@ -941,6 +952,15 @@ int jpet_set_a3_coef(float k) {
 }
 
 float jpet_get_a3_coef(void) { return g_a3_coef; }
+
+int jpet_set_gamma(float gamma) {
+    g_err.clear();
+    if (!std::isfinite(gamma)) return fail(JPET_E_INVAL, "gamma must be finite");
+    g_gamma = gamma;
+    return JPET_OK;
+}
+
+float jpet_get_gamma(void) { return g_gamma; }
 
 int jpet_set_option(const char* name, int64_t value) {
     g_err.clear();

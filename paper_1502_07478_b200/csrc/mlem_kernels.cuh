@@ -67,6 +67,12 @@ struct DevParams {
     float d1k;                         // 2 iz2          (delta term sec2^2 (y^2 + R^2))
     float d2k;                         // k^2 il2        (delta term sec2 t^2 y^2)
     float d3k;                         // 4 il2          (delta term sec2 (1 + 2 t^2) y dy)
+    // off-diagonal coefficient gamma of C^-1 (Eq. 12; 0 = the paper's diagonal case).  With
+    // a1 - a2 = 2 R sec2, o1 - o2 = 2 R sec2 t, b1 = b2, b3 = -2 dy sec, a3 = -k y sec t it adds
+    //   b.C^-1.a += -4 gamma R sec^3 dy,   a.C^-1.a += -4 gamma k R sec^3 t y,   o.C^-1.b += -4 gamma R sec^3 t dy
+    // and leaves b.C^-1.b (the 3-sigma ellipse) unchanged.
+    float gB;                          // 4 gamma R
+    float gD0;                         // 4 gamma R k
     // binning and shared-memory regions (pixel units)
     int Hy, Hz;                        // halo on each side of a sub-tile
     int Sy, Sz;                        // sub-tile size
@@ -209,6 +215,11 @@ __device__ __forceinline__ RowConsts row_setup(const EventConsts& e, int iy, int
     r.betas = kSqrtLH * p.bk * ysec * e.t * dy;
     r.delta = p.d1k * e.sec2 * e.sec2 * fmaf(y, y, p.R2) + p.d2k * ysec * e.t * e.t * y
               + p.d3k * ysec * fmaf(2.f * e.t, e.t, 1.f) * dy;
+    if (p.gB != 0.f) {                                     // Eq. 12 with gamma != 0
+        const float sec3 = e.sec2 * e.sec2 * rsqrt_approx(e.sec2);
+        r.betas -= kSqrtLH * p.gB * sec3 * dy;
+        r.delta -= sec3 * e.t * fmaf(p.gD0, y, 2.f * p.gB * dy);
+    }
     r.alphas = kSqrtLH * alpha;
     r.eps = 2.f * e.t * alpha;
     r.lo = lo;

@@ -56,6 +56,13 @@ __device__ __forceinline__ EventRec make_event_rec(float zu, float zd, float dl,
     r.D0 = fmaf(G1, yt * yt, p.d1k * s4 * p.R2);
     r.D1 = fmaf(2.f, G1, G2) * yt;
     r.D2 = G1 + G2;
+    if (p.gB != 0.f) {                                     // Eq. 12 with gamma != 0 (DevParams, mlem_kernels.cuh)
+        const float sec3 = sec2 * sec2 * rsqrt_approx(sec2);
+        const float G3 = sec3 * t;
+        r.B1 -= kSqrtLH * p.gB * sec3;
+        r.D0 -= p.gD0 * G3 * yt;
+        r.D1 -= (p.gD0 + 2.f * p.gB) * G3;
+    }
     r.H2p = -p.c2k * sec2 * p.half_sz2 * p.inv_px * p.inv_px;
     r.Z0 = (e.z_t - p.z0) * p.inv_px;
     r.T1 = t * p.inv_px;

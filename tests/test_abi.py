@@ -66,6 +66,13 @@ def test_argument_validation_needs_no_gpu():
     assert lib.jpet_set_option(b"chunk", -5) == binding.JPET_E_INVAL
     assert lib.jpet_set_a3_coef(ctypes.c_float(float("nan"))) == binding.JPET_E_INVAL
     assert abs(lib.jpet_get_a3_coef() - 2.0) < 1e-7
+    assert lib.jpet_set_gamma(ctypes.c_float(float("inf"))) == binding.JPET_E_INVAL
+    assert lib.jpet_get_gamma() == 0.0
+    # Eq. 12 must stay positive definite: |gamma| <= 0.5 / (sqrt(2) sigma_z sigma_dl), checked against the call's sigmas
+    assert lib.jpet_set_gamma(ctypes.c_float(1e-2)) == binding.JPET_OK
+    assert lib.jpet_mlem_iterate(None, 0, g, s, gr, None, None, None) == binding.JPET_E_INVAL
+    assert b"gamma" in lib.jpet_last_error()
+    assert lib.jpet_set_gamma(ctypes.c_float(0.0)) == binding.JPET_OK
 
 
 def test_product_does_not_reach_into_the_oracle():

@@ -28,6 +28,7 @@ def jp():
     jp.jpet_set_option("chunk", 0)
     jp.jpet_set_option("sub_tile_z", 0)
     jp.jpet_set_a3_coef(2.0)
+    jp.jpet_set_gamma(0.0)
 
 
 def geom(cfg):
@@ -96,6 +97,35 @@ def test_a3_coefficient_is_honoured(jp, oracle):
     d_gpu = (g1 - g2) / o2.max()
     assert np.max(np.abs(d_or)) > 1e-5
     assert np.max(np.abs(d_gpu - d_or)) < 0.3 * np.max(np.abs(d_or))
+
+
+@pytest.mark.parametrize("name,n,frac", [("cfg1", 20000, 0.4), ("cfg2", 100_000, -0.4), ("cfg4", 20000, 0.3), ("fig4", 100_000, 0.4)])
+def test_gamma_of_eq12(jp, oracle, name, n, frac):
+    """the general C^-1 of Eq. 12 with gamma = frac / (sqrt(2) sigma_z sigma_dl), on both
+    sides; the third-generation kernels (records), the polynomial exponent and the closed form (fig4), and the direct
+    kernel all carry the gamma terms.  The image moves by far more than the tolerance when gamma is switched on."""
+    cfg = synth.CONFIGS[name]
+    ev = synth.config_events(cfg, n=n)
+    rho = np.random.default_rng(2).uniform(0.5, 2.0, (cfg.n_y, cfg.n_z)).astype(np.float32)
+    gamma = frac / (np.sqrt(2.0) * cfg.sigma_z * cfg.sigma_dl)
+    base, _ = gpu_iterate(jp, ev, cfg, rho)
+    try:
+        jp.jpet_set_gamma(gamma)
+        oracle.set_gamma(jp.jpet_get_gamma())                 # the fp32 value the library holds
+        got, (ne, ns) = gpu_iterate(jp, ev, cfg, rho)
+        jp.jpet_set_option("force_direct", 1)
+        direct, _ = gpu_iterate(jp, ev[:20000], cfg, rho)
+        jp.jpet_set_option("force_direct", 0)
+        want, one, ons = oracle.mlem_iterate(ev, *geom(cfg), rho)
+        want_d, _, _ = oracle.mlem_iterate(ev[:20000], *geom(cfg), rho)
+    finally:
+        jp.jpet_set_option("force_direct", 0)
+        jp.jpet_set_gamma(0.0)
+        oracle.set_gamma(0.0)
+    assert rel_err(got, want) <= TOL_1
+    assert rel_err(direct, want_d) <= TOL_1
+    assert ns == ons and abs(ne - one) <= 1e-5 * one + 2
+    assert rel_err(base, want) > 20 * TOL_1
 
 
 def test_cfg1_ten_iterations(jp, oracle):
