@@ -235,6 +235,8 @@ constexpr int kShape3[4][3] = {{1, 19, 20}, {0, 17, 21}, {26, 28, 22}, {27, 23, 
 constexpr int kNumVariants3 = sizeof(kVariants3) / sizeof(kVariants3[0]);
 constexpr int kNumVariants = kNumVariants2 + kNumVariants3;
 
+int batch_chunk(int64_t n, const DevParams& dp);
+
 template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF, int MINB, bool PK>
 int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
     auto kern = jpet::mlem_rows_kernel<NW, NH, NR, NJ, HS, U, CF, MINB, PK>;
@@ -250,7 +252,7 @@ int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NW * 32, smem));
         if (per_sm < 1) return fail(JPET_E_CUDA, "event kernel does not fit on an SM (%zu B of shared memory)", smem);
         if (g_opt_ctas_per_sm > 0) per_sm = (int)std::min<int64_t>(per_sm, g_opt_ctas_per_sm);
-        int64_t max_items = bs.n / dp.chunk + (int64_t)dp.nby * dp.nbz + 1;
+        int64_t max_items = bs.n / batch_chunk(bs.n, dp) + (int64_t)dp.nby * dp.nbz + 1;
         int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(max_items, 1));
         if (g_opt_time_kernel) {
             if (g_tk_used + 2 > g_tk.size()) {
@@ -288,7 +290,7 @@ int launch_rows2(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NW * 32, smem));
         if (per_sm < 1) return fail(JPET_E_CUDA, "event kernel does not fit on an SM (%zu B of shared memory)", smem);
         if (g_opt_ctas_per_sm > 0) per_sm = (int)std::min<int64_t>(per_sm, g_opt_ctas_per_sm);
-        int64_t max_items = bs.n / dp.chunk + (int64_t)dp.nby * dp.nbz + 1;
+        int64_t max_items = bs.n / batch_chunk(bs.n, dp) + (int64_t)dp.nby * dp.nbz + 1;
         int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(max_items, 1));
         if (g_opt_time_kernel) {
             if (g_tk_used + 2 > g_tk.size()) {
@@ -326,7 +328,7 @@ int launch_rows3(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
         if (per_sm < 1) return fail(JPET_E_CUDA, "event kernel does not fit on an SM (%zu B of shared memory)", smem);
         if (g_opt_ctas_per_sm > 0) per_sm = (int)std::min<int64_t>(per_sm, g_opt_ctas_per_sm);
-        int64_t max_items = bs.n / dp.chunk + (int64_t)dp.nby * dp.nbz + 1;
+        int64_t max_items = bs.n / batch_chunk(bs.n, dp) + (int64_t)dp.nby * dp.nbz + 1;
         int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(max_items, 1));
         if (g_opt_time_kernel) {
             if (g_tk_used + 2 > g_tk.size()) {
@@ -536,8 +538,17 @@ int grid_for(int64_t M) { return (int)((M + 255) / 256); }
 
 int plan_stride() { return (g_ws.variant >= kNumVariants2 || kVariants[g_ws.variant].NA > 0) ? 16 : 3; }
 
+// Events per work item for a batch of n events: the plan's size, halved (not below 64) while the batch would give fewer
+// than four items per SM - small batches are launch- and tail-bound.
+int batch_chunk(int64_t n, const DevParams& dp) {
+    int chunk = dp.chunk;
+    if (g_opt_chunk > 0) return chunk;
+    while (chunk > 64 && n / chunk < 4 * (int64_t)g_ws.sm_count) chunk /= 2;
+    return chunk;
+}
+
 int ensure_binset(BinSet& bs, int64_t n, const DevParams& dp, bool need_sorted) {
-    size_t items_cap = (size_t)(n / dp.chunk) + (size_t)dp.nby * dp.nbz + 2;
+    size_t items_cap = (size_t)(n / batch_chunk(n, dp)) + (size_t)dp.nby * dp.nbz + 2;
     bs.stride = plan_stride();
     const size_t need_floats = (size_t)bs.stride * (size_t)std::max<int64_t>(n, 1);
     if (need_sorted && need_floats > bs.cap_events) {          // cap_events counts floats
@@ -590,7 +601,7 @@ int bin_batch(const float* events, int64_t n, BinSet& bs, const DevParams& dp, c
         jpet::bin_count_kernel<<<blocks, jpet::kBinBlock, hist_bytes, st>>>(events, (int)n, dp, g_ws.bin_of, counts, nb + 1, use_smem);
         g_launches++;
     }
-    jpet::bin_scan_kernel<<<1, 1024, 0, st>>>(counts, cursors, bs.items, bs.meta, nb, dp.chunk);
+    jpet::bin_scan_kernel<<<1, 1024, 0, st>>>(counts, cursors, bs.items, bs.meta, nb, batch_chunk(n, dp));
     g_launches++;
     if (n > 0) {
         if (bs.stride == 16)
