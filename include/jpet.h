@@ -140,6 +140,21 @@ void jpet_release(void);
 /* Text of the last error on the calling thread ("" if none).  The pointer stays valid until the next call. */
 const char *jpet_last_error(void);
 
+/* Host-side plan of the event kernel for a problem (no GPU needed; for tests and tuning): the kernel shape and the
+ * tiling that jpet_mlem_begin would choose with the current options, a3 coefficient and gamma.
+ *   out[0] variant id            out[1] degree of the exponent polynomial (0 = closed form rsqrt + ex2)
+ *   out[2] warps per event       out[3] event groups per CTA       out[4] / out[5] pixel capacity of piece A / B
+ *   out[6] HS (rows of a region) out[7] WZ (columns of a region)   out[8] / out[9] sub-tile Sy / Sz
+ *   out[10] / out[11] halo Hy / Hz                                 out[12] events per work item
+ *   out[13] dynamic shared memory per CTA [bytes]                  out[14] 1 = tiled (0: every event on the direct kernel)
+ *   out[15] / out[16] smallest / largest ellipse row count of the task table (0, 0: no table)
+ * n_out = number of int64 slots the caller provides (>= 17).  task_table_host (may be NULL) receives up to
+ * table_cap 32-bit words of the task table [(row count - out[15]) * 32 * out[2] + lane]: piece A in bits 0-15, piece B
+ * in bits 16-31; a 16-bit entry: bits 0-7 row, 8-9 part, 10-11 log2(parts), bit 15 valid (csrc/task_table.h).
+ * Returns the number of table words (>= 0), or a negative error code. */
+int64_t jpet_plan_describe(const jpet_geometry *geometry, const jpet_sigmas *sigmas, const jpet_grid *grid, int64_t *out,
+                           int32_t n_out, uint32_t *task_table_host, int64_t table_cap);
+
 /* ABI version of this header: bumped whenever a signature changes. */
 int jpet_abi_version(void);
 #define JPET_ABI_VERSION 1

@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     jpet_get_option,
     jpet_last_error,
     jpet_launch_count,
+    jpet_plan_describe,
     jpet_mlem_accumulate,
     jpet_mlem_begin,
     jpet_mlem_end,

@@ -15,7 +15,7 @@ JPET_OK, JPET_E_INVAL, JPET_E_CUDA = 0, -1, -2
 EXPORTS = (
     "jpet_sensitivity", "jpet_mlem_iterate", "jpet_reconstruct", "jpet_mlem_begin", "jpet_mlem_accumulate",
     "jpet_mlem_end", "jpet_mlem_iterate_host", "jpet_reconstruct_host", "jpet_get_counters", "jpet_count_evals",
-    "jpet_set_a3_coef", "jpet_get_a3_coef", "jpet_set_gamma", "jpet_get_gamma", "jpet_set_option", "jpet_get_option", "jpet_launch_count",
+    "jpet_set_a3_coef", "jpet_get_a3_coef", "jpet_set_gamma", "jpet_get_gamma", "jpet_plan_describe", "jpet_set_option", "jpet_get_option", "jpet_launch_count",
     "jpet_release", "jpet_last_error", "jpet_abi_version",
 )
 
@@ -73,6 +73,7 @@ def load(build_if_missing: bool = True) -> ctypes.CDLL:
         "jpet_get_a3_coef": (ctypes.c_float, []),
         "jpet_set_gamma": (ctypes.c_int, [ctypes.c_float]),
         "jpet_get_gamma": (ctypes.c_float, []),
+        "jpet_plan_describe": (i64, [G, S, Gr, p, i32, p, i64]),
         "jpet_set_option": (ctypes.c_int, [ctypes.c_char_p, i64]),
         "jpet_get_option": (i64, [ctypes.c_char_p]),
         "jpet_launch_count": (ctypes.c_uint64, []),
@@ -209,6 +210,29 @@ def jpet_set_a3_coef(k: float) -> None:
 
 def jpet_get_a3_coef() -> float:
     return float(load().jpet_get_a3_coef())
+
+
+PLAN_FIELDS = ("variant", "degree", "warps_per_event", "groups_per_cta", "cap_a", "cap_b", "HS", "WZ", "Sy", "Sz", "Hy", "Hz",
+               "chunk", "smem_bytes", "tiled", "nr_min", "nr_max")
+
+
+def jpet_plan_describe(R, L, sigma_z, sigma_dl, n_y, n_z, pixel):
+    """Host-side plan of the event kernel (no GPU needed): dict of PLAN_FIELDS plus "table", the task table as a
+    numpy uint32 array [row count - nr_min][32 * warps_per_event] (empty when the plan has none)."""
+    import numpy as np
+
+    g, s, gr = _structs(R, L, sigma_z, sigma_dl, n_y, n_z, pixel)
+    out = (ctypes.c_int64 * 17)()
+    n = load().jpet_plan_describe(g, s, gr, out, 17, None, 0)
+    if n < 0:
+        _check(int(n))
+    tab = np.zeros(int(n), dtype=np.uint32)
+    if n:
+        load().jpet_plan_describe(g, s, gr, out, 17, tab.ctypes.data, int(n))
+    plan = dict(zip(PLAN_FIELDS, [int(v) for v in out]))
+    lanes = 32 * max(plan["warps_per_event"], 1)
+    plan["table"] = tab.reshape(-1, lanes) if n else tab
+    return plan
 
 
 def jpet_set_gamma(gamma: float) -> None:

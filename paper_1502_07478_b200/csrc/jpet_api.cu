@@ -1056,6 +1056,29 @@ void jpet_release(void) {
 
 const char* jpet_last_error(void) { return g_err.c_str(); }
 
+int64_t jpet_plan_describe(const jpet_geometry* geometry, const jpet_sigmas* sigmas, const jpet_grid* grid, int64_t* out,
+                           int32_t n_out, uint32_t* task_table_host, int64_t table_cap) {
+    g_err.clear();
+    int rc = validate(geometry, sigmas, grid);
+    if (rc) return rc;
+    if (!sigmas) return fail(JPET_E_INVAL, "NULL sigmas");
+    if (!out || n_out < 17) return fail(JPET_E_INVAL, "out must hold at least 17 values");
+    DevParams dp;
+    int variant = 0;
+    size_t smem = 0;
+    std::vector<uint32_t> tab;
+    make_plan(*geometry, *sigmas, *grid, g_a3_coef, g_gamma, &dp, &variant, &smem, &tab);
+    const bool gen3 = variant >= kNumVariants2;
+    const Variant3 v3 = gen3 ? kVariants3[variant - kNumVariants2] : Variant3{0, 0, 0, 0, 0, 0, 0, 0};
+    const int64_t vals[17] = {variant, gen3 ? v3.DEG : 0, gen3 ? v3.NWE : 0, gen3 ? v3.NG : 0, gen3 ? v3.NJA : 0,
+                              gen3 ? v3.NJB : 0, dp.HS, dp.WZ, dp.Sy, dp.Sz, dp.Hy, dp.Hz, dp.chunk, (int64_t)smem,
+                              dp.t_max >= 0.f, dp.nr_min, dp.nr_max};
+    for (int i = 0; i < 17; ++i) out[i] = vals[i];
+    if (task_table_host)
+        for (int64_t i = 0; i < std::min<int64_t>(table_cap, (int64_t)tab.size()); ++i) task_table_host[i] = tab[(size_t)i];
+    return (int64_t)tab.size();
+}
+
 int jpet_abi_version(void) { return JPET_ABI_VERSION; }
 
 }  // extern "C"

@@ -148,6 +148,7 @@ def test_every_kernel_variant(jp, oracle, variant, name, n):
     try:
         got, (ne, ns) = gpu_iterate(jp, ev, cfg, rho)
         assert jp.jpet_get_option("last_variant") == variant
+        assert jp.jpet_get_option("last_overflow") == 0        # no piece longer than its register slot
     finally:
         jp.jpet_set_option("variant", -1)
     want, one, ons = oracle.mlem_iterate(ev, *geom(cfg), rho)
