@@ -229,9 +229,12 @@ constexpr Variant3 kVariants3[] = {
     {4, 4, 44, 0, 128, 1, 0, 8},     // 48: as 44, closed form
     {4, 4, 36, 0, 128, 1, 4, 8},     // 49: as 43, degree 4
     {4, 4, 44, 0, 128, 1, 5, 8},     // 50: as 44, degree 5
+    {1, 4, 20, 8, 64, 4, 4, 16},     // 51: as 38, blocks of 16 (config 2: 0.728 -> 0.710 ms)             (configs 2, 3)
+    {4, 4, 44, 0, 128, 1, 4, 16},    // 52: as 44, blocks of 16                                          (config 5)
+    {4, 4, 36, 0, 128, 1, 5, 16},    // 53: as 43, blocks of 16                                          (config 4)
 };
 // shapes in order of size: closed-form / degree-4 / degree-5 instances of each
-constexpr int kShape3[4][3] = {{1, 19, 20}, {0, 17, 21}, {26, 28, 22}, {27, 23, 29}};
+constexpr int kShape3[4][3] = {{1, 19, 20}, {0, 30, 21}, {26, 28, 32}, {27, 31, 29}};
 constexpr int kNumVariants3 = sizeof(kVariants3) / sizeof(kVariants3[0]);
 constexpr int kNumVariants = kNumVariants2 + kNumVariants3;
 
@@ -382,6 +385,9 @@ int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t sme
         case kNumVariants2 + 27: return launch_rows3<4, 4, 44, 0, 128, 1, 0, 8>(bs, dp, smem, st);
         case kNumVariants2 + 28: return launch_rows3<4, 4, 36, 0, 128, 1, 4, 8>(bs, dp, smem, st);
         case kNumVariants2 + 29: return launch_rows3<4, 4, 44, 0, 128, 1, 5, 8>(bs, dp, smem, st);
+        case kNumVariants2 + 30: return launch_rows3<1, 4, 20, 8, 64, 4, 4, 16>(bs, dp, smem, st);
+        case kNumVariants2 + 31: return launch_rows3<4, 4, 44, 0, 128, 1, 4, 16>(bs, dp, smem, st);
+        case kNumVariants2 + 32: return launch_rows3<4, 4, 36, 0, 128, 1, 5, 16>(bs, dp, smem, st);
         case 0: return launch_rows<1, 1, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
         case 1: return launch_rows<2, 1, 1, 20, 64, 4, true, 10, false>(bs, dp, smem, st);
         case 2: return launch_rows<4, 2, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);

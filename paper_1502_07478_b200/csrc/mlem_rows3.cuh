@@ -287,7 +287,7 @@ __device__ __forceinline__ void walk_block(Walk& s, float u0s, float pxs, float 
 
 template <int NJ, int HS, int DEG, int BW>
 __device__ __forceinline__ float piece_pass1(const Piece& pc, uint32_t w_addr, float pxs, int nblk, float (&preg)[NJ]) {
-    static_assert(NJ % 2 == 0 && NJ <= 12 * BW && (BW == 4 || BW == 8), "pixel capacity must be even and at most 12 blocks");
+    static_assert(NJ % 2 == 0 && NJ <= 12 * BW && (BW == 4 || BW == 8 || BW == 16), "pixel capacity must be even and at most 12 blocks");
     constexpr int NB = (NJ + BW - 1) / BW;
     Walk s;
     if constexpr (DEG > 0) {
@@ -337,12 +337,56 @@ __device__ __forceinline__ void smem_fma_if4(uint32_t addr, float P0, float P1, 
         : "memory");
 }
 
+// Eight at a time (blocks of 8 or 16 pixels): eight loads in flight before the first multiply-add.
+template <int IMM, int STRIDE, int J>
+__device__ __forceinline__ void smem_fma_if8(uint32_t addr, const float* P, float inv, int len) {
+    asm volatile(
+        "{\n\t.reg .pred p<8>;\n\t.reg .f32 t<8>;\n\t"
+        "setp.gt.s32 p0, %10, %11;\n\t"
+        "setp.gt.s32 p1, %10, %11 + 1;\n\t"
+        "setp.gt.s32 p2, %10, %11 + 2;\n\t"
+        "setp.gt.s32 p3, %10, %11 + 3;\n\t"
+        "setp.gt.s32 p4, %10, %11 + 4;\n\t"
+        "setp.gt.s32 p5, %10, %11 + 5;\n\t"
+        "setp.gt.s32 p6, %10, %11 + 6;\n\t"
+        "setp.gt.s32 p7, %10, %11 + 7;\n\t"
+        "@p0 ld.shared.f32 t0, [%0 + %12];\n\t"
+        "@p1 ld.shared.f32 t1, [%0 + %12 + %13];\n\t"
+        "@p2 ld.shared.f32 t2, [%0 + %12 + 2 * %13];\n\t"
+        "@p3 ld.shared.f32 t3, [%0 + %12 + 3 * %13];\n\t"
+        "@p4 ld.shared.f32 t4, [%0 + %12 + 4 * %13];\n\t"
+        "@p5 ld.shared.f32 t5, [%0 + %12 + 5 * %13];\n\t"
+        "@p6 ld.shared.f32 t6, [%0 + %12 + 6 * %13];\n\t"
+        "@p7 ld.shared.f32 t7, [%0 + %12 + 7 * %13];\n\t"
+        "@p0 fma.rn.f32 t0, %1, %9, t0;\n\t"
+        "@p1 fma.rn.f32 t1, %2, %9, t1;\n\t"
+        "@p2 fma.rn.f32 t2, %3, %9, t2;\n\t"
+        "@p3 fma.rn.f32 t3, %4, %9, t3;\n\t"
+        "@p4 fma.rn.f32 t4, %5, %9, t4;\n\t"
+        "@p5 fma.rn.f32 t5, %6, %9, t5;\n\t"
+        "@p6 fma.rn.f32 t6, %7, %9, t6;\n\t"
+        "@p7 fma.rn.f32 t7, %8, %9, t7;\n\t"
+        "@p0 st.shared.f32 [%0 + %12], t0;\n\t"
+        "@p1 st.shared.f32 [%0 + %12 + %13], t1;\n\t"
+        "@p2 st.shared.f32 [%0 + %12 + 2 * %13], t2;\n\t"
+        "@p3 st.shared.f32 [%0 + %12 + 3 * %13], t3;\n\t"
+        "@p4 st.shared.f32 [%0 + %12 + 4 * %13], t4;\n\t"
+        "@p5 st.shared.f32 [%0 + %12 + 5 * %13], t5;\n\t"
+        "@p6 st.shared.f32 [%0 + %12 + 6 * %13], t6;\n\t"
+        "@p7 st.shared.f32 [%0 + %12 + 7 * %13], t7;\n\t}"
+        ::"r"(addr), "f"(P[0]), "f"(P[1]), "f"(P[2]), "f"(P[3]), "f"(P[4]), "f"(P[5]), "f"(P[6]), "f"(P[7]), "f"(inv), "r"(len),
+          "n"(J), "n"(IMM), "n"(STRIDE)
+        : "memory");
+}
+
 // Pass 2: acc += P * inv over the same pixels (private region, one owner lane per pixel: plain read-modify-write).
 template <int JB, int NJ, int HS, int BW>
 __device__ __forceinline__ void scatter_block(uint32_t aa, const float (&preg)[NJ], float inv, int len) {
     static_for<0, BW / 4>([&](auto kc) {
-        constexpr int J = JB + 4 * decltype(kc)::value;
-        if constexpr (J + 3 < NJ) smem_fma_if4<4 * J * HS, 4 * HS, J>(aa, preg[J], preg[J + 1], preg[J + 2], preg[J + 3], inv, len);
+        constexpr int K = decltype(kc)::value, J = JB + 4 * K;
+        if constexpr (BW >= 8 && (K % 2 == 0) && J + 7 < NJ) smem_fma_if8<4 * J * HS, 4 * HS, J>(aa, &preg[J], inv, len);
+        else if constexpr (BW >= 8 && (K % 2 == 1) && J + 3 < NJ) { /* second half of an eight */ }
+        else if constexpr (J + 3 < NJ) smem_fma_if4<4 * J * HS, 4 * HS, J>(aa, preg[J], preg[J + 1], preg[J + 2], preg[J + 3], inv, len);
         else static_for<0, 4>([&](auto qc) {
             constexpr int Q = J + decltype(qc)::value;
             if constexpr (Q < NJ) smem_fma_if<4 * Q * HS, Q>(aa, preg[Q], inv, len);
