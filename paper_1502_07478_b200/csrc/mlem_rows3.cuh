@@ -217,7 +217,8 @@ __device__ __forceinline__ void walk_pair(Walk& s, float& p0, float& p1) {
 // DEG > 0: the pairs of a block in LOCKSTEP - all u' pairs, then one Horner step for every pair, ..., then the ex2, the
 // masks and the denominator terms (two accumulators).  ptxas keeps source order: written pair after pair it issued the
 // four dependent FFMA2 of a Horner chain back to back (4-cycle waits, the largest stall of the kernel in ncu).
-template <int JB, int NJ, int HS, int DEG, int BW>
+// NFULL: the first NFULL pixels of the block belong to the chord in EVERY lane of the warp (no masks for them).
+template <int JB, int NJ, int HS, int DEG, int BW, int NFULL = 0>
 __device__ __forceinline__ void walk_block_lockstep(Walk& s, float u0s, float pxs, float (&preg)[NJ]) {
     constexpr int NPAIR = (NJ - JB < BW ? NJ - JB : BW) / 2;
     const float vb = fmaf((float)JB, pxs, u0s);
@@ -243,7 +244,9 @@ __device__ __forceinline__ void walk_block_lockstep(Walk& s, float u0s, float px
     f32x2 DENB = pack2(0.f, 0.f);
     static_for<0, NPAIR>([&](auto kc) {
         constexpr int K = decltype(kc)::value, J = JB + 2 * K;
-        const float x0 = J < s.len ? x[2 * K] : 0.f, x1 = J + 1 < s.len ? x[2 * K + 1] : 0.f;
+        float x0 = x[2 * K], x1 = x[2 * K + 1];
+        if constexpr (J - JB >= NFULL) x0 = J < s.len ? x0 : 0.f;
+        if constexpr (J + 1 - JB >= NFULL) x1 = J + 1 < s.len ? x1 : 0.f;
         const f32x2 W2 = pack2(lds_imm<4 * J * HS>(s.wa), lds_imm<4 * (J + 1) * HS>(s.wa));
         if constexpr (K & 1) DENB = fma2(pack2(x0, x1), W2, DENB);
         else s.DEN2 = fma2(pack2(x0, x1), W2, s.DEN2);
@@ -253,10 +256,10 @@ __device__ __forceinline__ void walk_block_lockstep(Walk& s, float u0s, float px
     if constexpr (NPAIR > 1) s.DEN2 = add2(s.DEN2, DENB);
 }
 
-template <int JB, int NJ, int HS, int DEG, int BW>
+template <int JB, int NJ, int HS, int DEG, int BW, int NFULL = 0>
 __device__ __forceinline__ void walk_block(Walk& s, float u0s, float pxs, float (&preg)[NJ]) {
     if constexpr (DEG > 0) {
-        if constexpr (JB < NJ) walk_block_lockstep<JB, NJ, HS, DEG, BW>(s, u0s, pxs, preg);
+        if constexpr (JB < NJ) walk_block_lockstep<JB, NJ, HS, DEG, BW, NFULL>(s, u0s, pxs, preg);
     } else {
         const float vb = fmaf((float)JB, pxs, u0s);
         s.V2 = pack2(vb, vb + pxs);
@@ -285,8 +288,10 @@ __device__ __forceinline__ void walk_block(Walk& s, float u0s, float pxs, float 
         case 0: break;                                                         \
     }
 
+// full8 (warp-uniform): every lane of the warp has at least 8 pixels, so block 0 runs its first 8 pixels without masks.
 template <int NJ, int HS, int DEG, int BW>
-__device__ __forceinline__ float piece_pass1(const Piece& pc, uint32_t w_addr, float pxs, int nblk, float (&preg)[NJ]) {
+__device__ __forceinline__ float piece_pass1(const Piece& pc, uint32_t w_addr, float pxs, int nblk, float (&preg)[NJ],
+                                             bool full8 = false) {
     static_assert(NJ % 2 == 0 && NJ <= 12 * BW && (BW == 4 || BW == 8 || BW == 16), "pixel capacity must be even and at most 12 blocks");
     constexpr int NB = (NJ + BW - 1) / BW;
     Walk s;
@@ -302,7 +307,11 @@ __device__ __forceinline__ float piece_pass1(const Piece& pc, uint32_t w_addr, f
     s.wa = w_addr + pc.off;
     s.len = pc.rc.len;
     const float u0s = pc.rc.u0s;
-#define JPET_WALK(B) walk_block<(B) * BW, NJ, HS, DEG, BW>(s, u0s, pxs, preg)
+#define JPET_WALK(B)                                                                          \
+    do {                                                                                      \
+        if ((B) == 0 && DEG > 0 && BW >= 8 && NJ >= 8 && full8) walk_block<0, NJ, HS, DEG, BW, 8>(s, u0s, pxs, preg); \
+        else walk_block<(B) * BW, NJ, HS, DEG, BW>(s, u0s, pxs, preg);                        \
+    } while (0)
     JPET_BLOCK_CASES(JPET_WALK)
 #undef JPET_WALK
     float q0, q1;
@@ -379,12 +388,47 @@ __device__ __forceinline__ void smem_fma_if8(uint32_t addr, const float* P, floa
         : "memory");
 }
 
+// Unpredicated form of smem_fma_if8 (every lane owns all eight pixels).
+template <int IMM, int STRIDE>
+__device__ __forceinline__ void smem_fma8(uint32_t addr, const float* P, float inv) {
+    asm volatile(
+        "{\n\t.reg .f32 t<8>;\n\t"
+        "ld.shared.f32 t0, [%0 + %10];\n\t"
+        "ld.shared.f32 t1, [%0 + %10 + %11];\n\t"
+        "ld.shared.f32 t2, [%0 + %10 + 2 * %11];\n\t"
+        "ld.shared.f32 t3, [%0 + %10 + 3 * %11];\n\t"
+        "ld.shared.f32 t4, [%0 + %10 + 4 * %11];\n\t"
+        "ld.shared.f32 t5, [%0 + %10 + 5 * %11];\n\t"
+        "ld.shared.f32 t6, [%0 + %10 + 6 * %11];\n\t"
+        "ld.shared.f32 t7, [%0 + %10 + 7 * %11];\n\t"
+        "fma.rn.f32 t0, %1, %9, t0;\n\t"
+        "fma.rn.f32 t1, %2, %9, t1;\n\t"
+        "fma.rn.f32 t2, %3, %9, t2;\n\t"
+        "fma.rn.f32 t3, %4, %9, t3;\n\t"
+        "fma.rn.f32 t4, %5, %9, t4;\n\t"
+        "fma.rn.f32 t5, %6, %9, t5;\n\t"
+        "fma.rn.f32 t6, %7, %9, t6;\n\t"
+        "fma.rn.f32 t7, %8, %9, t7;\n\t"
+        "st.shared.f32 [%0 + %10], t0;\n\t"
+        "st.shared.f32 [%0 + %10 + %11], t1;\n\t"
+        "st.shared.f32 [%0 + %10 + 2 * %11], t2;\n\t"
+        "st.shared.f32 [%0 + %10 + 3 * %11], t3;\n\t"
+        "st.shared.f32 [%0 + %10 + 4 * %11], t4;\n\t"
+        "st.shared.f32 [%0 + %10 + 5 * %11], t5;\n\t"
+        "st.shared.f32 [%0 + %10 + 6 * %11], t6;\n\t"
+        "st.shared.f32 [%0 + %10 + 7 * %11], t7;\n\t}"
+        ::"r"(addr), "f"(P[0]), "f"(P[1]), "f"(P[2]), "f"(P[3]), "f"(P[4]), "f"(P[5]), "f"(P[6]), "f"(P[7]), "f"(inv),
+          "n"(IMM), "n"(STRIDE)
+        : "memory");
+}
+
 // Pass 2: acc += P * inv over the same pixels (private region, one owner lane per pixel: plain read-modify-write).
-template <int JB, int NJ, int HS, int BW>
+template <int JB, int NJ, int HS, int BW, int NFULL = 0>
 __device__ __forceinline__ void scatter_block(uint32_t aa, const float (&preg)[NJ], float inv, int len) {
     static_for<0, BW / 4>([&](auto kc) {
         constexpr int K = decltype(kc)::value, J = JB + 4 * K;
-        if constexpr (BW >= 8 && (K % 2 == 0) && J + 7 < NJ) smem_fma_if8<4 * J * HS, 4 * HS, J>(aa, &preg[J], inv, len);
+        if constexpr (NFULL == 8 && K == 0 && J + 7 < NJ) smem_fma8<4 * J * HS, 4 * HS>(aa, &preg[J], inv);
+        else if constexpr (BW >= 8 && (K % 2 == 0) && J + 7 < NJ) smem_fma_if8<4 * J * HS, 4 * HS, J>(aa, &preg[J], inv, len);
         else if constexpr (BW >= 8 && (K % 2 == 1) && J + 3 < NJ) { /* second half of an eight */ }
         else if constexpr (J + 3 < NJ) smem_fma_if4<4 * J * HS, 4 * HS, J>(aa, preg[J], preg[J + 1], preg[J + 2], preg[J + 3], inv, len);
         else static_for<0, 4>([&](auto qc) {
@@ -395,9 +439,13 @@ __device__ __forceinline__ void scatter_block(uint32_t aa, const float (&preg)[N
 }
 
 template <int NJ, int HS, int BW>
-__device__ __forceinline__ void piece_pass2(uint32_t aa, const float (&preg)[NJ], float inv, int len, int nblk) {
+__device__ __forceinline__ void piece_pass2(uint32_t aa, const float (&preg)[NJ], float inv, int len, int nblk, bool full8 = false) {
     constexpr int NB = (NJ + BW - 1) / BW;
-#define JPET_SCATTER(B) scatter_block<(B) * BW, NJ, HS, BW>(aa, preg, inv, len)
+#define JPET_SCATTER(B)                                                                      \
+    do {                                                                                     \
+        if ((B) == 0 && BW >= 8 && NJ >= 8 && full8) scatter_block<0, NJ, HS, BW, 8>(aa, preg, inv, len); \
+        else scatter_block<(B) * BW, NJ, HS, BW>(aa, preg, inv, len);                        \
+    } while (0)
     JPET_BLOCK_CASES(JPET_SCATTER)
 #undef JPET_SCATTER
 }
@@ -431,7 +479,9 @@ __device__ __forceinline__ void process_event_rows3(const float4 r0, const float
     pieces_setup<NJA, NJB, HS, DEG>(tab_n[glane], r0, r1, r2, r3, p, ry0, rz0, col_lo, col_hi, A, B, overflow);
     const int nbA = (__reduce_max_sync(0xffffffffu, A.rc.len) + BW - 1) / BW;
     float pregA[NJA];
-    float denom = piece_pass1<NJA, HS, DEG, BW>(A, w_addr, p.pxs, nbA, pregA);
+    // (one-warp groups only: in the 512-thread CTAs of the four-warp groups the second copy of block 0 costs more than it saves)
+    const bool fullA = NWE == 1 && DEG > 0 && BW >= 8 && NJA >= 8 && __reduce_min_sync(0xffffffffu, A.rc.len) >= 8;
+    float denom = piece_pass1<NJA, HS, DEG, BW>(A, w_addr, p.pxs, nbA, pregA, fullA);
     my_evals += A.rc.len;
     constexpr int NJB1 = NJB > 0 ? NJB : 2;
     float pregB[NJB1];
@@ -454,7 +504,7 @@ __device__ __forceinline__ void process_event_rows3(const float4 r0, const float
     const bool ok = (denom > 0.f) && (denom < 3.0e38f);
     if (!ok) { if (glane == 0) my_skipped += 1; return; }
     const float inv = 1.f / denom;
-    piece_pass2<NJA, HS, BW>(a_addr + A.off, pregA, inv, A.rc.len, nbA);
+    piece_pass2<NJA, HS, BW>(a_addr + A.off, pregA, inv, A.rc.len, nbA, fullA);
     if constexpr (NJB > 0) piece_pass2<NJB, HS, BW>(a_addr + B.off, pregB, inv, B.rc.len, nbB);
 }
 
