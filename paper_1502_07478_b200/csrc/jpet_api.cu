@@ -232,6 +232,8 @@ constexpr Variant3 kVariants3[] = {
     {1, 4, 20, 8, 64, 4, 4, 16},     // 51: as 38, blocks of 16 (config 2: 0.728 -> 0.710 ms)             (configs 2, 3)
     {4, 4, 44, 0, 128, 1, 4, 16},    // 52: as 44, blocks of 16                                          (config 5)
     {4, 4, 36, 0, 128, 1, 5, 16},    // 53: as 43, blocks of 16                                          (config 4)
+    {3, 4, 36, 8, 128, 1, 5, 16},    // 54: three warps per event: 96 central rows + the few rows beyond them as B pieces (config 4)
+    {3, 4, 44, 8, 128, 1, 4, 16},    // 55: as 54 for chords of up to 44 pixels, degree 4
 };
 // shapes in order of size: closed-form / degree-4 / degree-5 instances of each
 constexpr int kShape3[4][3] = {{1, 19, 20}, {0, 30, 21}, {26, 28, 32}, {27, 31, 29}};
@@ -388,6 +390,8 @@ int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t sme
         case kNumVariants2 + 30: return launch_rows3<1, 4, 20, 8, 64, 4, 4, 16>(bs, dp, smem, st);
         case kNumVariants2 + 31: return launch_rows3<4, 4, 44, 0, 128, 1, 4, 16>(bs, dp, smem, st);
         case kNumVariants2 + 32: return launch_rows3<4, 4, 36, 0, 128, 1, 5, 16>(bs, dp, smem, st);
+        case kNumVariants2 + 33: return launch_rows3<3, 4, 36, 8, 128, 1, 5, 16>(bs, dp, smem, st);
+        case kNumVariants2 + 34: return launch_rows3<3, 4, 44, 8, 128, 1, 4, 16>(bs, dp, smem, st);
         case 0: return launch_rows<1, 1, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
         case 1: return launch_rows<2, 1, 1, 20, 64, 4, true, 10, false>(bs, dp, smem, st);
         case 2: return launch_rows<4, 2, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
@@ -479,6 +483,9 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
             return 1.4427 * (0.5 * eb * std::pow(xb, deg - 1) / (1.0 - xb) + 0.5 * std::pow(xb, deg + 1) / (deg + 1));
         };
         const int deg_sel = g_opt_poly_off ? 0 : (trunc_err(4) <= 2e-5 ? 1 : (trunc_err(5) <= 2e-5 ? 2 : 0));
+        // ellipses of at most ~100 rows on three warps instead of four (config 4: 91 rows on 128 lanes leave a quarter of
+        // the lanes idle; 14.60 -> 14.02 ms per 5x10^6 events), the few rows beyond 96 as B pieces
+        if (deg_sel == 2 && nr_hi > 64 && nr_hi <= 104 && fits3(kVariants3[33])) v = kNumVariants2 + 33;
         for (int sh = 0; sh < 4 && v < 0; ++sh)
             if (fits3(kVariants3[kShape3[sh][deg_sel]])) v = kNumVariants2 + kShape3[sh][deg_sel];
         const int order[] = {14, 12, 15, 16, 0, 8, 9, 10, 5};
