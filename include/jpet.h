@@ -124,9 +124,14 @@ float jpet_get_gamma(void);
  *   "chunk"        events per work item of the tiled path; 0 = automatic
  *   "sub_tile_z"   width in pixels of the image sub-tiles the events are sorted by; 0 = automatic
  *   "ctas_per_sm"  cap on resident CTAs per SM for the persistent grid; 0 = automatic
- *   "time_kernel"  1 = bracket each tiled event-kernel launch with CUDA events on its stream; the duration of the
- *                  last launch is then read with jpet_get_option("last_kernel_ns") (synchronises on that launch)
- * jpet_get_option also answers "last_variant", "last_tiled", "last_smem_bytes" (what the last iteration used).
+ *   "poly_off"     1 = never evaluate the exponent of Eq. 7 as a polynomial in u (always rsqrt + ex2); 0 = automatic:
+ *                  the plan bounds the truncation error and picks degree 4, 5 or the closed form
+ *   "time_kernel"  1 = bracket each tiled event-kernel launch with CUDA events on its stream; the summed duration of
+ *                  the launches of the last iteration (one per batch of events) is then read with
+ *                  jpet_get_option("last_kernel_ns") (synchronises on the last one), their number with
+ *                  "last_kernel_launches"
+ * jpet_get_option also answers "last_variant", "last_tiled", "last_smem_bytes" (what the last iteration used) and
+ * "last_overflow" (row pieces that did not fit their register slot: 0 by construction; synchronises the device).
  * Returns JPET_E_INVAL for an unknown name or a value out of range. */
 int jpet_set_option(const char *name, int64_t value);
 int64_t jpet_get_option(const char *name);
