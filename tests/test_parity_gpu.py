@@ -384,3 +384,43 @@ def test_direct_path_and_chunking(jp, oracle):
     finally:
         jp.jpet_set_option("force_direct", 0)
         jp.jpet_set_option("chunk", 0)
+
+
+def test_random_geometries(jp, oracle):
+    """Forty seeded random problems - strip distance and length, both sigmas, non-square grids of 5 to 72 pixels a side,
+    pixel sizes, every third one with the off-diagonal gamma of Eq. 12 - dense enough in events that ellipse-boundary
+    ties (R20) stay below the tolerance: whatever kernel shape, degree or fall-back the plan picks must match the oracle."""
+    import torch
+
+    rng = np.random.default_rng(1)
+    done, shapes = 0, set()
+    try:
+        while done < 40:
+            R, L = float(rng.uniform(100, 600)), float(rng.uniform(200, 900))
+            sz, sdl = float(rng.uniform(2, 30)), float(rng.uniform(8, 120))
+            if (1.07 * sz + 1.8 * sz * sz / sdl) / R > 0.45:          # outside the domain of validity (DESIGN.md R17)
+                continue
+            n_y, n_z = int(rng.integers(5, 72)), int(rng.integers(5, 72))
+            pixel = float(min(0.95 * R / (0.5 * n_y), rng.uniform(0.6, 8.0)))
+            hy, hz = 0.5 * n_y * pixel, 0.5 * n_z * pixel
+            phantom = (synth.Primitive("E", 0.0, 0.0, 0.7 * min(hy, 0.8 * R), 0.7 * min(hz, 0.45 * L), 0.0, 1.0),)
+            ev = synth.generate_events(phantom, int(rng.integers(30000, 60000)), R, L, sz, sdl, seed=int(rng.integers(1 << 30)))
+            rho = rng.uniform(0.5, 2.0, (n_y, n_z)).astype(np.float32)
+            gamma = float(rng.uniform(-0.4, 0.4) / (np.sqrt(2) * sz * sdl)) if done % 3 == 0 else 0.0
+            jp.jpet_set_gamma(gamma)
+            oracle.set_gamma(jp.jpet_get_gamma())
+            g = (R, L, sz, sdl, n_y, n_z, pixel)
+            r = torch.from_numpy(rho).cuda().reshape(-1)
+            out = torch.empty_like(r)
+            jp.jpet_mlem_iterate(torch.from_numpy(ev).cuda(), *g, r, out)
+            ne, ns = jp.jpet_get_counters()
+            want, one, ons = oracle.mlem_iterate(ev, *g, rho)
+            got = out.cpu().numpy().astype(np.float64).reshape(n_y, n_z)
+            assert rel_err(got, want) <= TOL_1, (g, gamma, jp.jpet_get_option("last_variant"))
+            assert ns == ons and abs(ne - one) <= 1e-5 * one + 3 and jp.jpet_get_option("last_overflow") == 0
+            shapes.add((jp.jpet_get_option("last_variant"), jp.jpet_get_option("last_tiled")))
+            done += 1
+    finally:
+        jp.jpet_set_gamma(0.0)
+        oracle.set_gamma(0.0)
+    assert len(shapes) >= 5          # the sweep exercises several kernel shapes and the direct fall-back
