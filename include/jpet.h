@@ -126,6 +126,8 @@ float jpet_get_gamma(void);
  *   "ctas_per_sm"  cap on resident CTAs per SM for the persistent grid; 0 = automatic
  *   "poly_off"     1 = never evaluate the exponent of Eq. 7 as a polynomial in u (always rsqrt + ex2); 0 = automatic:
  *                  the plan bounds the truncation error and picks degree 4, 5 or the closed form
+ *   "pdl"          1 (default) = launch the kernels of an iteration with programmatic stream serialisation (each starts
+ *                  with griddepcontrol.wait: only launch latency overlaps the previous kernel); 0 = plain launches
  *   "time_kernel"  1 = bracket each tiled event-kernel launch with CUDA events on its stream; the summed duration of
  *                  the launches of the last iteration (one per batch of events) is then read with
  *                  jpet_get_option("last_kernel_ns") (synchronises on the last one), their number with

@@ -32,6 +32,7 @@ int64_t g_opt_time_kernel = 0;   // 1 = bracket the tiled event kernel with CUDA
 std::vector<cudaEvent_t> g_tk;    // event pairs around the tiled event kernel launches since the last begin
 size_t g_tk_used = 0;
 int64_t g_opt_variant = -1;      // -1 = automatic
+int64_t g_opt_pdl = 1;           // 1 = launch the kernels of an iteration with programmatic stream serialisation
 int64_t g_opt_poly_off = 0;      // 1 = never pick a polynomial-exponent variant automatically
 int64_t g_opt_ctas_per_sm = 0;   // 0 = automatic
 constexpr int64_t kMaxBatch = 10000000;          // events per launch (BASELINE config 5: 10M-event batches)
@@ -93,6 +94,7 @@ struct Workspace {
     size_t cap_bin_of = 0;
     int* counts = nullptr;      // [nb + 1] counts, then [nb + 1] cursors
     size_t cap_counts = 0;
+    int counts_clean_nb = -1;   // bin count of the layout the (zeroed) counts buffer was last used with
     BinSet scratch;             // used by iterate / accumulate
     std::vector<BinSet> kept;   // used by reconstruct: one per batch, binned once
     float* kept_sorted = nullptr;
@@ -242,6 +244,25 @@ constexpr int kNumVariants = kNumVariants2 + kNumVariants3;
 
 int batch_chunk(int64_t n, const DevParams& dp);
 
+// Kernel launch with the programmatic-stream-serialisation attribute (PDL): the kernel may be scheduled while the
+// previous kernel of the stream drains; every kernel launched this way starts with pdl_wait() (mlem_kernels.cuh), so
+// it reads nothing the previous kernel wrote before that kernel has completed.  Hides most of the launch gaps between
+// the eight kernels of an iteration (config 2: a 0.8 ms step).
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = g_opt_pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF, int MINB, bool PK>
 int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
     auto kern = jpet::mlem_rows_kernel<NW, NH, NR, NJ, HS, U, CF, MINB, PK>;
@@ -273,7 +294,8 @@ int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t
     }
     // direct path for the events of the last bin (all events when no region fits shared memory)
     int dgrid = dp.t_max >= 0.f ? g_ws.sm_count : g_ws.sm_count * 16;
-    jpet::mlem_rows_direct_kernel<<<dgrid, 128, 0, stream>>>(bs.sorted, bs.stride, bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.counters);
+    CUDA_TRY(launch_pdl(jpet::mlem_rows_direct_kernel, dim3(dgrid), dim3(128), 0, stream, bs.sorted, bs.stride, bs.meta, dp, g_ws.wT,
+                        g_ws.accT, g_ws.counters));
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     return JPET_OK;
@@ -311,7 +333,8 @@ int launch_rows2(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_
         CUDA_TRY(cudaGetLastError());
     }
     int dgrid = dp.t_max >= 0.f ? g_ws.sm_count : g_ws.sm_count * 16;
-    jpet::mlem_rows_direct_kernel<<<dgrid, 128, 0, stream>>>(bs.sorted, bs.stride, bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.counters);
+    CUDA_TRY(launch_pdl(jpet::mlem_rows_direct_kernel, dim3(dgrid), dim3(128), 0, stream, bs.sorted, bs.stride, bs.meta, dp, g_ws.wT,
+                        g_ws.accT, g_ws.counters));
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     return JPET_OK;
@@ -342,14 +365,15 @@ int launch_rows3(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_
             }
             CUDA_TRY(cudaEventRecord(g_tk[g_tk_used], stream));
         }
-        kern<<<grid, NT, smem, stream>>>(reinterpret_cast<const jpet::EventRec*>(bs.sorted), bs.items, bs.meta, dp, g_ws.wT,
-                                         g_ws.accT, g_ws.tab, g_ws.counters);
+        CUDA_TRY(launch_pdl(kern, dim3(grid), dim3(NT), smem, stream, reinterpret_cast<const jpet::EventRec*>(bs.sorted), bs.items,
+                            bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.tab, g_ws.counters));
         g_launches++;
         if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk[g_tk_used + 1], stream)); g_tk_used += 2; }
         CUDA_TRY(cudaGetLastError());
     }
     int dgrid = dp.t_max >= 0.f ? g_ws.sm_count : g_ws.sm_count * 16;
-    jpet::mlem_rows_direct_kernel<<<dgrid, 128, 0, stream>>>(bs.sorted, bs.stride, bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.counters);
+    CUDA_TRY(launch_pdl(jpet::mlem_rows_direct_kernel, dim3(dgrid), dim3(128), 0, stream, bs.sorted, bs.stride, bs.meta, dp, g_ws.wT,
+                        g_ws.accT, g_ws.counters));
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     return JPET_OK;
@@ -602,24 +626,29 @@ int bin_batch(const float* events, int64_t n, BinSet& bs, const DevParams& dp, c
         g_ws.counts = nullptr; g_ws.cap_counts = 0;
         CUDA_TRY(cudaMalloc(&g_ws.counts, sizeof(int) * 2 * (size_t)(nb + 1)));
         g_ws.cap_counts = (size_t)(2 * (nb + 1));
+        g_ws.counts_clean_nb = -1;
     }
     int* counts = g_ws.counts;
     int* cursors = g_ws.counts + (nb + 1);
-    CUDA_TRY(cudaMemsetAsync(counts, 0, sizeof(int) * (nb + 1), st));
+    if (g_ws.counts_clean_nb != nb) {        // bin_scan_kernel leaves the counts zeroed: a memset only when the layout changes
+        CUDA_TRY(cudaMemsetAsync(counts, 0, sizeof(int) * (nb + 1), st));
+        g_ws.counts_clean_nb = nb;
+    }
     const int per_block = jpet::kBinBlock * jpet::kBinPer;
     const int blocks = (int)((n + per_block - 1) / per_block);
     const int use_smem = nb + 1 <= jpet::kBinSmemMax;
     const size_t hist_bytes = use_smem ? sizeof(int) * (size_t)(nb + 1) : 0;
     if (n > 0) {
-        jpet::bin_count_kernel<<<blocks, jpet::kBinBlock, hist_bytes, st>>>(events, (int)n, dp, g_ws.bin_of, counts, nb + 1, use_smem);
+        CUDA_TRY(launch_pdl(jpet::bin_count_kernel, dim3(blocks), dim3(jpet::kBinBlock), hist_bytes, st, events, (int)n, dp, g_ws.bin_of,
+                            counts, nb + 1, use_smem));
         g_launches++;
     }
-    jpet::bin_scan_kernel<<<1, 1024, 0, st>>>(counts, cursors, bs.items, bs.meta, nb, batch_chunk(n, dp));
+    CUDA_TRY(launch_pdl(jpet::bin_scan_kernel, dim3(1), dim3(1024), 0, st, counts, cursors, bs.items, bs.meta, nb, batch_chunk(n, dp)));
     g_launches++;
     if (n > 0) {
         if (bs.stride == 16)
-            jpet::bin_scatter_rec_kernel<<<blocks, jpet::kBinBlock, hist_bytes, st>>>(
-                events, (int)n, g_ws.bin_of, cursors, reinterpret_cast<jpet::EventRec*>(bs.sorted), dp, nb + 1, use_smem);
+            CUDA_TRY(launch_pdl(jpet::bin_scatter_rec_kernel, dim3(blocks), dim3(jpet::kBinBlock), hist_bytes, st, events, (int)n,
+                                g_ws.bin_of, cursors, reinterpret_cast<jpet::EventRec*>(bs.sorted), dp, nb + 1, use_smem));
         else
             jpet::bin_scatter_kernel<<<blocks, jpet::kBinBlock, hist_bytes, st>>>(events, (int)n, g_ws.bin_of, cursors, bs.sorted, nb + 1, use_smem);
         g_launches++;
@@ -630,7 +659,8 @@ int bin_batch(const float* events, int64_t n, BinSet& bs, const DevParams& dp, c
 }
 
 int run_binset(BinSet& bs, cudaStream_t st) {
-    CUDA_TRY(cudaMemsetAsync(bs.meta + 3, 0, sizeof(int), st));      // work counter
+    // the work counter meta[3] is zero here: bin_scan_kernel zeroes it and mlem_rows_direct_kernel, the last kernel of every
+    // run over a sorted set, zeroes it again
     return dispatch_rows(g_ws.variant, bs, g_ws.dp, g_ws.smem, st);
 }
 
@@ -670,7 +700,8 @@ int do_begin(const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr,
                                  cudaMemcpyHostToDevice, st));
     }
     g_tk_used = 0;                 // last_kernel_ns covers the event-kernel launches of one iteration
-    jpet::prepass_kernel<<<grid_for(M), 256, 0, st>>>(g_ws.s, rho_in, g_ws.wT, g_ws.accT, gr->n_y, gr->n_z, g_ws.counters);
+    CUDA_TRY(launch_pdl(jpet::prepass_kernel, dim3(grid_for(M)), dim3(256), 0, st, (const float*)g_ws.s, rho_in, g_ws.wT, g_ws.accT,
+                        gr->n_y, gr->n_z, g_ws.counters));
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     g_ws.open = true;
@@ -694,7 +725,8 @@ int do_accumulate(const float* events, int64_t n, cudaStream_t st) {
 int do_end(const float* rho_in, float* rho_out, cudaStream_t st) {
     if (!g_ws.open) return fail(JPET_E_INVAL, "jpet_mlem_end without jpet_mlem_begin");
     if (!rho_in || !rho_out) return fail(JPET_E_INVAL, "NULL image pointer");
-    jpet::finalise_kernel<<<grid_for(g_ws.M), 256, 0, st>>>(g_ws.s, rho_in, g_ws.accT, rho_out, g_ws.grid.n_y, g_ws.grid.n_z);
+    CUDA_TRY(launch_pdl(jpet::finalise_kernel, dim3(grid_for(g_ws.M)), dim3(256), 0, st, (const float*)g_ws.s, rho_in,
+                        (const float*)g_ws.accT, rho_out, g_ws.grid.n_y, g_ws.grid.n_z));
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     g_ws.open = false;
@@ -1007,6 +1039,8 @@ int jpet_set_option(const char* name, int64_t value) {
         g_opt_variant = value;
     } else if (!strcmp(name, "poly_off")) {
         g_opt_poly_off = value != 0;
+    } else if (!strcmp(name, "pdl")) {
+        g_opt_pdl = value != 0;
     } else if (!strcmp(name, "ctas_per_sm")) {
         if (value < 0 || value > 32) return fail(JPET_E_INVAL, "ctas_per_sm must be 0 (auto) .. 32");
         g_opt_ctas_per_sm = value;
@@ -1035,6 +1069,7 @@ int64_t jpet_get_option(const char* name) {
     if (!strcmp(name, "last_kernel_launches")) return (int64_t)(g_tk_used / 2);
     if (!strcmp(name, "variant")) return g_opt_variant;
     if (!strcmp(name, "poly_off")) return g_opt_poly_off;
+    if (!strcmp(name, "pdl")) return g_opt_pdl;
     if (!strcmp(name, "ctas_per_sm")) return g_opt_ctas_per_sm;
     if (!strcmp(name, "last_variant")) return g_ws.variant;
     if (!strcmp(name, "last_smem_bytes")) return (int64_t)g_ws.smem;
@@ -1052,6 +1087,7 @@ uint64_t jpet_launch_count(void) { return g_launches.load(); }
 void jpet_release(void) {
     cudaFree(g_ws.s); cudaFree(g_ws.wT); cudaFree(g_ws.accT); cudaFree(g_ws.rho_a); cudaFree(g_ws.rho_b);
     cudaFree(g_ws.counters); cudaFree(g_ws.stage); cudaFree(g_ws.bin_of); cudaFree(g_ws.counts); cudaFree(g_ws.kept_sorted);
+    g_ws.counts_clean_nb = -1;
     cudaFree(g_ws.tab);
     free_binset(g_ws.scratch);
     for (auto& bs : g_ws.kept) free_binset(bs);

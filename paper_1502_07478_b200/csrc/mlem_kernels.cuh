@@ -105,6 +105,11 @@ __device__ __forceinline__ void red_add_f32(float* addr, float v) {
     asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
 }
 
+// Programmatic dependent launch (jpet_api.cu launches the kernels of an iteration with the stream-serialisation
+// attribute): everything before this call may overlap the tail of the previous kernel in the stream; nothing that
+// the previous kernel wrote is read before it.  A no-op for a kernel launched without the attribute.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 constexpr float kLH = 0.72134752044448170368f;       // log2(e) / 2
 constexpr float kSqrtLH = 0.84932180028801904272f;   // sqrt(log2(e) / 2)
 
@@ -124,6 +129,7 @@ __global__ void sensitivity_kernel(float* __restrict__ s, int n_y, int n_z, doub
 // wT[iz * n_y + iy] = s[iy * n_z + iz] * rho_in[...]; accT = 0; counters = 0
 __global__ void prepass_kernel(const float* __restrict__ s, const float* __restrict__ rho_in, float* __restrict__ wT,
                                float* __restrict__ accT, int n_y, int n_z, unsigned long long* __restrict__ counters) {
+    pdl_wait();
     int i = blockIdx.x * blockDim.x + threadIdx.x;   // transposed index: consecutive threads = consecutive iy
     if (i < n_y * n_z) {
         int iz = i / n_y, iy = i - iz * n_y;
@@ -136,6 +142,7 @@ __global__ void prepass_kernel(const float* __restrict__ s, const float* __restr
 
 __global__ void finalise_kernel(const float* __restrict__ s, const float* rho_in, const float* __restrict__ accT,
                                 float* rho_out, int n_y, int n_z) {
+    pdl_wait();
     int i = blockIdx.x * blockDim.x + threadIdx.x;   // row-major index
     if (i >= n_y * n_z) return;
     int iy = i / n_z, iz = i - iy * n_z;
@@ -265,6 +272,7 @@ constexpr int kBinBlock = 256, kBinPer = 8, kBinSmemMax = 12288;   // threads, e
 __global__ void __launch_bounds__(kBinBlock)
 bin_count_kernel(const float* __restrict__ events, int n, const __grid_constant__ DevParams p, int* __restrict__ bin_of,
                  int* __restrict__ counts, int nb1, int use_smem) {
+    pdl_wait();
     extern __shared__ int hist[];
     const int tid = threadIdx.x;
     if (use_smem) {
@@ -294,8 +302,9 @@ bin_count_kernel(const float* __restrict__ events, int n, const __grid_constant_
 // (chunk events) come first in the list, the partly filled last item of every bin after them, so that the persistent
 // event kernel ends on small items.
 // meta[0] = number of items, meta[1] = start of the direct bin, meta[2] = its count, meta[3] = work counter (zeroed)
-__global__ void bin_scan_kernel(const int* __restrict__ counts, int* __restrict__ cursors, WorkItem* __restrict__ items,
+__global__ void bin_scan_kernel(int* __restrict__ counts, int* __restrict__ cursors, WorkItem* __restrict__ items,
                                 int* __restrict__ meta, int nb, int chunk) {
+    pdl_wait();
     __shared__ int s_ev[1024], s_it[1024], s_pt[1024];
     const int tid = threadIdx.x, T = blockDim.x;
     const int per = (nb + 1 + T - 1) / T;                  // bins per thread, contiguous
@@ -318,6 +327,7 @@ __global__ void bin_scan_kernel(const int* __restrict__ counts, int* __restrict_
     int ev_off = s_ev[tid] - ev, it_off = s_it[tid] - it, pt_off = n_full + s_pt[tid] - pt;
     for (int b = b0; b < b1; ++b) {
         int c = counts[b];
+        counts[b] = 0;                                     // ready for the next batch (no memset between batches)
         cursors[b] = ev_off;
         if (b < nb) {
             int k = 0;
@@ -337,6 +347,7 @@ __global__ void bin_scan_kernel(const int* __restrict__ counts, int* __restrict_
 __global__ void __launch_bounds__(kBinBlock)
 bin_scatter_kernel(const float* __restrict__ events, int n, const int* __restrict__ bin_of, int* __restrict__ cursors,
                    float* __restrict__ sorted, int nb1, int use_smem) {
+    pdl_wait();
     extern __shared__ int hist[];
     const int tid = threadIdx.x;
     const int base = blockIdx.x * (kBinBlock * kBinPer);
@@ -753,9 +764,10 @@ mlem_rows_kernel(const float* __restrict__ sorted, const WorkItem* __restrict__ 
 // event when a region does not fit shared memory.  One warp per event, thread <-> row, w read from the global
 // transposed image, back-projection with red.global.add.f32, P recomputed in the second pass.  Simple on purpose.
 __global__ void __launch_bounds__(128)
-mlem_rows_direct_kernel(const float* __restrict__ sorted, int stride, const int* __restrict__ meta,
+mlem_rows_direct_kernel(const float* __restrict__ sorted, int stride, int* __restrict__ meta,
                         const __grid_constant__ DevParams p, const float* __restrict__ wT, float* __restrict__ accT,
                         unsigned long long* __restrict__ counters) {
+    pdl_wait();
     const int lane = threadIdx.x & 31;
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
     const int start = meta[1], count = meta[2];
@@ -788,6 +800,9 @@ mlem_rows_direct_kernel(const float* __restrict__ sorted, int stride, const int*
     for (int d = 16; d > 0; d >>= 1) my_evals += __shfl_xor_sync(0xffffffffu, my_evals, d);
     if (lane == 0 && my_evals) atomicAdd(counters + 0, my_evals);
     if (lane == 0 && my_skipped) atomicAdd(counters + 1, my_skipped);
+    // this kernel always follows the tiled event kernel in the stream: reset the work counter for the next run over
+    // the same sorted events (jpet_reconstruct sorts once and iterates)
+    if (blockIdx.x == 0 && threadIdx.x == 0) meta[3] = 0;
 }
 
 // |E_j| only (jpet_count_evals): thread per event, rows in a loop, no kernel values.

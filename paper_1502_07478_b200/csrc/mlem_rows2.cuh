@@ -79,6 +79,7 @@ __device__ __forceinline__ EventRec make_event_rec(float zu, float zd, float dl,
 __global__ void __launch_bounds__(kBinBlock)
 bin_scatter_rec_kernel(const float* __restrict__ events, int n, const int* __restrict__ bin_of, int* __restrict__ cursors,
                        EventRec* __restrict__ sorted, const __grid_constant__ DevParams p, int nb1, int use_smem) {
+    pdl_wait();
     extern __shared__ int hist[];
     const int tid = threadIdx.x;
     const int base = blockIdx.x * (kBinBlock * kBinPer);

@@ -515,6 +515,7 @@ __global__ void __launch_bounds__(NWE * NG * 32, MINB)
 mlem_rows3_kernel(const EventRec* __restrict__ sorted, const WorkItem* __restrict__ items, int* __restrict__ meta,
                   const __grid_constant__ DevParams p, const float* __restrict__ wT, float* __restrict__ accT,
                   const uint32_t* __restrict__ tab, unsigned long long* __restrict__ counters) {
+    pdl_wait();
     constexpr int GT = NWE * NG * 32, GL = NWE * 32;
     extern __shared__ __align__(16) float smem[];
     const int WZ = p.WZ, RS = HS * WZ;
