@@ -16,7 +16,12 @@
 //     the host from the ellipse geometry (task_table.h) and kept in shared memory - no index arithmetic;
 //   * the row constants of the two pieces are evaluated together in packed fp32x2 arithmetic;
 //   * pixel walks are nested (each block of pixels is entered only if the previous one was), pairs of pixels
-//     per fp32x2 operation, warp-uniform bounds from redux; the ragged ends of the rows are masked per pair.
+//     per fp32x2 operation, warp-uniform bounds from redux; the ragged ends of the rows are masked per pair;
+//   * DEG > 0: the exponent of Eq. 7 as a degree-DEG polynomial in u along a piece (poly_coeffs2): one ex2 per kernel
+//     value instead of rsqrt + ex2, the Horner steps of all pairs of a block (BW = 16 pixels: 8 chains) in lockstep;
+//   * the back-projection pass issues its shared-memory read-modify-writes eight at a time; when every lane of a
+//     one-warp group owns at least 8 pixels of its central row, the first 8 run without masks and predicates;
+//   * every kernel of an iteration starts with pdl_wait() and is launched with programmatic stream serialisation.
 //
 // Citations are /root/reference/PAPER.md lines.  Nothing here is shared with oracle/.
 #pragma once
