@@ -8,7 +8,8 @@ over the workload's events.  Default workload: BASELINE.json configs[1] (200x200
 sigma 10/40) - `cfg2` of paper_1502_07478_b200.synth; the other configs can be named with --workload.
 The JSON line carries `value` (device-resident inputs, CUDA-event timing, L2 flushed between steps), `e2e`
 (host buffers through jpet_mlem_iterate_host, copies inside the timed region), `roofline` for the event
-kernel (ALU/SFU bound), `cpu_baseline` (the fp64 oracle on the box's host cores)
+kernel (ALU/SFU bound), `reconstruct` (jpet_reconstruct over the workload's iteration count:
+one sort for all iterations), `cpu_baseline` (the fp64 oracle on the box's host cores)
 and `clocks` sampled with nvidia-smi during the timed region.
 N > 1 (torchrun): independent replicas, one per GPU ("replicas only": north_star fixes one GPU, no sharding).
 """
@@ -289,6 +290,21 @@ def main():
         e2e = {"value": world * n_events * k_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": int(events.nbytes + 4 * M),
                "d2h_bytes_per_step": int(4 * M), "steps": k_e2e, "ms_per_step": dt / k_e2e * 1e3,
                "timing": "host wall clock around the blocking call"}
+    # ---- whole reconstruction: jpet_reconstruct sorts the events once for all iterations --------
+    reconstruct = None
+    if not args.no_e2e:
+        n_it = max(2, cfg.n_iter)
+        jp.jpet_reconstruct(ev_d, *g, rho[0], rho[1], 2)      # warm-up: allocates the buffer of the kept sorted records
+        barrier()
+        a, d = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        jp.jpet_reconstruct(ev_d, *g, rho[0], rho[1], n_it)
+        d.record(stream)
+        barrier()
+        rec_ms = ranks.max(a.elapsed_time(d)) / n_it
+        reconstruct = {"n_iter": n_it, "ms_per_iteration": rec_ms, "events_per_s_per_iteration": world * n_events / (rec_ms * 1e-3),
+                       "note": "jpet_reconstruct: one sort for all iterations, no L2 flush between iterations"}
+
     clocks = sampler.summary()
 
     if rank != 0:
@@ -327,7 +343,7 @@ def main():
                        "tiled": bool(jp.jpet_get_option("last_tiled")), "smem_bytes": jp.jpet_get_option("last_smem_bytes")},
             "kernel_evals_per_s": world * n_evals / (ms_per_step * 1e-3), "kernel_evals_per_iteration": n_evals,
             "px_per_event": n_evals / max(n_events, 1), "events_skipped": n_skipped,
-            "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu_baseline, "clocks": clocks}
+            "e2e": e2e, "reconstruct": reconstruct, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu_baseline, "clocks": clocks}
     print(json.dumps(line))
     ranks.close()
 
