@@ -236,9 +236,12 @@ constexpr Variant3 kVariants3[] = {
     {4, 4, 36, 0, 128, 1, 5, 16},    // 53: as 43, blocks of 16                                          (config 4)
     {3, 4, 36, 8, 128, 1, 5, 16},    // 54: three warps per event: 96 central rows + the few rows beyond them as B pieces (config 4)
     {3, 4, 44, 8, 128, 1, 4, 16},    // 55: as 54 for chords of up to 44 pixels, degree 4
+    {1, 4, 20, 8, 64, 4, 4, 32},     // 56: as 51, one block per piece (config 2: 0.694 -> 0.680 ms)       (configs 2, 3)
+    {4, 4, 44, 0, 128, 1, 4, 32},    // 57: as 52, blocks of 32
+    {3, 4, 36, 8, 128, 1, 5, 32},    // 58: as 54, blocks of 32 (13.96 -> 13.08 ms per 5x10^6 events)       (config 4)
 };
 // shapes in order of size: closed-form / degree-4 / degree-5 instances of each
-constexpr int kShape3[4][3] = {{1, 19, 20}, {0, 30, 21}, {26, 28, 32}, {27, 31, 29}};
+constexpr int kShape3[4][3] = {{1, 19, 20}, {0, 35, 21}, {26, 28, 32}, {27, 31, 29}};
 constexpr int kNumVariants3 = sizeof(kVariants3) / sizeof(kVariants3[0]);
 constexpr int kNumVariants = kNumVariants2 + kNumVariants3;
 
@@ -416,6 +419,9 @@ int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t sme
         case kNumVariants2 + 32: return launch_rows3<4, 4, 36, 0, 128, 1, 5, 16>(bs, dp, smem, st);
         case kNumVariants2 + 33: return launch_rows3<3, 4, 36, 8, 128, 1, 5, 16>(bs, dp, smem, st);
         case kNumVariants2 + 34: return launch_rows3<3, 4, 44, 8, 128, 1, 4, 16>(bs, dp, smem, st);
+        case kNumVariants2 + 35: return launch_rows3<1, 4, 20, 8, 64, 4, 4, 32>(bs, dp, smem, st);
+        case kNumVariants2 + 36: return launch_rows3<4, 4, 44, 0, 128, 1, 4, 32>(bs, dp, smem, st);
+        case kNumVariants2 + 37: return launch_rows3<3, 4, 36, 8, 128, 1, 5, 32>(bs, dp, smem, st);
         case 0: return launch_rows<1, 1, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
         case 1: return launch_rows<2, 1, 1, 20, 64, 4, true, 10, false>(bs, dp, smem, st);
         case 2: return launch_rows<4, 2, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
@@ -509,7 +515,7 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
         const int deg_sel = g_opt_poly_off ? 0 : (trunc_err(4) <= 2e-5 ? 1 : (trunc_err(5) <= 2e-5 ? 2 : 0));
         // ellipses of at most ~100 rows on three warps instead of four (config 4: 91 rows on 128 lanes leave a quarter of
         // the lanes idle; 14.60 -> 14.02 ms per 5x10^6 events), the few rows beyond 96 as B pieces
-        if (deg_sel == 2 && nr_hi > 64 && nr_hi <= 104 && fits3(kVariants3[33])) v = kNumVariants2 + 33;
+        if (deg_sel == 2 && nr_hi > 64 && nr_hi <= 104 && fits3(kVariants3[37])) v = kNumVariants2 + 37;
         for (int sh = 0; sh < 4 && v < 0; ++sh)
             if (fits3(kVariants3[kShape3[sh][deg_sel]])) v = kNumVariants2 + kShape3[sh][deg_sel];
         const int order[] = {14, 12, 15, 16, 0, 8, 9, 10, 5};

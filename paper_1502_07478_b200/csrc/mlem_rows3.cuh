@@ -297,7 +297,7 @@ __device__ __forceinline__ void walk_block(Walk& s, float u0s, float pxs, float 
 template <int NJ, int HS, int DEG, int BW>
 __device__ __forceinline__ float piece_pass1(const Piece& pc, uint32_t w_addr, float pxs, int nblk, float (&preg)[NJ],
                                              bool full8 = false) {
-    static_assert(NJ % 2 == 0 && NJ <= 12 * BW && (BW == 4 || BW == 8 || BW == 16), "pixel capacity must be even and at most 12 blocks");
+    static_assert(NJ % 2 == 0 && NJ <= 12 * BW && (BW == 4 || BW == 8 || BW == 16 || BW == 32), "pixel capacity must be even and at most 12 blocks");
     constexpr int NB = (NJ + BW - 1) / BW;
     Walk s;
     if constexpr (DEG > 0) {

@@ -136,7 +136,7 @@ def test_cfg1_ten_iterations(jp, oracle):
     assert rel_err(got, want) <= TOL_10
 
 
-@pytest.mark.parametrize("variant", list(range(56)))
+@pytest.mark.parametrize("variant", list(range(59)))
 @pytest.mark.parametrize("name,n", [("cfg1", 7777), ("cfg2", 30011), ("cfg4", 5003)])
 def test_every_kernel_variant(jp, oracle, variant, name, n):
     """Each event-kernel shape (warps per CTA, row parts, row passes, cached pixels) on small, medium and large
