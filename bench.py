@@ -322,7 +322,7 @@ def main():
     achieved = n_evals / kern_s
     # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu --set full capture of this
     # workload (profiles/r1f_ncu_full_mlem_rows3_kernel_cfg2.txt); null for workloads without a capture
-    ncu_traffic = {"cfg2": 64_323_328 + 579_584}.get(cfg.name) if n_events == cfg.n_events else None
+    ncu_traffic = {"cfg2": 64_319_744 + 626_432}.get(cfg.name) if n_events == cfg.n_events else None
     roofline = {"bound": "alu", "kernel": "mlem_rows3_kernel", "achieved": achieved / 1e9, "peak": peak_evals / 1e9,
                 "unit": "Geval/s", "frac": achieved / peak_evals, "traffic": ncu_traffic, "traffic_unit": "bytes per launch",
                 "peak_source": f"{n_sm} SMs x 16 MUFU/clk / 2 MUFU per eval x {sm_mhz_peak:.0f} MHz ({peak_kind} sm_max_mhz)",
