@@ -239,9 +239,11 @@ constexpr Variant3 kVariants3[] = {
     {1, 4, 20, 8, 64, 4, 4, 32},     // 56: as 51, one block per piece (config 2: 0.694 -> 0.680 ms)       (configs 2, 3)
     {4, 4, 44, 0, 128, 1, 4, 32},    // 57: as 52, blocks of 32
     {3, 4, 36, 8, 128, 1, 5, 32},    // 58: as 54, blocks of 32 (13.96 -> 13.08 ms per 5x10^6 events)       (config 4)
+    {1, 4, 12, 0, 64, 4, 4, 16},     // 59: as 40, one block per piece
+    {1, 4, 12, 0, 64, 4, 0, 16},     // 60: as 22 (closed form), one block per piece (fig4: 0.813 -> 0.794 ms)   (fig4)
 };
 // shapes in order of size: closed-form / degree-4 / degree-5 instances of each
-constexpr int kShape3[4][3] = {{1, 19, 20}, {0, 35, 21}, {26, 28, 32}, {27, 31, 29}};
+constexpr int kShape3[4][3] = {{39, 19, 20}, {0, 35, 21}, {26, 28, 32}, {27, 31, 29}};
 constexpr int kNumVariants3 = sizeof(kVariants3) / sizeof(kVariants3[0]);
 constexpr int kNumVariants = kNumVariants2 + kNumVariants3;
 
@@ -422,6 +424,8 @@ int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t sme
         case kNumVariants2 + 35: return launch_rows3<1, 4, 20, 8, 64, 4, 4, 32>(bs, dp, smem, st);
         case kNumVariants2 + 36: return launch_rows3<4, 4, 44, 0, 128, 1, 4, 32>(bs, dp, smem, st);
         case kNumVariants2 + 37: return launch_rows3<3, 4, 36, 8, 128, 1, 5, 32>(bs, dp, smem, st);
+        case kNumVariants2 + 38: return launch_rows3<1, 4, 12, 0, 64, 4, 4, 16>(bs, dp, smem, st);
+        case kNumVariants2 + 39: return launch_rows3<1, 4, 12, 0, 64, 4, 0, 16>(bs, dp, smem, st);
         case 0: return launch_rows<1, 1, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
         case 1: return launch_rows<2, 1, 1, 20, 64, 4, true, 10, false>(bs, dp, smem, st);
         case 2: return launch_rows<4, 2, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);

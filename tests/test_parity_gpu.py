@@ -136,7 +136,7 @@ def test_cfg1_ten_iterations(jp, oracle):
     assert rel_err(got, want) <= TOL_10
 
 
-@pytest.mark.parametrize("variant", list(range(59)))
+@pytest.mark.parametrize("variant", list(range(61)))
 @pytest.mark.parametrize("name,n", [("cfg1", 7777), ("cfg2", 30011), ("cfg4", 5003)])
 def test_every_kernel_variant(jp, oracle, variant, name, n):
     """Each event-kernel shape (warps per CTA, row parts, row passes, cached pixels) on small, medium and large
@@ -190,7 +190,7 @@ def test_paper_shaped_workload_fig4(jp, oracle):
     ev = synth.config_events(cfg, n=500_000)
     ones = np.ones((cfg.n_y, cfg.n_z))
     got, (ne, ns) = gpu_iterate(jp, ev, cfg, ones)
-    assert jp.jpet_get_option("last_tiled") == 1 and jp.jpet_get_option("last_variant") in (21, 22)   # closed-form shapes
+    assert jp.jpet_get_option("last_tiled") == 1 and jp.jpet_get_option("last_variant") in (21, 22, 60)   # closed-form shapes
     want, one, ons = oracle.mlem_iterate(ev, *geom(cfg), ones)
     assert rel_err(got, want) <= TOL_1
     assert ns == ons and abs(ne - one) <= 1e-5 * one

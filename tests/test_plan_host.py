@@ -21,7 +21,7 @@ def decode(entry):
 
 
 @pytest.mark.parametrize("name,variant,degree,warps", [("cfg1", 40, 4, 1), ("cfg2", 56, 4, 1), ("cfg3", 56, 4, 1),
-                                                       ("cfg4", 58, 5, 3), ("cfg5", 52, 4, 4), ("fig4", 22, 0, 1)])
+                                                       ("cfg4", 58, 5, 3), ("cfg5", 52, 4, 4), ("fig4", 60, 0, 1)])
 def test_plan_of_every_workload(name, variant, degree, warps):
     """Shape and degree per workload, and the tiling identities the kernels rely on."""
     cfg = synth.CONFIGS[name]
