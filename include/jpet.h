@@ -26,8 +26,11 @@
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-pointer
  *     calls are asynchronous on that stream and never synchronise the device; host-pointer calls return
  *     after their result has landed in the host buffer;
- *   - the library keeps one workspace per process and is not re-entrant: calls must not overlap in time
- *     from several host threads.
+ *   - the library keeps one workspace per CUDA device (the current device of the calling thread selects it) and is
+ *     not re-entrant: calls must not overlap in time from several host threads.  Calls on different streams of one
+ *     device are ordered by the library (each call waits, on its stream, for the previous call's work), so the
+ *     workspace is never used by two streams at once; a3 coefficient, gamma, the sigma_z edge coefficient and the
+ *     tuning options are process-wide.
  *   - arithmetic is fp32 (accumulation: fp32 partial sums per work item in shared memory, merged into the image
  *     with fp32 atomics, so the summation order - and the last bits - vary from run to run); the sensitivity
  *     image is evaluated in fp64 and rounded once to fp32.
@@ -47,6 +50,9 @@ extern "C" {
                                could go non-positive inside the 3-sigma ellipse, or a sequencing error
                                (accumulate/end without begin) */
 #define JPET_E_CUDA (-2)    /* a CUDA call failed (allocation, launch, copy); text in jpet_last_error() */
+#define JPET_E_INTERNAL (-3) /* the event kernel met a record it cannot hold (a row piece longer than its register slot, a
+                               row count outside the task table): 0 by construction; reported by jpet_get_counters
+                               instead of returning a truncated image */
 
 typedef struct { float R; float L; } jpet_geometry;               /* strips y = +-R, |z| <= L/2 */
 typedef struct { float sigma_z; float sigma_dl; } jpet_sigmas;    /* C^-1 = diag(1/sz^2, 1/sz^2, 1/sdl^2), gamma = 0
@@ -96,7 +102,7 @@ int jpet_reconstruct_host(const float *events_host, int64_t n, const jpet_geomet
 /* Counters of the most recent iteration on `cuda_stream` (synchronises that stream):
  *   n_evals   = sum_j |E_j|  - unique (event, pixel-centre-inside-ellipse) pairs, the "kernel evaluations"
  *   n_skipped = events skipped as described above
- * Either pointer may be NULL. */
+ * Either pointer may be NULL.  Returns JPET_E_INTERNAL if the event kernel flagged a record it could not hold. */
 int jpet_get_counters(uint64_t *n_evals_host, uint64_t *n_skipped_host, void *cuda_stream);
 
 /* Counts |E_j| without evaluating the kernel (for evals/s when no iteration has been run).  Synchronises. */
@@ -117,8 +123,59 @@ float jpet_get_a3_coef(void);
 int jpet_set_gamma(float gamma);
 float jpet_get_gamma(void);
 
+/* sigma_z as a function of the hit position (C^-1 "depends on the z~u and z~d ... on the order of 10% from
+ * the center (lowest) to the edge (highest)"; the paper gives no functional form - DESIGN.md reading R22):
+ *   sigma_z(z) = sigma_z * (1 + eta * min(1, (2 z / L)^2)),   C^-1 = diag(1/sigma_z(z~u)^2, 1/sigma_z(z~d)^2, 1/sigma_dl^2) (+ gamma)
+ * per event.  eta = 0 (default) is the constant sigma_z the paper works with; 0.1 is the paper's 10 %.  Process-wide,
+ * takes effect at the next begin / iterate / reconstruct / count call; JPET_E_INVAL outside [0, 1]. */
+int jpet_set_sigma_z_edge(float eta);
+float jpet_get_sigma_z_edge(void);
+
+/* Direct reconstruction (Eq. 2, Fig. 4b): every event is reconstructed to (y~, z~) and counted in the
+ * pixel that contains the point (pixel (iy, iz) covers [y_c - pixel/2, y_c + pixel/2) x [z_c - pixel/2, z_c + pixel/2)).
+ *   hist_dev       : uint32 [n_y*n_z], INCREMENTED (zero it first for a fresh histogram)
+ *   n_outside_host : events whose point falls outside the grid or has a non-finite component (not counted); may be
+ *                    NULL; when given the call synchronises the stream, otherwise it is asynchronous. */
+int jpet_direct_histogram(const float *events_dev, int64_t n, const jpet_geometry *geometry, const jpet_grid *grid,
+                          uint32_t *hist_dev, uint64_t *n_outside_host, void *cuda_stream);
+
+/* Event simulation on the device (the recipe of DESIGN.md section 5, phantom rule
+ * PAPER.md:245): event slot i = first + k (k = 0..n-1) is drawn from its own counter-based random stream
+ * Philox4x32-10(key = seed, counter = (slot, attempt, 0, 0)): attempt a = 0, 1, ... draws (y, z) uniform in the
+ * phantom's bounding rectangle, accepts it with probability intensity / max intensity (first primitive in the list
+ * wins), draws theta uniform on (-pi/2, pi/2), keeps the emission if both strips are hit, and smears
+ * (z_u, z_d, dl) with N(0, sigma_z), N(0, sigma_z), N(0, sigma_dl) (Box-Muller).  Slot i is therefore the same event
+ * whatever n, first or the launch shape.  kind: 0 = ellipse, 1 = box; centre (cy, cz), half sizes (hy, hz) [mm],
+ * phi_deg counter-clockwise in the (z horizontal, y vertical) plane.  events_dev: float32 [n][3], written. */
+typedef struct { int32_t kind; float cy, cz, hy, hz, phi_deg, intensity; } jpet_primitive;
+int jpet_generate_events(const jpet_primitive *phantom_host, int32_t n_primitives, int64_t n, int64_t first,
+                         const jpet_geometry *geometry, const jpet_sigmas *sigmas, uint64_t seed, float *events_dev,
+                         void *cuda_stream);
+
+/* Multi-GPU event sharding (the paper's CPU scheme - a private rho_new per thread, summed at the
+ * end of the iteration, PAPER.md:157 - lifted to devices): every rank runs begin + accumulate over its shard of the
+ * events, then the accumulators are summed and every rank finalises.
+ *   jpet_mlem_accumulator     device pointer and length of the accumulator of the open iteration (transposed image,
+ *                             float32 [n_z][n_y]); valid until the next begin on a different grid or jpet_release -
+ *                             for an NCCL all-reduce in place, or for the IPC export below
+ *   jpet_mlem_end_peers       step 4 with the accumulator read as the sum of n_peers device buffers (this rank's own
+ *                             included, same order on every rank so all ranks get identical bits): the all-reduce
+ *                             fused into the finalise kernel over peer (NVLink) mappings.  The caller guarantees that
+ *                             every peer has finished its accumulate (a barrier after a stream synchronise) and does
+ *                             not start its next begin before all ranks have finished this call.
+ *   jpet_ipc_export / open / close   cudaIpc handle (64 bytes) of a device buffer of this process, its mapping in
+ *                             another process on the same node, and the unmapping. */
+#define JPET_MAX_PEERS 16
+int jpet_mlem_accumulator(float **acc_dev, int64_t *n_floats);
+int jpet_mlem_end_peers(const float *rho_in_dev, float *rho_out_dev, const float *const *peer_acc_dev, int32_t n_peers,
+                        void *cuda_stream);
+int jpet_ipc_export(const void *dev_ptr, void *handle64_out);
+int jpet_ipc_open(const void *handle64, void **dev_ptr_out);
+int jpet_ipc_close(void *dev_ptr);
+
 /* Tuning knobs (do not change results beyond fp32 summation order).  name/value pairs:
- *   "variant"      event-kernel shape id; -1 = automatic
+ *   "variant"      event-kernel shape id (index into the shape list of csrc/jpet_api.cu, see DESIGN.md "Kernels";
+ *                  jpet_plan_describe reports it); -1 = automatic
  *   "force_direct" 1 = skip the shared-memory tiled path: every event goes through the direct kernel
  *                  (w from global memory, red.global.add into the image); 0 = automatic
  *   "chunk"        events per work item of the tiled path; 0 = automatic
@@ -132,6 +189,12 @@ float jpet_get_gamma(void);
  *                  the launches of the last iteration (one per batch of events) is then read with
  *                  jpet_get_option("last_kernel_ns") (synchronises on the last one), their number with
  *                  "last_kernel_launches"
+ *   "stage_bytes"  device staging budget of the host-buffer calls (default 4 GiB; 0 = default): events beyond it are
+ *                  streamed through a two-slot ring, once per iteration
+ *   "exact_kernel" > 0: replace Eq. 7 by the integral it approximates (P = int dtheta/pi N(e~; e(y,z,theta), C)
+ *                  over (-pi/2, pi/2)) evaluated with that many trapezoid nodes in tan(theta) over +-8 sigma around the
+ *                  integrand's peak, on the same 3-sigma pixel set; every event takes the direct kernel (a diagnostic mode,
+ *                  ~50x slower); 0 (default) = Eq. 7
  * jpet_get_option also answers "last_variant", "last_tiled", "last_smem_bytes" (what the last iteration used) and
  * "last_overflow" (row pieces that did not fit their register slot: 0 by construction; synchronises the device).
  * Returns JPET_E_INVAL for an unknown name or a value out of range. */
@@ -149,7 +212,7 @@ const char *jpet_last_error(void);
 
 /* Host-side plan of the event kernel for a problem (no GPU needed; for tests and tuning): the kernel shape and the
  * tiling that jpet_mlem_begin would choose with the current options, a3 coefficient and gamma.
- *   out[0] variant id            out[1] degree of the exponent polynomial (0 = closed form rsqrt + ex2)
+ *   out[0] shape id              out[1] degree of the exponent polynomial (0 = closed form rsqrt + ex2)
  *   out[2] warps per event       out[3] event groups per CTA       out[4] / out[5] pixel capacity of piece A / B
  *   out[6] HS (rows of a region) out[7] WZ (columns of a region)   out[8] / out[9] sub-tile Sy / Sz
  *   out[10] / out[11] halo Hy / Hz                                 out[12] events per work item
@@ -162,9 +225,12 @@ const char *jpet_last_error(void);
 int64_t jpet_plan_describe(const jpet_geometry *geometry, const jpet_sigmas *sigmas, const jpet_grid *grid, int64_t *out,
                            int32_t n_out, uint32_t *task_table_host, int64_t table_cap);
 
+/* Name of an event-kernel shape id ("" if out of range); the pointer is static. */
+const char *jpet_shape_name(int32_t shape);
+
 /* ABI version of this header: bumped whenever a signature changes. */
 int jpet_abi_version(void);
-#define JPET_ABI_VERSION 1
+#define JPET_ABI_VERSION 2
 
 #ifdef __cplusplus
 }

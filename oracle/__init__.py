@@ -24,7 +24,7 @@ DEFAULT_A3_COEF = 2.0  # reading R5: a = d e / d theta; 1.0 = E
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (plain C, -O2, OpenMP); returns the path of the shared library."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-fno-fast-math", "-o", _LIB, _SRC, "-lm"]
+        cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-fno-fast-math", "-ffp-contract=off", "-o", _LIB, _SRC, "-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 
@@ -61,6 +61,30 @@ def _load():
     lib.jo_set_gamma.argtypes = [d]
     lib.jo_get_gamma.restype = d
     lib.jo_get_gamma.argtypes = []
+    lib.jo_set_sigma_z_edge.restype = None
+    lib.jo_set_sigma_z_edge.argtypes = [d]
+    lib.jo_get_sigma_z_edge.restype = d
+    lib.jo_get_sigma_z_edge.argtypes = []
+    lib.jo_sigma_z_at.restype = d
+    lib.jo_sigma_z_at.argtypes = [d, d, d]
+    lib.jo_cinv.restype = None
+    lib.jo_cinv.argtypes = [d, d, d, d, d, p]
+    lib.jo_bCb_c.restype = d
+    lib.jo_bCb_c.argtypes = [d, d, d, p]
+    lib.jo_kernel_c.restype = d
+    lib.jo_kernel_c.argtypes = [d, d, d, d, d, d, p, d]
+    lib.jo_kernel_exact.restype = d
+    lib.jo_kernel_exact.argtypes = [d, d, p, d, p, i]
+    lib.jo_bbox_half_extents_c.restype = None
+    lib.jo_bbox_half_extents_c.argtypes = [d, p, p]
+    lib.jo_set_exact_kernel.restype = None
+    lib.jo_set_exact_kernel.argtypes = [i]
+    lib.jo_get_exact_kernel.restype = i
+    lib.jo_get_exact_kernel.argtypes = []
+    lib.jo_direct_histogram.restype = ctypes.c_uint64
+    lib.jo_direct_histogram.argtypes = [p, i64, d, i, i, d, p]
+    lib.jo_generate_events.restype = i
+    lib.jo_generate_events.argtypes = [p, i, i64, i64, d, d, d, d, ctypes.c_uint64, p]
     _lib = lib
     return lib
 
@@ -73,6 +97,79 @@ def set_gamma(gamma: float) -> None:
 
 def get_gamma() -> float:
     return float(_load().jo_get_gamma())
+
+
+def set_sigma_z_edge(eta: float) -> None:
+    """Coefficient eta of sigma_z(z) = sigma_z (1 + eta min(1, (2z/L)^2)) (reading R22); 0 = constant
+    (default).  Process-wide: set it back to 0 after use."""
+    _load().jo_set_sigma_z_edge(float(eta))
+
+
+def get_sigma_z_edge() -> float:
+    return float(_load().jo_get_sigma_z_edge())
+
+
+def sigma_z_at(z_hit, L, sigma_z) -> float:
+    return float(_load().jo_sigma_z_at(z_hit, L, sigma_z))
+
+
+def cinv(z_u_t, z_d_t, L, sigma_z, sigma_dl) -> np.ndarray:
+    """Eq. 12 for one event: 3x3 inverse covariance at the event's hit positions (current gamma, eta)."""
+    C = np.empty((3, 3), dtype=np.float64)
+    _load().jo_cinv(z_u_t, z_d_t, L, sigma_z, sigma_dl, C.ctypes.data)
+    return C
+
+
+def bCb_c(dy, dz, tan_t, Cinv) -> float:
+    C = np.ascontiguousarray(Cinv, dtype=np.float64)
+    return float(_load().jo_bCb_c(dy, dz, tan_t, C.ctypes.data))
+
+
+def kernel_c(y, z, tan_t, y_t, z_t, R, Cinv, a3_coef=DEFAULT_A3_COEF) -> float:
+    """Eq. 7-11 with a given inverse covariance matrix."""
+    C = np.ascontiguousarray(Cinv, dtype=np.float64)
+    return float(_load().jo_kernel_c(y, z, tan_t, y_t, z_t, R, C.ctypes.data, a3_coef))
+
+
+def kernel_exact(y, z, event, R, Cinv, n_theta=20001) -> float:
+    """The integral Eq. 7 approximates: int dtheta/pi N(e~; e(y, z, theta), C), trapezoid rule."""
+    C = np.ascontiguousarray(Cinv, dtype=np.float64)
+    e = np.ascontiguousarray(event, dtype=np.float64)
+    return float(_load().jo_kernel_exact(y, z, e.ctypes.data, R, C.ctypes.data, int(n_theta)))
+
+
+def bbox_half_extents_c(tan_t, Cinv):
+    C = np.ascontiguousarray(Cinv, dtype=np.float64)
+    out = (ctypes.c_double * 2)()
+    _load().jo_bbox_half_extents_c(tan_t, C.ctypes.data, out)
+    return float(out[0]), float(out[1])
+
+
+def set_exact_kernel(n_theta: int) -> None:
+    """> 0: mlem_iterate / reconstruct use kernel_exact with that many nodes instead of Eq. 7.  Process-wide."""
+    _load().jo_set_exact_kernel(int(n_theta))
+
+
+def direct_histogram(events, R, n_y, n_z, pixel, hist=None):
+    """Eq. 2 + binning (Fig. 4b). Returns (hist uint32 [n_y, n_z], n_outside); `hist` is incremented when given."""
+    ev = _events_f32(events)
+    h = np.zeros((n_y, n_z), dtype=np.uint32) if hist is None else hist
+    assert h.dtype == np.uint32 and h.flags.c_contiguous and h.size == n_y * n_z
+    out = _load().jo_direct_histogram(ev.ctypes.data, ev.shape[0], R, n_y, n_z, pixel, h.ctypes.data)
+    return h, int(out)
+
+
+def generate_events(phantom, n, R, L, sigma_z, sigma_dl, seed, first=0) -> np.ndarray:
+    """Counter-based event simulation (same generator as the CUDA path, fp64). phantom: objects with kind ('E'/'B'),
+    cy, cz, hy, hz, phi_deg, intensity. Returns float32 [n, 3]."""
+    prims = np.array([[{"E": 0.0, "B": 1.0}.get(q.kind, float(q.kind)), q.cy, q.cz, q.hy, q.hz, q.phi_deg, q.intensity]
+                      for q in phantom], dtype=np.float64)
+    out = np.empty((n, 3), dtype=np.float32)
+    rc = _load().jo_generate_events(prims.ctypes.data, len(phantom), int(n), int(first), R, L, sigma_z, sigma_dl,
+                                    int(seed), out.ctypes.data)
+    if rc != 0:
+        raise RuntimeError("jo_generate_events failed")
+    return out
 
 
 def num_threads() -> int:

@@ -80,6 +80,53 @@ static double jo_gamma = 0.0;
 void jo_set_gamma(double gamma) { jo_gamma = gamma; }
 double jo_get_gamma(void) { return jo_gamma; }
 
+/* ---- sigma_z as a function of the hit position (reading R22) ---------------------
+ * C^-1 "depends on the z~u and z~d ... Experimentally we have found this dependence to be quite weak
+ * on the order of 10% from the center (lowest) to the edge (highest)".  The paper gives no functional form; the
+ * reading is  sigma_z(z) = sigma_z (1 + eta min(1, (2 z / L)^2)):  lowest at the strip centre, (1 + eta) sigma_z at
+ * and beyond the strip ends, eta = 0.1 for the paper's 10 %.  eta = 0 (default) is the constant sigma_z the paper
+ * works with.  Process-wide like gamma.                                                                      */
+static double jo_sz_eta = 0.0;
+void jo_set_sigma_z_edge(double eta) { jo_sz_eta = eta; }
+double jo_get_sigma_z_edge(void) { return jo_sz_eta; }
+
+double jo_sigma_z_at(double z_hit, double L, double sigma_z)
+{
+    double q = 2.0 * z_hit / L;
+    q = q * q;
+    if (q > 1.0) q = 1.0;
+    return sigma_z * (1.0 + jo_sz_eta * q);
+}
+
+/* ---- Eq. 12 for one event: 1/sigma_z^2 taken at the event's own hit positions ------------------ */
+void jo_cinv(double z_u_t, double z_d_t, double L, double sigma_z, double sigma_dl, double Cinv[3][3])
+{
+    double su = jo_sigma_z_at(z_u_t, L, sigma_z), sd = jo_sigma_z_at(z_d_t, L, sigma_z);
+    const double g = jo_gamma;
+    Cinv[0][0] = 1.0 / (su * su); Cinv[0][1] = 0.0;             Cinv[0][2] = g;
+    Cinv[1][0] = 0.0;             Cinv[1][1] = 1.0 / (sd * sd); Cinv[1][2] = -g;
+    Cinv[2][0] = g;               Cinv[2][1] = -g;              Cinv[2][2] = 1.0 / (sigma_dl * sigma_dl);
+}
+
+/* b of Eq. 10 for a pixel at offset (dy, dz) from the reconstructed point */
+static void jo_vec_b(double dy, double dz, double tan_t, double b[3])
+{
+    double icos = sqrt(1.0 + tan_t * tan_t);
+    b[0] = dz - dy * tan_t;
+    b[1] = dz - dy * tan_t;
+    b[2] = -2.0 * dy * icos;
+}
+
+/* b C^-1 b with the full matrix ("this term defines an 3 sigma ellipse") */
+double jo_bCb_c(double dy, double dz, double tan_t, const double Cinv[3][3])
+{
+    double b[3], q = 0.0;
+    jo_vec_b(dy, dz, tan_t, b);
+    for (int k = 0; k < 3; ++k)
+        for (int l = 0; l < 3; ++l) q += b[k] * Cinv[k][l] * b[l];
+    return q;
+}
+
 /* ---- b C^-1 b (first line of B.3) ------------------------------------------------------
  * b = (u, u, -2 dy / cos) has equal first and second components (Eq. 10), so the gamma terms of Eq. 12,
  * 2 gamma (b1 - b2) b3, vanish: B.3 and the 3-sigma ellipse do not depend on gamma.                      */
@@ -95,17 +142,12 @@ double jo_bCb(double dy, double dz, double tan_t, double sigma_z, double sigma_d
  * set: the paper's diagonal case).  a3_coef multiplies the third component of a: 2 gives a = d e/d theta (default, R5),
  * 1 gives Eq. 9 exactly as printed.  Prefactor: det^(1/2) of the INVERSE covariance over 2 pi^2 (R4).
  * No truncation here: the 3-sigma rule is applied by the caller.                                        */
-double jo_kernel(double y, double z, double tan_t, double y_t, double z_t,
-                 double R, double sigma_z, double sigma_dl, double a3_coef)
+double jo_kernel_c(double y, double z, double tan_t, double y_t, double z_t, double R, const double Cinv[3][3], double a3_coef)
 {
     double dy = y - y_t;                       /* Eq. 11 */
     double dz = z - z_t;
     double icos = sqrt(1.0 + tan_t * tan_t);   /* cos^-1(theta~) */
     double icos2 = icos * icos;                /* cos^-2(theta~) */
-    const double g = jo_gamma;
-    double Cinv[3][3] = { { 1.0 / (sigma_z * sigma_z), 0.0, g },                     /* Eq. 12 */
-                          { 0.0, 1.0 / (sigma_z * sigma_z), -g },
-                          { g, -g, 1.0 / (sigma_dl * sigma_dl) } };
 
     double o[3], a[3], b[3];
     o[0] = -(dy + y_t - R) * tan_t * icos2;                       /* Eq. 8 */
@@ -136,6 +178,48 @@ double jo_kernel(double y, double z, double tan_t, double y_t, double z_t,
     return sqrt_det_Cinv / (2.0 * JO_PI * JO_PI * sqrt(D)) * exp(-0.5 * (bCb - bCa * bCa / D));   /* Eq. 7 */
 }
 
+/* the same with the constant matrix of Eq. 12: sigma_z everywhere, gamma = jo_gamma */
+double jo_kernel(double y, double z, double tan_t, double y_t, double z_t,
+                 double R, double sigma_z, double sigma_dl, double a3_coef)
+{
+    const double g = jo_gamma;
+    double Cinv[3][3] = { { 1.0 / (sigma_z * sigma_z), 0.0, g },                     /* Eq. 12 */
+                          { 0.0, 1.0 / (sigma_z * sigma_z), -g },
+                          { g, -g, 1.0 / (sigma_dl * sigma_dl) } };
+    return jo_kernel_c(y, z, tan_t, y_t, z_t, R, Cinv, a3_coef);
+}
+
+/* ---- the integral that Eq. 7 approximates (reading R15: emission angle uniform on (-pi/2, pi/2)) ------
+ *   P_exact(e~ | y, z) = int dtheta / pi  N(e~; e(y, z, theta), C),
+ * e(y, z, theta) = (z + (R - y) tan, z - (R + y) tan, -2 y / cos): where the photons of an emission at (y, z) along theta
+ * hit the strips and their path difference (Eq. 1 on the LOR); N the normal density with inverse
+ * covariance Cinv.  Composite trapezoid rule with n_theta nodes over the open interval.  e_t = (z_u~, z_d~, dl~).  */
+double jo_kernel_exact(double y, double z, const double e_t[3], double R, const double Cinv[3][3], int n_theta)
+{
+    double det_Cinv = Cinv[0][0] * (Cinv[1][1] * Cinv[2][2] - Cinv[1][2] * Cinv[2][1])
+                    - Cinv[0][1] * (Cinv[1][0] * Cinv[2][2] - Cinv[1][2] * Cinv[2][0])
+                    + Cinv[0][2] * (Cinv[1][0] * Cinv[2][1] - Cinv[1][1] * Cinv[2][0]);
+    if (!(det_Cinv > 0.0) || n_theta < 2) return 0.0;
+    const double norm = sqrt(det_Cinv) / pow(2.0 * JO_PI, 1.5);
+    const double lo = -0.5 * JO_PI + 1e-9, hi = 0.5 * JO_PI - 1e-9, h = (hi - lo) / (double)(n_theta - 1);
+    double sum = 0.0;
+    for (int k = 0; k < n_theta; ++k) {
+        double theta = lo + h * (double)k;
+        double e[3] = { z + (R - y) * tan(theta), z - (R + y) * tan(theta), -2.0 * y / cos(theta) };
+        double d[3] = { e[0] - e_t[0], e[1] - e_t[1], e[2] - e_t[2] };
+        double chi2 = 0.0;
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) chi2 += d[a] * Cinv[a][b] * d[b];
+        double f = norm * exp(-0.5 * chi2);
+        sum += (k == 0 || k == n_theta - 1) ? 0.5 * f : f;
+    }
+    return sum * h / JO_PI;
+}
+
+static int jo_exact_nodes = 0;          /* > 0: jo_mlem_iterate uses jo_kernel_exact with that many nodes instead of Eq. 7 */
+void jo_set_exact_kernel(int n_theta) { jo_exact_nodes = n_theta; }
+int jo_get_exact_kernel(void) { return jo_exact_nodes; }
+
 /* ---- convenience for quadrature tests: P(e~_j | pixel (y, z)) for many events (double [n][3]) ---------
  * Eq. 2 then Eq. 7 per event; inside3s[j] = 1 when the pixel centre is inside event j's 3-sigma ellipse. */
 void jo_kernel_events(const double *events, int64_t n, double y, double z, double R, double sigma_z,
@@ -157,6 +241,17 @@ void jo_bbox_half_extents(double tan_t, double sigma_z, double sigma_dl, double 
     double A = 2.0 * tan_t * tan_t / (sigma_z * sigma_z) + 4.0 * icos2 / (sigma_dl * sigma_dl);
     double B = 2.0 / (sigma_z * sigma_z);
     double C = -2.0 * tan_t / (sigma_z * sigma_z);
+    out[0] = 3.0 / sqrt(A - C * C / B);                            /* B.2 */
+    out[1] = 3.0 / sqrt(B - C * C / A);
+}
+
+/* the same for a general matrix: A, B, C of the ellipse A dy^2 + 2 C dy dz + B dz^2 = 9 read off the quadratic form
+ * b C^-1 b itself (B.3 is that form written out for the constant diagonal matrix) */
+void jo_bbox_half_extents_c(double tan_t, const double Cinv[3][3], double out[2])
+{
+    double A = jo_bCb_c(1.0, 0.0, tan_t, Cinv);
+    double B = jo_bCb_c(0.0, 1.0, tan_t, Cinv);
+    double C = 0.5 * (jo_bCb_c(1.0, 1.0, tan_t, Cinv) - A - B);
     out[0] = 3.0 / sqrt(A - C * C / B);                            /* B.2 */
     out[1] = 3.0 / sqrt(B - C * C / A);
 }
@@ -218,11 +313,14 @@ int jo_mlem_iterate(const float *events, int64_t n, double R, double L, double s
             jo_eq2((double)events[3 * j + 0], (double)events[3 * j + 1], (double)events[3 * j + 2], R, e);
             double tan_t = e[0], y_t = e[1], z_t = e[2];
             if (!isfinite(tan_t) || !isfinite(y_t) || !isfinite(z_t)) { n_skipped++; continue; }
+            double e_t[3] = { (double)events[3 * j + 0], (double)events[3 * j + 1], (double)events[3 * j + 2] };
+            double Cinv[3][3];
+            jo_cinv(e_t[0], e_t[1], L, sigma_z, sigma_dl, Cinv);     /* Eq. 12 at this event's hit positions */
 
             int iy0 = 0, iy1 = n_y - 1, iz0 = 0, iz1 = n_z - 1;
             if (!brute) {                                           /* bounding box in pixel space */
                 double h[2];
-                jo_bbox_half_extents(tan_t, sigma_z, sigma_dl, h);
+                jo_bbox_half_extents_c(tan_t, Cinv, h);
                 double fy0 = ceil((y_t - h[0]) / pixel + 0.5 * (double)(n_y - 1));
                 double fy1 = floor((y_t + h[0]) / pixel + 0.5 * (double)(n_y - 1));
                 double fz0 = ceil((z_t - h[1]) / pixel + 0.5 * (double)(n_z - 1));
@@ -238,7 +336,7 @@ int jo_mlem_iterate(const float *events, int64_t n, double R, double L, double s
             for (int iy = iy0; iy <= iy1; ++iy) {                   /* Listing 1 line 6 */
                 for (int iz = iz0; iz <= iz1; ++iz) {
                     double y = jo_pixel_y(iy, n_y, pixel), z = jo_pixel_z(iz, n_z, pixel);
-                    if (!(jo_bCb(y - y_t, z - z_t, tan_t, sigma_z, sigma_dl) <= 9.0)) continue;   /* centre inside 3 sigma */
+                    if (!(jo_bCb_c(y - y_t, z - z_t, tan_t, Cinv) <= 9.0)) continue;   /* centre inside 3 sigma */
                     if (cnt == cap) {
                         cap *= 2;
                         double *k2 = (double *)realloc(kernel, cap * sizeof(double));
@@ -248,7 +346,8 @@ int jo_mlem_iterate(const float *events, int64_t n, double R, double L, double s
                         if (!k2 || !p2) { failed = 1; break; }
                     }
                     int i = iy * n_z + iz;
-                    kernel[cnt] = jo_kernel(y, z, tan_t, y_t, z_t, R, sigma_z, sigma_dl, a3_coef);   /* line 7 */
+                    kernel[cnt] = jo_exact_nodes > 0 ? jo_kernel_exact(y, z, e_t, R, Cinv, jo_exact_nodes)
+                                                     : jo_kernel_c(y, z, tan_t, y_t, z_t, R, Cinv, a3_coef);   /* line 7 */
                     pix[cnt] = i;
                     denominator += kernel[cnt] * w[i];              /* line 8, with s(i) of Eq. 3 */
                     cnt++;
@@ -308,4 +407,114 @@ int jo_num_threads(void)
 #else
     return 1;
 #endif
+}
+
+/* ---- direct reconstruction (Eq. 2; Fig. 4b): histogram of the reconstructed points ------------------
+ * Every event is reconstructed to (y~, z~) with Eq. 2 and counted in the pixel that contains the point; pixel
+ * (iy, iz) covers [y_c - pixel/2, y_c + pixel/2) x [z_c - pixel/2, z_c + pixel/2).  The pixel index is an integer
+ * decided by floating point, so both sides take that decision in the SAME precision, the kernel's: IEEE binary32,
+ * round to nearest, in the order written in include/jpet.h / DESIGN.md section 6 (this file is compiled with
+ * -ffp-contract=off, so the only fused operations are the fmaf calls written here):
+ *     t = (z_u - z_d) * inv2R,  sec = sqrt(fma(t, t, 1)),  y~ = (-0.5 dl) / sec,  z~ = fma(y~, t, 0.5 (z_u + z_d)),
+ *     iy = floor(fma(y~, inv_px, oy)),  oy = (n_y - 1) / 2 + 1/2   (likewise iz)
+ * with inv2R = fp32(1 / (2 R)), inv_px = fp32(1 / pixel).  hist (uint32 [n_y*n_z]) is INCREMENTED.
+ * Returns the number of events outside the grid (or with a non-finite component).                           */
+uint64_t jo_direct_histogram(const float *events, int64_t n, double R, int n_y, int n_z, double pixel, uint32_t *hist)
+{
+    const float inv2R = (float)(1.0 / (2.0 * (double)(float)R)), inv_px = (float)(1.0 / (double)(float)pixel);
+    const float oy = (float)(0.5 * (n_y - 1) + 0.5), oz = (float)(0.5 * (n_z - 1) + 0.5);
+    uint64_t outside = 0;
+    for (int64_t j = 0; j < n; ++j) {
+        const float zu = events[3 * j + 0], zd = events[3 * j + 1], dl = events[3 * j + 2];
+        const float t = (zu - zd) * inv2R;
+        const float sec = sqrtf(fmaf(t, t, 1.0f));
+        const float y_t = (-0.5f * dl) / sec;
+        const float z_t = fmaf(y_t, t, 0.5f * (zu + zd));
+        const float fy = floorf(fmaf(y_t, inv_px, oy)), fz = floorf(fmaf(z_t, inv_px, oz));
+        if (!(fy >= 0.0f && fy < (float)n_y && fz >= 0.0f && fz < (float)n_z)) { outside++; continue; }
+        hist[(size_t)(int)fy * (size_t)n_z + (size_t)(int)fz] += 1u;
+    }
+    return outside;
+}
+
+/* ---- event simulation (recipe of SURVEY.md 8(d) / DESIGN.md section 5) -----------------------------
+ * The same counter-based generator as the CUDA path, written out in fp64: event slot i draws from Philox4x32-10
+ * (Salmon et al., SC'11: ten rounds of two 32x32 -> 64-bit multiplications, multipliers 0xD2511F53 / 0xCD9E8D57, key
+ * increments 0x9E3779B9 / 0xBB67AE85) with key = (seed low, seed high) and counter = (slot low, slot high, attempt,
+ * block).  A 32-bit word x becomes the uniform ((x >> 8) + 0.5) 2^-24.  Attempt a = 0, 1, ...:
+ *   block 0 -> (u0, u1, u2, u3):  y = y0 + (y1 - y0) u0,  z = z0 + (z1 - z0) u1 in the phantom's bounding rectangle;
+ *              accepted if u2 < intensity(y, z) / max intensity (first primitive in the list wins);
+ *              theta = pi (u3 - 1/2); hits z_u = z + (R - y) tan, z_d = z - (R + y) tan; kept if both |.| <= L/2;
+ *   block 1 -> (g0, g1, g2, g3):  Box-Muller  r0 = sqrt(-2 ln g0), r1 = sqrt(-2 ln g2):
+ *              z_u~ = z_u + sigma_z r0 cos(2 pi g1),  z_d~ = z_d + sigma_z r0 sin(2 pi g1),
+ *              dl~ = -2 y / cos(theta) + sigma_dl r1 cos(2 pi g3)                       (Eq. 1 on the LOR).
+ * prims: double [n_prim][7] = (kind 0 ellipse / 1 box, cy, cz, hy, hz, phi_deg, intensity).  out: float32 [n][3].    */
+static void jo_philox4x32_10(uint32_t c[4], uint32_t k0, uint32_t k1)
+{
+    for (int r = 0; r < 10; ++r) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * c[0], p1 = (uint64_t)0xCD9E8D57u * c[2];
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c[1] ^ k0, n1 = (uint32_t)p1, n2 = (uint32_t)(p0 >> 32) ^ c[3] ^ k1, n3 = (uint32_t)p0;
+        c[0] = n0; c[1] = n1; c[2] = n2; c[3] = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+}
+
+static double jo_uniform24(uint32_t x) { return ((double)(x >> 8) + 0.5) / 16777216.0; }
+
+static double jo_phantom_intensity(const double *prims, int n_prim, double y, double z)
+{
+    for (int k = 0; k < n_prim; ++k) {
+        const double *q = prims + 7 * k;
+        double phi = q[5] * JO_PI / 180.0, c = cos(phi), s = sin(phi);
+        double dz = z - q[2], dy = y - q[1];
+        double a = (c * dz + s * dy) / q[4], b = (-s * dz + c * dy) / q[3];
+        int in = q[0] == 0.0 ? (a * a + b * b <= 1.0) : (fabs(a) <= 1.0 && fabs(b) <= 1.0);
+        if (in) return q[6];
+    }
+    return 0.0;
+}
+
+int jo_generate_events(const double *prims, int n_prim, int64_t n, int64_t first, double R, double L, double sigma_z,
+                       double sigma_dl, uint64_t seed, float *out)
+{
+    if (n_prim < 1 || n < 0 || !prims || (n > 0 && !out)) return -1;
+    double y0 = 1e300, y1 = -1e300, z0 = 1e300, z1 = -1e300, rho_max = 0.0;
+    for (int k = 0; k < n_prim; ++k) {                             /* bounding rectangle of the rotated primitives */
+        const double *q = prims + 7 * k;
+        double phi = q[5] * JO_PI / 180.0, c = fabs(cos(phi)), s = fabs(sin(phi)), ey, ez;
+        if (q[0] == 0.0) { ez = hypot(q[4] * c, q[3] * s); ey = hypot(q[4] * s, q[3] * c); }
+        else { ez = q[4] * c + q[3] * s; ey = q[4] * s + q[3] * c; }
+        if (q[1] - ey < y0) y0 = q[1] - ey;
+        if (q[1] + ey > y1) y1 = q[1] + ey;
+        if (q[2] - ez < z0) z0 = q[2] - ez;
+        if (q[2] + ez > z1) z1 = q[2] + ez;
+        if (q[6] > rho_max) rho_max = q[6];
+    }
+    if (!(rho_max > 0.0)) return -1;
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int64_t i = 0; i < n; ++i) {
+        const uint64_t slot = (uint64_t)first + (uint64_t)i;
+        float zu = NAN, zd = NAN, dl = NAN;
+        for (uint32_t a = 0; a < 65536u; ++a) {
+            uint32_t c[4] = { (uint32_t)slot, (uint32_t)(slot >> 32), a, 0u };
+            jo_philox4x32_10(c, k0, k1);
+            double y = y0 + (y1 - y0) * jo_uniform24(c[0]), z = z0 + (z1 - z0) * jo_uniform24(c[1]);
+            if (!(jo_uniform24(c[2]) < jo_phantom_intensity(prims, n_prim, y, z) / rho_max)) continue;
+            double theta = JO_PI * (jo_uniform24(c[3]) - 0.5);
+            double hu = z + (R - y) * tan(theta), hd = z - (R + y) * tan(theta);
+            if (!(fabs(hu) <= 0.5 * L && fabs(hd) <= 0.5 * L)) continue;
+            uint32_t g[4] = { (uint32_t)slot, (uint32_t)(slot >> 32), a, 1u };
+            jo_philox4x32_10(g, k0, k1);
+            double r0 = sqrt(-2.0 * log(jo_uniform24(g[0]))), r1 = sqrt(-2.0 * log(jo_uniform24(g[2])));
+            zu = (float)(hu + sigma_z * r0 * cos(2.0 * JO_PI * jo_uniform24(g[1])));
+            zd = (float)(hd + sigma_z * r0 * sin(2.0 * JO_PI * jo_uniform24(g[1])));
+            dl = (float)(-2.0 * y / cos(theta) + sigma_dl * r1 * cos(2.0 * JO_PI * jo_uniform24(g[3])));
+            break;
+        }
+        out[3 * i + 0] = zu; out[3 * i + 1] = zd; out[3 * i + 2] = dl;
+    }
+    return 0;
 }

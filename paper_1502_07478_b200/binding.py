@@ -10,13 +10,16 @@ import os
 
 from . import build as _build
 
-JPET_OK, JPET_E_INVAL, JPET_E_CUDA = 0, -1, -2
+JPET_OK, JPET_E_INVAL, JPET_E_CUDA, JPET_E_INTERNAL = 0, -1, -2, -3
+JPET_MAX_PEERS = 16
 
 EXPORTS = (
     "jpet_sensitivity", "jpet_mlem_iterate", "jpet_reconstruct", "jpet_mlem_begin", "jpet_mlem_accumulate",
     "jpet_mlem_end", "jpet_mlem_iterate_host", "jpet_reconstruct_host", "jpet_get_counters", "jpet_count_evals",
-    "jpet_set_a3_coef", "jpet_get_a3_coef", "jpet_set_gamma", "jpet_get_gamma", "jpet_plan_describe", "jpet_set_option", "jpet_get_option", "jpet_launch_count",
-    "jpet_release", "jpet_last_error", "jpet_abi_version",
+    "jpet_set_a3_coef", "jpet_get_a3_coef", "jpet_set_gamma", "jpet_get_gamma", "jpet_set_sigma_z_edge", "jpet_get_sigma_z_edge",
+    "jpet_direct_histogram", "jpet_generate_events", "jpet_mlem_accumulator", "jpet_mlem_end_peers", "jpet_ipc_export",
+    "jpet_ipc_open", "jpet_ipc_close", "jpet_plan_describe", "jpet_set_option", "jpet_get_option", "jpet_launch_count",
+    "jpet_shape_name", "jpet_release", "jpet_last_error", "jpet_abi_version",
 )
 
 
@@ -30,6 +33,11 @@ class Sigmas(ctypes.Structure):
 
 class Grid(ctypes.Structure):
     _fields_ = [("n_y", ctypes.c_int32), ("n_z", ctypes.c_int32), ("pixel", ctypes.c_float)]
+
+
+class Primitive(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_int32), ("cy", ctypes.c_float), ("cz", ctypes.c_float), ("hy", ctypes.c_float),
+                ("hz", ctypes.c_float), ("phi_deg", ctypes.c_float), ("intensity", ctypes.c_float)]
 
 
 class JpetError(RuntimeError):
@@ -73,6 +81,16 @@ def load(build_if_missing: bool = True) -> ctypes.CDLL:
         "jpet_get_a3_coef": (ctypes.c_float, []),
         "jpet_set_gamma": (ctypes.c_int, [ctypes.c_float]),
         "jpet_get_gamma": (ctypes.c_float, []),
+        "jpet_set_sigma_z_edge": (ctypes.c_int, [ctypes.c_float]),
+        "jpet_get_sigma_z_edge": (ctypes.c_float, []),
+        "jpet_direct_histogram": (ctypes.c_int, [p, i64, G, Gr, p, u64p, p]),
+        "jpet_generate_events": (ctypes.c_int, [ctypes.POINTER(Primitive), i32, i64, i64, G, S, ctypes.c_uint64, p, p]),
+        "jpet_mlem_accumulator": (ctypes.c_int, [ctypes.POINTER(ctypes.c_void_p), ctypes.POINTER(i64)]),
+        "jpet_mlem_end_peers": (ctypes.c_int, [p, p, ctypes.POINTER(ctypes.c_void_p), i32, p]),
+        "jpet_ipc_export": (ctypes.c_int, [p, p]),
+        "jpet_ipc_open": (ctypes.c_int, [p, ctypes.POINTER(ctypes.c_void_p)]),
+        "jpet_ipc_close": (ctypes.c_int, [p]),
+        "jpet_shape_name": (ctypes.c_char_p, [i32]),
         "jpet_plan_describe": (i64, [G, S, Gr, p, i32, p, i64]),
         "jpet_set_option": (ctypes.c_int, [ctypes.c_char_p, i64]),
         "jpet_get_option": (i64, [ctypes.c_char_p]),
@@ -241,6 +259,96 @@ def jpet_set_gamma(gamma: float) -> None:
 
 def jpet_get_gamma() -> float:
     return float(load().jpet_get_gamma())
+
+
+def jpet_set_sigma_z_edge(eta: float) -> None:
+    _check(load().jpet_set_sigma_z_edge(float(eta)))
+
+
+def jpet_get_sigma_z_edge() -> float:
+    return float(load().jpet_get_sigma_z_edge())
+
+
+def jpet_direct_histogram(events_dev, R, L, n_y, n_z, pixel, hist_dev, count_outside=True, stream=None):
+    """Eq. 2 + binning (Fig. 4b): increments hist_dev (int32 CUDA tensor [n_y*n_z], read as uint32); returns the number of
+    events outside the grid (synchronises) or None when count_outside is False (asynchronous)."""
+    import torch
+
+    if not isinstance(hist_dev, torch.Tensor) or not hist_dev.is_cuda or hist_dev.dtype != torch.int32 or not hist_dev.is_contiguous() \
+            or hist_dev.numel() != n_y * n_z:
+        raise TypeError(f"hist_dev must be a contiguous int32 CUDA tensor of {n_y * n_z} elements")
+    g, _, gr = _structs(R, L, 1.0, 1.0, n_y, n_z, pixel)
+    ev, n = _events_ptr(events_dev, True)
+    out = ctypes.c_uint64(0)
+    _check(load().jpet_direct_histogram(ev, n, g, gr, hist_dev.data_ptr(), ctypes.byref(out) if count_outside else None,
+                                        _stream_handle(stream)))
+    return int(out.value) if count_outside else None
+
+
+def jpet_generate_events(phantom, n, R, L, sigma_z, sigma_dl, seed, events_dev, first=0, stream=None):
+    """Event simulation on the device. phantom: sequence of objects with kind ('E' / 'B' or 0 / 1), cy, cz, hy, hz, phi_deg,
+    intensity (synth.Primitive fits); events_dev: float32 CUDA tensor [n, 3], written."""
+    prims = (Primitive * len(phantom))()
+    for k, q in enumerate(phantom):
+        kind = {"E": 0, "B": 1}.get(q.kind, q.kind)
+        prims[k] = Primitive(int(kind), q.cy, q.cz, q.hy, q.hz, q.phi_deg, q.intensity)
+    g, s, _ = _structs(R, L, sigma_z, sigma_dl, 1, 1, 1.0)
+    ev, n_ev = _events_ptr(events_dev, True)
+    if n_ev != n:
+        raise ValueError(f"events_dev must be [{n}, 3]")
+    _check(load().jpet_generate_events(prims, len(phantom), int(n), int(first), g, s, int(seed), ev, _stream_handle(stream)))
+    return events_dev
+
+
+class _DeviceArray:
+    """A raw device pointer seen through __cuda_array_interface__ (so that torch can wrap it without a copy)."""
+
+    def __init__(self, ptr: int, n: int):
+        self.__cuda_array_interface__ = {"shape": (n,), "typestr": "<f4", "data": (ptr, False), "version": 2}
+
+
+def device_view(ptr: int, n: int):
+    """float32 CUDA tensor over n floats at device pointer ptr (no copy, no ownership)."""
+    import torch
+
+    return torch.as_tensor(_DeviceArray(int(ptr), int(n)), device="cuda")
+
+
+def jpet_mlem_accumulator():
+    """The accumulator of the open iteration (between begin and end) as a float32 CUDA tensor view [n_z * n_y]."""
+    ptr, n = ctypes.c_void_p(0), ctypes.c_int64(0)
+    _check(load().jpet_mlem_accumulator(ctypes.byref(ptr), ctypes.byref(n)))
+    return device_view(ptr.value, n.value)
+
+
+def jpet_mlem_end_peers(rho_in_dev, rho_out_dev, peers, stream=None):
+    """Step 4 with the accumulator read as the sum of `peers`: CUDA tensors or raw device pointers (IPC mappings)."""
+    arr = (ctypes.c_void_p * len(peers))()
+    for k, q in enumerate(peers):
+        arr[k] = q if isinstance(q, int) else _dev_f32(q, None, "peer accumulator")
+    _check(load().jpet_mlem_end_peers(_dev_f32(rho_in_dev, None, "rho_in_dev"), _dev_f32(rho_out_dev, None, "rho_out_dev"), arr,
+                                      len(peers), _stream_handle(stream)))
+    return rho_out_dev
+
+
+def jpet_ipc_export(dev_ptr: int) -> bytes:
+    buf = ctypes.create_string_buffer(64)
+    _check(load().jpet_ipc_export(ctypes.c_void_p(int(dev_ptr)), buf))
+    return buf.raw
+
+
+def jpet_ipc_open(handle: bytes) -> int:
+    out = ctypes.c_void_p(0)
+    _check(load().jpet_ipc_open(ctypes.create_string_buffer(handle, 64), ctypes.byref(out)))
+    return int(out.value)
+
+
+def jpet_ipc_close(dev_ptr: int) -> None:
+    _check(load().jpet_ipc_close(ctypes.c_void_p(int(dev_ptr))))
+
+
+def jpet_shape_name(shape: int) -> str:
+    return load().jpet_shape_name(int(shape)).decode()
 
 
 def jpet_set_option(name: str, value: int) -> None:

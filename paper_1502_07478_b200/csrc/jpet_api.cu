@@ -1,4 +1,6 @@
-// jpet_api.cu - C-ABI of include/jpet.h: argument checks, workspace, kernel launches.  No torch types.
+// jpet_api.cu - C-ABI of include/jpet.h: argument checks, per-device workspaces, the plan, kernel launches.
+// No torch types.  The tiled event kernel is instantiated in rows_inst_*.cu (one file per group of shapes, compiled in
+// parallel by build.py) and reached through launch_rows_shape() of rows_launch.h.
 #include "../../include/jpet.h"
 
 #include <cuda_runtime.h>
@@ -9,34 +11,22 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <memory>
 #include <string>
 #include <vector>
 
-#include "mlem_kernels.cuh"
-#include "mlem_rows2.cuh"
-#include "mlem_rows3.cuh"
+#include "generator.cuh"
+#include "histogram.cuh"
+#include "image_kernels.cuh"
+#include "mlem_direct.cuh"
+#include "rows_launch.h"
+#include "sort_kernels.cuh"
 #include "task_table.h"
 
-namespace {
-
-using jpet::DevParams;
-
-thread_local std::string g_err;
+namespace jpet_host {
 std::atomic<uint64_t> g_launches{0};
-float g_a3_coef = 2.0f;
-float g_gamma = 0.0f;             // off-diagonal coefficient of C^-1 (Eq. 12); 0 = the paper's diagonal case
-int64_t g_opt_force_direct = 0;  // 1 = every event takes the direct (global-memory) path
-int64_t g_opt_chunk = 0;         // events per work item, 0 = automatic
-int64_t g_opt_sz = 0;            // sub-tile width in pixels, 0 = automatic
-int64_t g_opt_time_kernel = 0;   // 1 = bracket the tiled event kernel with CUDA events (bench.py's roofline)
-std::vector<cudaEvent_t> g_tk;    // event pairs around the tiled event kernel launches since the last begin
-size_t g_tk_used = 0;
-int64_t g_opt_variant = -1;      // -1 = automatic
-int64_t g_opt_pdl = 1;           // 1 = launch the kernels of an iteration with programmatic stream serialisation
-int64_t g_opt_poly_off = 0;      // 1 = never pick a polynomial-exponent variant automatically
-int64_t g_opt_ctas_per_sm = 0;   // 0 = automatic
-constexpr int64_t kMaxBatch = 10000000;          // events per launch (BASELINE config 5: 10M-event batches)
-constexpr int64_t kStageBytes = 4ll << 30;       // device staging budget of the host-buffer calls
+thread_local std::string g_err;
 
 int fail(int code, const char* fmt, ...) {
     char buf[512];
@@ -47,6 +37,48 @@ int fail(int code, const char* fmt, ...) {
     g_err = buf;
     return code;
 }
+}  // namespace jpet_host
+
+namespace jpet_host {
+int launch_rows_shape(const RowsLaunch& rl) {
+    int rc = launch_rows_group0(rl);
+    if (rc == -100) rc = launch_rows_group1(rl);
+    if (rc == -100) rc = launch_rows_group2(rl);
+    if (rc == -100) rc = launch_rows_group3(rl);
+    if (rc == -100) rc = fail(JPET_E_INVAL, "unknown kernel shape %d", rl.plan->shape);
+    return rc;
+}
+}  // namespace jpet_host
+
+namespace {
+
+using jpet::DevParams;
+using jpet_host::BinSet;
+using jpet_host::fail;
+using jpet_host::g_err;
+using jpet_host::g_launches;
+using jpet_host::kNumShapes;
+using jpet_host::kShapes;
+using jpet_host::Shape;
+
+// ---- process-wide settings (include/jpet.h: a3 coefficient, gamma, sigma_z edge coefficient, tuning options) ------
+struct Options {
+    float a3_coef = 2.0f;
+    float gamma = 0.0f;           // off-diagonal coefficient of C^-1 (Eq. 12); 0 = the paper's diagonal case
+    float sz_eta = 0.0f;          // sigma_z(z) = sigma_z (1 + eta (2z/L)^2); 0 = constant
+    int64_t force_direct = 0;     // 1 = every event takes the direct (global-memory) path
+    int64_t chunk = 0;            // events per work item, 0 = automatic
+    int64_t sz = 0;               // sub-tile width in pixels, 0 = automatic
+    int64_t time_kernel = 0;      // 1 = bracket the tiled event kernel with CUDA events (bench.py's roofline)
+    int64_t variant = -1;         // shape id, -1 = automatic
+    int64_t pdl = 1;              // 1 = launch the kernels of an iteration with programmatic stream serialisation
+    int64_t poly_off = 0;         // 1 = never pick a polynomial-exponent shape automatically
+    int64_t ctas_per_sm = 0;      // 0 = automatic
+    int64_t stage_bytes = 0;      // device staging budget of the host-buffer calls; 0 = default
+    int64_t exact_kernel = 0;     // > 0: theta-quadrature nodes of the exact-kernel mode
+} g_opt;
+constexpr int64_t kMaxBatch = 10000000;          // events per launch (BASELINE config 5: 10M-event batches)
+constexpr int64_t kStageDefault = 4ll << 30;
 
 #define CUDA_TRY(expr)                                                                              \
     do {                                                                                            \
@@ -55,23 +87,25 @@ int fail(int code, const char* fmt, ...) {
             return fail(JPET_E_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
     } while (0)
 
-// One batch of events sorted by sub-tile, with its work-item list (device memory).
-struct BinSet {
-    float* sorted = nullptr;            // [n][stride], regular bins first, the direct bin last
-    int stride = 3;                     // floats per event: 3 = raw triple, 16 = EventRec (second-generation kernel)
-    jpet::WorkItem* items = nullptr;
-    int* meta = nullptr;                // 0: #items, 1: direct start, 2: direct count, 3: work counter
-    int64_t n = 0;
-    size_t cap_events = 0, cap_items = 0;
-    bool owns_sorted = true;
-};
-
+// Everything the plan depends on; compared field by field (no padding bytes involved).
 struct PlanKey {
-    jpet_geometry g; jpet_sigmas sg; jpet_grid gr; float a3, gamma;
-    int64_t variant, sz, chunk, force_direct;
+    jpet_geometry g{0, 0};
+    jpet_sigmas sg{0, 0};
+    jpet_grid gr{0, 0, 0};
+    float a3 = 0, gamma = 0, sz_eta = 0;
+    int64_t variant = 0, sz = 0, chunk = 0, force_direct = 0, poly_off = 0, exact = 0;
+    bool operator==(const PlanKey& o) const {
+        return g.R == o.g.R && g.L == o.g.L && sg.sigma_z == o.sg.sigma_z && sg.sigma_dl == o.sg.sigma_dl && gr.n_y == o.gr.n_y &&
+               gr.n_z == o.gr.n_z && gr.pixel == o.gr.pixel && a3 == o.a3 && gamma == o.gamma && sz_eta == o.sz_eta &&
+               variant == o.variant && sz == o.sz && chunk == o.chunk && force_direct == o.force_direct && poly_off == o.poly_off &&
+               exact == o.exact;
+    }
 };
 
+// One per CUDA device (the current device of the calling thread selects it).
 struct Workspace {
+    int device = -1;
+    int sm_count = 0;
     // problem the workspace is currently set up for
     jpet_geometry geom{0, 0};
     jpet_sigmas sig{0, 0};
@@ -79,19 +113,19 @@ struct Workspace {
     bool s_valid = false;
     bool open = false;          // between begin and end
     int M = 0;
-    DevParams dp{};
-    int variant = 0;
-    size_t smem = 0;
+    jpet_host::RowsPlan plan;   // DevParams, shape, shared memory, task table pointer
+    PlanKey plan_key;
+    bool plan_valid = false;
     // device buffers
     float* s = nullptr;
     float* wT = nullptr;
     float* accT = nullptr;
     float* rho_a = nullptr;
     float* rho_b = nullptr;
-    unsigned long long* counters = nullptr;
+    unsigned long long* counters = nullptr;      // 0 evals, 1 skipped, 2 overflow flags, 3 scratch
     size_t cap_M = 0;
-    int* bin_of = nullptr;      // scratch of the binning pass
-    size_t cap_bin_of = 0;
+    int2* place = nullptr;      // scratch of the binning pass: (bin, packed rows) per event
+    size_t cap_place = 0;
     int* counts = nullptr;      // [nb + 1] counts, then [nb + 1] cursors
     size_t cap_counts = 0;
     int counts_clean_nb = -1;   // bin count of the layout the (zeroed) counts buffer was last used with
@@ -103,14 +137,65 @@ struct Workspace {
     size_t cap_stage = 0;       // bytes
     cudaStream_t copy_stream = nullptr, compute_stream = nullptr;
     cudaEvent_t ev_copy[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
-    PlanKey plan_key{};
-    bool plan_valid = false;
-    uint32_t* tab = nullptr;    // task table of the third-generation kernel (device copy of tab_host)
+    bool slot_used[2] = {false, false};          // ring slots of the staging buffer that a kernel may still be reading
+    uint32_t* tab = nullptr;    // task table (device copy of tab_host)
     size_t cap_tab = 0;
     std::vector<uint32_t> tab_host, tab_uploaded;
-    int sm_count = 0;
-    int device = -1;
-} g_ws;
+    bool sort_attr_set = false;
+    // ordering between streams: every call waits, on its stream, for the previous call's work
+    cudaEvent_t ev_last = nullptr;
+    cudaStream_t last_stream = nullptr;
+    bool have_last = false;
+    // CUDA-event pairs around the tiled event kernel launches since the last begin ("time_kernel")
+    std::vector<cudaEvent_t> tk;
+    size_t tk_used = 0;
+};
+std::map<int, std::unique_ptr<Workspace>> g_ctx;
+int g_last_device = -1;      // device of the most recent call that touched a workspace (jpet_get_option "last_*")
+
+int current_ws(Workspace** out) {
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    auto& slot = g_ctx[dev];
+    if (!slot) {
+        slot.reset(new Workspace());
+        slot->device = dev;
+        CUDA_TRY(cudaDeviceGetAttribute(&slot->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    }
+    g_last_device = dev;
+    *out = slot.get();
+    return JPET_OK;
+}
+
+// The workspace of the calling thread's current device if one exists (accumulate / end / counters follow a begin).
+Workspace* device_ws() {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return nullptr;
+    auto it = g_ctx.find(dev);
+    if (it == g_ctx.end()) return nullptr;
+    g_last_device = dev;
+    return it->second.get();
+}
+
+Workspace* last_ws() {
+    auto it = g_ctx.find(g_last_device);
+    return it == g_ctx.end() ? nullptr : it->second.get();
+}
+
+// Stream ordering (include/jpet.h): the workspace is used by one stream at a time.
+int enter(Workspace& w, cudaStream_t st) {
+    if (w.have_last && w.last_stream != st) CUDA_TRY(cudaStreamWaitEvent(st, w.ev_last, 0));
+    return JPET_OK;
+}
+int leave(Workspace& w, cudaStream_t st) {
+    if (!w.ev_last) CUDA_TRY(cudaEventCreateWithFlags(&w.ev_last, cudaEventDisableTiming));
+    CUDA_TRY(cudaEventRecord(w.ev_last, st));
+    w.last_stream = st;
+    w.have_last = true;
+    return JPET_OK;
+}
+
+double sigma_z_max(const jpet_sigmas& sg) { return (double)sg.sigma_z * (1.0 + (double)g_opt.sz_eta); }
 
 int validate(const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr) {
     if (!g || !gr) return fail(JPET_E_INVAL, "NULL geometry or grid");
@@ -125,133 +210,41 @@ int validate(const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr)
         if (!(sg->sigma_z > 0.f) || !(sg->sigma_dl > 0.f) || !std::isfinite(sg->sigma_z) || !std::isfinite(sg->sigma_dl))
             return fail(JPET_E_INVAL, "sigmas must be positive and finite");
         // D = a.C^-1.a + 2 o.C^-1.b stays positive inside the 3-sigma ellipse when this ratio is < 1
-        // (bound derived in DESIGN.md "Domain"); we ask for a factor 2 of margin.
-        double ratio = (1.07 * sg->sigma_z + 1.8 * (double)sg->sigma_z * sg->sigma_z / sg->sigma_dl) / g->R;
+        // (bound derived in DESIGN.md "Domain"); we ask for a factor 2 of margin.  With a position-dependent sigma_z
+        // the largest value (strip edge) enters.
+        const double szm = sigma_z_max(*sg);
+        double ratio = (1.07 * szm + 1.8 * szm * szm / sg->sigma_dl) / g->R;
         if (ratio > 0.5) return fail(JPET_E_INVAL, "sigmas too large against R: Eq. 7's square root could go non-positive");
         // Eq. 12 is positive definite for gamma^2 < 1 / (2 sigma_z^2 sigma_dl^2); half of that keeps D > 0 as well
         // (a.C^-1.a changes by at most 2 |gamma| k y sigma_z^2 sin(theta) / R of itself)
-        if (std::fabs((double)g_gamma) * std::sqrt(2.0) * sg->sigma_z * sg->sigma_dl > 0.5)
+        if (std::fabs((double)g_opt.gamma) * std::sqrt(2.0) * szm * sg->sigma_dl > 0.5)
             return fail(JPET_E_INVAL, "|gamma| must be at most 0.5 / (sqrt(2) sigma_z sigma_dl) (Eq. 12 positive definite, D > 0)");
-        if (3.0 * sg->sigma_dl / gr->pixel > 60000.0 || 4.3 * sg->sigma_z / gr->pixel > 60000.0)
+        if (3.0 * sg->sigma_dl / gr->pixel > 60000.0 || 4.3 * szm / gr->pixel > 60000.0)
             return fail(JPET_E_INVAL, "ellipse spans too many pixels");
     }
     return JPET_OK;
 }
 
-int ensure_device() {
-    int dev = 0;
-    CUDA_TRY(cudaGetDevice(&dev));
-    if (dev != g_ws.device) {
-        if (g_ws.device >= 0) jpet_release();
-        g_ws.device = dev;
-        CUDA_TRY(cudaDeviceGetAttribute(&g_ws.sm_count, cudaDevAttrMultiProcessorCount, dev));
+int ensure_images(Workspace& w, int M) {
+    if ((size_t)M > w.cap_M) {
+        cudaFree(w.s); cudaFree(w.wT); cudaFree(w.accT); cudaFree(w.rho_a); cudaFree(w.rho_b);
+        w.s = w.wT = w.accT = w.rho_a = w.rho_b = nullptr;
+        w.cap_M = 0;
+        CUDA_TRY(cudaMalloc(&w.s, sizeof(float) * M));
+        CUDA_TRY(cudaMalloc(&w.wT, sizeof(float) * M));
+        CUDA_TRY(cudaMalloc(&w.accT, sizeof(float) * M));
+        CUDA_TRY(cudaMalloc(&w.rho_a, sizeof(float) * M));
+        CUDA_TRY(cudaMalloc(&w.rho_b, sizeof(float) * M));
+        w.cap_M = M;
+        w.s_valid = false;
     }
+    if (!w.counters) CUDA_TRY(cudaMalloc(&w.counters, 4 * sizeof(unsigned long long)));
     return JPET_OK;
 }
-
-int ensure_images(int M) {
-    if ((size_t)M > g_ws.cap_M) {
-        cudaFree(g_ws.s); cudaFree(g_ws.wT); cudaFree(g_ws.accT); cudaFree(g_ws.rho_a); cudaFree(g_ws.rho_b);
-        g_ws.s = g_ws.wT = g_ws.accT = g_ws.rho_a = g_ws.rho_b = nullptr;
-        g_ws.cap_M = 0;
-        CUDA_TRY(cudaMalloc(&g_ws.s, sizeof(float) * M));
-        CUDA_TRY(cudaMalloc(&g_ws.wT, sizeof(float) * M));
-        CUDA_TRY(cudaMalloc(&g_ws.accT, sizeof(float) * M));
-        CUDA_TRY(cudaMalloc(&g_ws.rho_a, sizeof(float) * M));
-        CUDA_TRY(cudaMalloc(&g_ws.rho_b, sizeof(float) * M));
-        g_ws.cap_M = M;
-        g_ws.s_valid = false;
-    }
-    if (!g_ws.counters) CUDA_TRY(cudaMalloc(&g_ws.counters, 4 * sizeof(unsigned long long)));
-    return JPET_OK;
-}
-
-// ---- event-kernel variants: NW warps per CTA, rows split in NH parts, NR row passes, NJ cached pixels,
-// HS = region row stride (compile time, so every shared-memory access has an immediate offset) ---------------
-// Second-generation shapes (mlem_rows2.cuh) have NA > 0: NA blocks of 32 central rows, NH parts per row, NBW = 1
-// adds the warp that takes the cap rows; NW = NA * NH + NBW.
-struct Variant { int NW, NH, NR, NJ, HS, U, CF, MINB, PK, NA, NBW; };
-constexpr Variant kVariants[] = {
-    {1, 1, 1, 12, 64, 4, 1, 1, 0},    // 0: <= 32 rows, chords <= 12 px                            (config 1)
-    {2, 1, 1, 20, 64, 4, 1, 10, 0},   // 1: <= 64 rows, chords <= 20 px, <= 96 registers           (configs 2, 3)
-    {4, 2, 1, 12, 64, 4, 1, 1, 0},    // 2: <= 64 rows, chords <= 24 px in two halves
-    {4, 1, 1, 36, 128, 4, 1, 1, 0},   // 3: <= 128 rows, chords <= 36 px
-    {8, 2, 1, 20, 128, 4, 1, 1, 0},   // 4: <= 128 rows, chords <= 40 px in two halves             (config 4)
-    {8, 2, 1, 24, 160, 4, 1, 1, 0},   // 5: <= 128 rows, chords <= 48 px in two halves
-    {4, 1, 1, 44, 160, 4, 1, 1, 0},   // 6: <= 128 rows, chords <= 44 px                           (config 5)
-    {1, 1, 2, 20, 64, 4, 1, 1, 0},    // 7: <= 64 rows in two passes of one warp, chords <= 20 px
-    {2, 1, 1, 20, 64, 4, 1, 10, 1},   // 8: as 1, packed fp32x2 arithmetic
-    {8, 2, 1, 20, 128, 4, 1, 1, 1},   // 9: as 4, packed
-    {4, 1, 1, 44, 160, 4, 1, 1, 1},   // 10: as 6, packed
-    {1, 1, 1, 12, 64, 4, 1, 1, 1},    // 11: as 0, packed
-    {2, 1, 1, 20, 64, 4, 1, 10, 1, 1, 1},    // 12: rows2, 32 central rows + cap warp, chords <= 20      (configs 2, 3)
-    {2, 1, 1, 20, 64, 4, 1, 10, 0, 1, 1},    // 13: as 12, scalar arithmetic
-    {1, 1, 1, 12, 64, 4, 1, 1, 1, 1, 0},     // 14: rows2, <= 32 rows, chords <= 12                       (config 1)
-    {7, 2, 1, 20, 128, 4, 1, 1, 1, 3, 1},    // 15: rows2, 96 central rows in halves + cap warp, chords <= 40 (config 4)
-    {8, 2, 1, 24, 160, 4, 1, 1, 1, 4, 0},    // 16: rows2, <= 128 rows in halves, chords <= 48            (config 5)
-    {8, 2, 1, 20, 128, 4, 1, 1, 1, 4, 0},    // 17: rows2, <= 128 rows in halves, chords <= 40
-    {7, 2, 1, 24, 160, 4, 1, 1, 1, 3, 1},    // 18: rows2, 96 central rows in halves + cap warp, chords <= 48
-    {4, 1, 1, 44, 160, 4, 1, 1, 1, 4, 0},    // 19: rows2, <= 128 rows, chords <= 44
-    {4, 1, 1, 36, 128, 4, 1, 1, 1, 3, 1},    // 20: rows2, 96 central rows + cap warp, chords <= 36
-};
-constexpr int kNumVariants2 = sizeof(kVariants) / sizeof(kVariants[0]);
-// Third-generation shapes (mlem_rows3.cuh), variant id = kNumVariants2 + index: NWE warps per event, NG event groups
-// per CTA, NJA / NJB pixel capacity of the two pieces a lane walks (NJB = 0: one piece), region row stride HS.
-// DEG: 0 = closed form (rsqrt + ex2 per pixel), 4 / 5 = exponent as a polynomial in u (one ex2 per pixel; make_plan
-// bounds the truncation error and picks the degree); BW: pixels per block of the walks.
-struct Variant3 { int NWE, NG, NJA, NJB, HS, MINB, DEG, BW; };
-constexpr Variant3 kVariants3[] = {
-    {1, 4, 20, 8, 64, 4, 0, 8},      // 21: <= 64 rows, chords <= 20 px, four independent warps per CTA      (configs 2, 3)
-    {1, 4, 12, 0, 64, 4, 0, 8},      // 22: <= 32 rows, chords <= 12 px                                     (config 1)
-    {4, 1, 36, 0, 128, 1, 0, 8},     // 23: <= 128 rows, chords <= 36 px, one row per lane                   (config 4)
-    {4, 1, 44, 0, 128, 1, 0, 8},     // 24: <= 128 rows, chords <= 44 px, one row per lane                   (config 5)
-    {2, 2, 36, 28, 128, 1, 0, 8},    // 25: <= 128 rows on two warps: 64 central rows + caps, chords <= 36
-    {1, 8, 20, 8, 64, 2, 0, 8},      // 26: as 21, eight warps per CTA
-    {1, 2, 20, 8, 64, 8, 0, 8},      // 27: as 21, two warps per CTA
-    {1, 4, 20, 8, 64, 3, 0, 8},      // 28: as 21, at most 3 CTAs per SM (more registers)
-    {1, 4, 20, 8, 64, 2, 0, 8},      // 29: as 21, at most 2 CTAs per SM
-    {1, 4, 20, 8, 64, 4, 4, 4},      // 30: as 21, polynomial exponent of degree 4, blocks of 4          (configs 2, 3)
-    {1, 4, 12, 0, 64, 4, 4, 4},      // 31: as 22, degree 4                                              (config 1)
-    {4, 1, 36, 0, 128, 1, 5, 8},     // 32: as 23, degree 5                                              (config 4)
-    {4, 1, 44, 0, 128, 1, 4, 8},     // 33: as 24, degree 4                                              (config 5)
-    {1, 4, 20, 8, 64, 4, 5, 4},      // 34: as 30, degree 5
-    {1, 4, 12, 0, 64, 4, 5, 4},      // 35: as 31, degree 5
-    {4, 1, 36, 0, 128, 1, 4, 8},     // 36: as 32, degree 4
-    {4, 1, 44, 0, 128, 1, 5, 8},     // 37: as 33, degree 5
-    {1, 4, 20, 8, 64, 4, 4, 8},      // 38: as 30, blocks of 8
-    {1, 4, 20, 8, 64, 4, 0, 4},      // 39: as 21, blocks of 4
-    {1, 4, 12, 0, 64, 4, 4, 8},      // 40: as 31, blocks of 8
-    {1, 4, 12, 0, 64, 4, 5, 8},      // 41: as 40, degree 5
-    {1, 4, 20, 8, 64, 4, 5, 8},      // 42: as 38, degree 5
-    {4, 4, 36, 0, 128, 1, 5, 8},     // 43: as 32, four event groups per CTA (one CTA of 16 warps per SM)
-    {4, 4, 44, 0, 128, 1, 4, 8},     // 44: as 33, four event groups per CTA
-    {4, 3, 36, 0, 128, 1, 5, 8},     // 45: as 32, three event groups per CTA
-    {4, 3, 44, 0, 128, 1, 4, 8},     // 46: as 33, three event groups per CTA
-    {4, 4, 36, 0, 128, 1, 0, 8},     // 47: as 43, closed form
-    {4, 4, 44, 0, 128, 1, 0, 8},     // 48: as 44, closed form
-    {4, 4, 36, 0, 128, 1, 4, 8},     // 49: as 43, degree 4
-    {4, 4, 44, 0, 128, 1, 5, 8},     // 50: as 44, degree 5
-    {1, 4, 20, 8, 64, 4, 4, 16},     // 51: as 38, blocks of 16 (config 2: 0.728 -> 0.710 ms)             (configs 2, 3)
-    {4, 4, 44, 0, 128, 1, 4, 16},    // 52: as 44, blocks of 16                                          (config 5)
-    {4, 4, 36, 0, 128, 1, 5, 16},    // 53: as 43, blocks of 16                                          (config 4)
-    {3, 4, 36, 8, 128, 1, 5, 16},    // 54: three warps per event: 96 central rows + the few rows beyond them as B pieces (config 4)
-    {3, 4, 44, 8, 128, 1, 4, 16},    // 55: as 54 for chords of up to 44 pixels, degree 4
-    {1, 4, 20, 8, 64, 4, 4, 32},     // 56: as 51, one block per piece (config 2: 0.694 -> 0.680 ms)       (configs 2, 3)
-    {4, 4, 44, 0, 128, 1, 4, 32},    // 57: as 52, blocks of 32
-    {3, 4, 36, 8, 128, 1, 5, 32},    // 58: as 54, blocks of 32 (13.96 -> 13.08 ms per 5x10^6 events)       (config 4)
-    {1, 4, 12, 0, 64, 4, 4, 16},     // 59: as 40, one block per piece
-    {1, 4, 12, 0, 64, 4, 0, 16},     // 60: as 22 (closed form), one block per piece (fig4: 0.813 -> 0.794 ms)   (fig4)
-};
-// shapes in order of size: closed-form / degree-4 / degree-5 instances of each
-constexpr int kShape3[4][3] = {{39, 19, 20}, {0, 35, 21}, {26, 28, 32}, {27, 31, 29}};
-constexpr int kNumVariants3 = sizeof(kVariants3) / sizeof(kVariants3[0]);
-constexpr int kNumVariants = kNumVariants2 + kNumVariants3;
-
-int batch_chunk(int64_t n, const DevParams& dp);
 
 // Kernel launch with the programmatic-stream-serialisation attribute (PDL): the kernel may be scheduled while the
-// previous kernel of the stream drains; every kernel launched this way starts with pdl_wait() (mlem_kernels.cuh), so
-// it reads nothing the previous kernel wrote before that kernel has completed.  Hides most of the launch gaps between
+// previous kernel of the stream drains; every kernel launched this way starts with pdl_wait() (common.cuh), so it
+// reads nothing the previous kernel wrote before that kernel has completed.  Hides most of the launch gaps between
 // the eight kernels of an iteration (config 2: a 0.8 ms step).
 template <typename... KArgs, typename... Args>
 cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
@@ -264,205 +257,68 @@ cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t sme
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = g_opt_pdl ? 1 : 0;
+    cfg.numAttrs = g_opt.pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
 }
 
-template <int NW, int NH, int NR, int NJ, int HS, int U, bool CF, int MINB, bool PK>
-int launch_rows(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
-    auto kern = jpet::mlem_rows_kernel<NW, NH, NR, NJ, HS, U, CF, MINB, PK>;
-    if (bs.stride != 3) return fail(JPET_E_INVAL, "internal: first-generation kernel needs raw event triples");
-    if (dp.t_max >= 0.f) {     // tiled path
-        if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
-        static size_t attr_set = 0;
-        if (smem > 40 * 1024 && smem > attr_set) {
-            CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            attr_set = smem;
-        }
-        int per_sm = 0;
-        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NW * 32, smem));
-        if (per_sm < 1) return fail(JPET_E_CUDA, "event kernel does not fit on an SM (%zu B of shared memory)", smem);
-        if (g_opt_ctas_per_sm > 0) per_sm = (int)std::min<int64_t>(per_sm, g_opt_ctas_per_sm);
-        int64_t max_items = bs.n / batch_chunk(bs.n, dp) + (int64_t)dp.nby * dp.nbz + 1;
-        int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(max_items, 1));
-        if (g_opt_time_kernel) {
-            if (g_tk_used + 2 > g_tk.size()) {
-                g_tk.resize(g_tk_used + 2, nullptr);
-                CUDA_TRY(cudaEventCreate(&g_tk[g_tk_used])); CUDA_TRY(cudaEventCreate(&g_tk[g_tk_used + 1]));
-            }
-            CUDA_TRY(cudaEventRecord(g_tk[g_tk_used], stream));
-        }
-        kern<<<grid, NW * 32, smem, stream>>>(bs.sorted, bs.items, bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.counters);
-        g_launches++;
-        if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk[g_tk_used + 1], stream)); g_tk_used += 2; }
-        CUDA_TRY(cudaGetLastError());
-    }
-    // direct path for the events of the last bin (all events when no region fits shared memory)
-    int dgrid = dp.t_max >= 0.f ? g_ws.sm_count : g_ws.sm_count * 16;
-    CUDA_TRY(launch_pdl(jpet::mlem_rows_direct_kernel, dim3(dgrid), dim3(128), 0, stream, bs.sorted, bs.stride, bs.meta, dp, g_ws.wT,
-                        g_ws.accT, g_ws.counters));
-    g_launches++;
-    CUDA_TRY(cudaGetLastError());
-    return JPET_OK;
+// Events per work item for a batch of n events: the plan's size, halved (not below 64) while the batch would give fewer
+// than four items per SM - small batches are launch- and tail-bound.
+int batch_chunk(const Workspace& w, int64_t n) {
+    int chunk = w.plan.dp.chunk;
+    if (g_opt.chunk > 0) return chunk;
+    while (chunk > 64 && n / chunk < 4 * (int64_t)w.sm_count) chunk /= 2;
+    return chunk;
 }
 
-template <int NA, int NH, int NBW, int NJ, int HS, int U, bool PK, int MINB>
-int launch_rows2(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
-    constexpr int NW = NA * NH + NBW;
-    auto kern = jpet::mlem_rows2_kernel<NA, NH, NBW, NJ, HS, U, PK, MINB>;
-    if (bs.stride != 16) return fail(JPET_E_INVAL, "internal: rows2 kernel needs event records");
+// The tiled event kernel over the regular bins of a sorted batch, then the direct kernel over its last bin (all events
+// when no region fits shared memory, or in the exact-kernel mode).
+int run_binset(Workspace& w, BinSet& bs, cudaStream_t st) {
+    const DevParams& dp = w.plan.dp;
     if (dp.t_max >= 0.f) {
-        if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
-        static size_t attr_set = 0;
-        if (smem > 40 * 1024 && smem > attr_set) {
-            CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            attr_set = smem;
-        }
-        int per_sm = 0;
-        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NW * 32, smem));
-        if (per_sm < 1) return fail(JPET_E_CUDA, "event kernel does not fit on an SM (%zu B of shared memory)", smem);
-        if (g_opt_ctas_per_sm > 0) per_sm = (int)std::min<int64_t>(per_sm, g_opt_ctas_per_sm);
-        int64_t max_items = bs.n / batch_chunk(bs.n, dp) + (int64_t)dp.nby * dp.nbz + 1;
-        int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(max_items, 1));
-        if (g_opt_time_kernel) {
-            if (g_tk_used + 2 > g_tk.size()) {
-                g_tk.resize(g_tk_used + 2, nullptr);
-                CUDA_TRY(cudaEventCreate(&g_tk[g_tk_used])); CUDA_TRY(cudaEventCreate(&g_tk[g_tk_used + 1]));
+        if (g_opt.time_kernel) {
+            if (w.tk_used + 2 > w.tk.size()) {
+                w.tk.resize(w.tk_used + 2, nullptr);
+                CUDA_TRY(cudaEventCreate(&w.tk[w.tk_used])); CUDA_TRY(cudaEventCreate(&w.tk[w.tk_used + 1]));
             }
-            CUDA_TRY(cudaEventRecord(g_tk[g_tk_used], stream));
+            CUDA_TRY(cudaEventRecord(w.tk[w.tk_used], st));
         }
-        kern<<<grid, NW * 32, smem, stream>>>(reinterpret_cast<const jpet::EventRec*>(bs.sorted), bs.items, bs.meta, dp,
-                                             g_ws.wT, g_ws.accT, g_ws.counters);
-        g_launches++;
-        if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk[g_tk_used + 1], stream)); g_tk_used += 2; }
-        CUDA_TRY(cudaGetLastError());
+        jpet_host::RowsLaunch rl;
+        rl.bs = &bs; rl.plan = &w.plan; rl.wT = w.wT; rl.accT = w.accT; rl.tab = w.tab; rl.counters = w.counters;
+        rl.sm_count = w.sm_count; rl.device = w.device; rl.stream = st; rl.pdl = g_opt.pdl != 0;
+        rl.ctas_per_sm = (int)g_opt.ctas_per_sm;
+        rl.max_items = bs.n / batch_chunk(w, bs.n) + (int64_t)dp.nby * dp.nbz + 1;
+        int rc = jpet_host::launch_rows_shape(rl);
+        if (rc) return rc;
+        if (g_opt.time_kernel) { CUDA_TRY(cudaEventRecord(w.tk[w.tk_used + 1], st)); w.tk_used += 2; }
     }
-    int dgrid = dp.t_max >= 0.f ? g_ws.sm_count : g_ws.sm_count * 16;
-    CUDA_TRY(launch_pdl(jpet::mlem_rows_direct_kernel, dim3(dgrid), dim3(128), 0, stream, bs.sorted, bs.stride, bs.meta, dp, g_ws.wT,
-                        g_ws.accT, g_ws.counters));
+    // the work counter meta[3] is zero before the tiled kernel: bin_scan_kernel zeroes it and the direct kernel, the last
+    // kernel of every run over a sorted set, zeroes it again (jpet_reconstruct sorts once and iterates)
+    const int dgrid = dp.t_max >= 0.f ? w.sm_count : w.sm_count * 16;
+    if (g_opt.exact_kernel > 0)
+        CUDA_TRY(launch_pdl(jpet::mlem_rows_direct_kernel<true>, dim3(dgrid), dim3(128), 0, st, (const float*)bs.sorted, 16, bs.meta, dp,
+                            (const float*)w.wT, w.accT, w.counters, (int)g_opt.exact_kernel));
+    else
+        CUDA_TRY(launch_pdl(jpet::mlem_rows_direct_kernel<false>, dim3(dgrid), dim3(128), 0, st, (const float*)bs.sorted, 16, bs.meta, dp,
+                            (const float*)w.wT, w.accT, w.counters, 0));
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     return JPET_OK;
-}
-
-template <int NWE, int NG, int NJA, int NJB, int HS, int MINB, int DEG, int BW>
-int launch_rows3(const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t stream) {
-    constexpr int NT = NWE * NG * 32;
-    auto kern = jpet::mlem_rows3_kernel<NWE, NG, NJA, NJB, HS, MINB, DEG, BW>;
-    if (bs.stride != 16) return fail(JPET_E_INVAL, "internal: rows3 kernel needs event records");
-    if (dp.t_max >= 0.f) {
-        if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
-        static size_t attr_set = 0;
-        if (smem > 40 * 1024 && smem > attr_set) {
-            CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            attr_set = smem;
-        }
-        int per_sm = 0;
-        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
-        if (per_sm < 1) return fail(JPET_E_CUDA, "event kernel does not fit on an SM (%zu B of shared memory)", smem);
-        if (g_opt_ctas_per_sm > 0) per_sm = (int)std::min<int64_t>(per_sm, g_opt_ctas_per_sm);
-        int64_t max_items = bs.n / batch_chunk(bs.n, dp) + (int64_t)dp.nby * dp.nbz + 1;
-        int grid = (int)std::min<int64_t>((int64_t)g_ws.sm_count * per_sm, std::max<int64_t>(max_items, 1));
-        if (g_opt_time_kernel) {
-            if (g_tk_used + 2 > g_tk.size()) {
-                g_tk.resize(g_tk_used + 2, nullptr);
-                CUDA_TRY(cudaEventCreate(&g_tk[g_tk_used])); CUDA_TRY(cudaEventCreate(&g_tk[g_tk_used + 1]));
-            }
-            CUDA_TRY(cudaEventRecord(g_tk[g_tk_used], stream));
-        }
-        CUDA_TRY(launch_pdl(kern, dim3(grid), dim3(NT), smem, stream, reinterpret_cast<const jpet::EventRec*>(bs.sorted), bs.items,
-                            bs.meta, dp, g_ws.wT, g_ws.accT, g_ws.tab, g_ws.counters));
-        g_launches++;
-        if (g_opt_time_kernel) { CUDA_TRY(cudaEventRecord(g_tk[g_tk_used + 1], stream)); g_tk_used += 2; }
-        CUDA_TRY(cudaGetLastError());
-    }
-    int dgrid = dp.t_max >= 0.f ? g_ws.sm_count : g_ws.sm_count * 16;
-    CUDA_TRY(launch_pdl(jpet::mlem_rows_direct_kernel, dim3(dgrid), dim3(128), 0, stream, bs.sorted, bs.stride, bs.meta, dp, g_ws.wT,
-                        g_ws.accT, g_ws.counters));
-    g_launches++;
-    CUDA_TRY(cudaGetLastError());
-    return JPET_OK;
-}
-
-int dispatch_rows(int variant, const BinSet& bs, const DevParams& dp, size_t smem, cudaStream_t st) {
-    switch (variant) {
-        case kNumVariants2 + 0: return launch_rows3<1, 4, 20, 8, 64, 4, 0, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 1: return launch_rows3<1, 4, 12, 0, 64, 4, 0, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 2: return launch_rows3<4, 1, 36, 0, 128, 1, 0, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 3: return launch_rows3<4, 1, 44, 0, 128, 1, 0, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 4: return launch_rows3<2, 2, 36, 28, 128, 1, 0, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 5: return launch_rows3<1, 8, 20, 8, 64, 2, 0, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 6: return launch_rows3<1, 2, 20, 8, 64, 8, 0, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 7: return launch_rows3<1, 4, 20, 8, 64, 3, 0, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 8: return launch_rows3<1, 4, 20, 8, 64, 2, 0, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 9: return launch_rows3<1, 4, 20, 8, 64, 4, 4, 4>(bs, dp, smem, st);
-        case kNumVariants2 + 10: return launch_rows3<1, 4, 12, 0, 64, 4, 4, 4>(bs, dp, smem, st);
-        case kNumVariants2 + 11: return launch_rows3<4, 1, 36, 0, 128, 1, 5, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 12: return launch_rows3<4, 1, 44, 0, 128, 1, 4, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 13: return launch_rows3<1, 4, 20, 8, 64, 4, 5, 4>(bs, dp, smem, st);
-        case kNumVariants2 + 14: return launch_rows3<1, 4, 12, 0, 64, 4, 5, 4>(bs, dp, smem, st);
-        case kNumVariants2 + 15: return launch_rows3<4, 1, 36, 0, 128, 1, 4, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 16: return launch_rows3<4, 1, 44, 0, 128, 1, 5, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 17: return launch_rows3<1, 4, 20, 8, 64, 4, 4, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 18: return launch_rows3<1, 4, 20, 8, 64, 4, 0, 4>(bs, dp, smem, st);
-        case kNumVariants2 + 19: return launch_rows3<1, 4, 12, 0, 64, 4, 4, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 20: return launch_rows3<1, 4, 12, 0, 64, 4, 5, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 21: return launch_rows3<1, 4, 20, 8, 64, 4, 5, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 22: return launch_rows3<4, 4, 36, 0, 128, 1, 5, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 23: return launch_rows3<4, 4, 44, 0, 128, 1, 4, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 24: return launch_rows3<4, 3, 36, 0, 128, 1, 5, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 25: return launch_rows3<4, 3, 44, 0, 128, 1, 4, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 26: return launch_rows3<4, 4, 36, 0, 128, 1, 0, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 27: return launch_rows3<4, 4, 44, 0, 128, 1, 0, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 28: return launch_rows3<4, 4, 36, 0, 128, 1, 4, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 29: return launch_rows3<4, 4, 44, 0, 128, 1, 5, 8>(bs, dp, smem, st);
-        case kNumVariants2 + 30: return launch_rows3<1, 4, 20, 8, 64, 4, 4, 16>(bs, dp, smem, st);
-        case kNumVariants2 + 31: return launch_rows3<4, 4, 44, 0, 128, 1, 4, 16>(bs, dp, smem, st);
-        case kNumVariants2 + 32: return launch_rows3<4, 4, 36, 0, 128, 1, 5, 16>(bs, dp, smem, st);
-        case kNumVariants2 + 33: return launch_rows3<3, 4, 36, 8, 128, 1, 5, 16>(bs, dp, smem, st);
-        case kNumVariants2 + 34: return launch_rows3<3, 4, 44, 8, 128, 1, 4, 16>(bs, dp, smem, st);
-        case kNumVariants2 + 35: return launch_rows3<1, 4, 20, 8, 64, 4, 4, 32>(bs, dp, smem, st);
-        case kNumVariants2 + 36: return launch_rows3<4, 4, 44, 0, 128, 1, 4, 32>(bs, dp, smem, st);
-        case kNumVariants2 + 37: return launch_rows3<3, 4, 36, 8, 128, 1, 5, 32>(bs, dp, smem, st);
-        case kNumVariants2 + 38: return launch_rows3<1, 4, 12, 0, 64, 4, 4, 16>(bs, dp, smem, st);
-        case kNumVariants2 + 39: return launch_rows3<1, 4, 12, 0, 64, 4, 0, 16>(bs, dp, smem, st);
-        case 0: return launch_rows<1, 1, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
-        case 1: return launch_rows<2, 1, 1, 20, 64, 4, true, 10, false>(bs, dp, smem, st);
-        case 2: return launch_rows<4, 2, 1, 12, 64, 4, true, 1, false>(bs, dp, smem, st);
-        case 3: return launch_rows<4, 1, 1, 36, 128, 4, true, 1, false>(bs, dp, smem, st);
-        case 4: return launch_rows<8, 2, 1, 20, 128, 4, true, 1, false>(bs, dp, smem, st);
-        case 5: return launch_rows<8, 2, 1, 24, 160, 4, true, 1, false>(bs, dp, smem, st);
-        case 6: return launch_rows<4, 1, 1, 44, 160, 4, true, 1, false>(bs, dp, smem, st);
-        case 7: return launch_rows<1, 1, 2, 20, 64, 4, true, 1, false>(bs, dp, smem, st);
-        case 8: return launch_rows<2, 1, 1, 20, 64, 4, true, 10, true>(bs, dp, smem, st);
-        case 9: return launch_rows<8, 2, 1, 20, 128, 4, true, 1, true>(bs, dp, smem, st);
-        case 10: return launch_rows<4, 1, 1, 44, 160, 4, true, 1, true>(bs, dp, smem, st);
-        case 11: return launch_rows<1, 1, 1, 12, 64, 4, true, 1, true>(bs, dp, smem, st);
-        case 12: return launch_rows2<1, 1, 1, 20, 64, 4, true, 10>(bs, dp, smem, st);
-        case 13: return launch_rows2<1, 1, 1, 20, 64, 4, false, 10>(bs, dp, smem, st);
-        case 14: return launch_rows2<1, 1, 0, 12, 64, 4, true, 1>(bs, dp, smem, st);
-        case 15: return launch_rows2<3, 2, 1, 20, 128, 4, true, 1>(bs, dp, smem, st);
-        case 16: return launch_rows2<4, 2, 0, 24, 160, 4, true, 1>(bs, dp, smem, st);
-        case 17: return launch_rows2<4, 2, 0, 20, 128, 4, true, 1>(bs, dp, smem, st);
-        case 18: return launch_rows2<3, 2, 1, 24, 160, 4, true, 1>(bs, dp, smem, st);
-        case 19: return launch_rows2<4, 1, 0, 44, 160, 4, true, 1>(bs, dp, smem, st);
-        case 20: return launch_rows2<3, 1, 1, 36, 128, 4, true, 1>(bs, dp, smem, st);
-        default: return fail(JPET_E_INVAL, "unknown kernel variant %d", variant);
-    }
 }
 
 // Constants of the event kernel (computed in double, rounded once), the tiling of the image into
-// sub-tiles + halo regions, and the kernel variant.
-void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& gr, float a3, float gamma, DevParams* out,
-               int* variant, size_t* smem_out, std::vector<uint32_t>* tab_out = nullptr) {
+// sub-tiles + halo regions, and the kernel shape.
+void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& gr, jpet_host::RowsPlan* out,
+               std::vector<uint32_t>* tab_out = nullptr) {
     DevParams p{};
+    const float a3 = g_opt.a3_coef, gamma = g_opt.gamma;
     const double LH = 0.72134752044448170368;
+    const double eta = g_opt.sz_eta, szm = sigma_z_max(sg);          // largest sigma_z an event can see
     double iz2 = 1.0 / ((double)sg.sigma_z * sg.sigma_z), il2 = 1.0 / ((double)sg.sigma_dl * sg.sigma_dl);
     double px = gr.pixel;
     p.n_y = gr.n_y; p.n_z = gr.n_z;
     p.px = (float)px; p.inv_px = (float)(1.0 / px);
     p.y0 = (float)(-0.5 * (gr.n_y - 1) * px); p.z0 = (float)(-0.5 * (gr.n_z - 1) * px);
-    p.inv2R = (float)(1.0 / (2.0 * g.R)); p.R2 = (float)((double)g.R * g.R);
+    p.inv2R = (float)(1.0 / (2.0 * g.R)); p.R2 = (float)((double)g.R * g.R); p.R = g.R;
     p.hy_coef = (float)(1.5 * sg.sigma_dl);
     p.half_sz2 = (float)(0.5 * (double)sg.sigma_z * sg.sigma_z);
     p.c1s = (float)(-LH * 2.0 * iz2);
@@ -478,82 +334,66 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     p.d3k = (float)(4.0 * il2);
     p.gB = (float)(4.0 * (double)gamma * g.R);
     p.gD0 = (float)(4.0 * (double)gamma * g.R * a3);
+    p.sz_eta = (float)eta;
+    p.inv_hL2 = (float)(4.0 / ((double)g.L * g.L));
     // ellipse extents in pixels: half height 1.5 sigma_dl cos(theta), half width 3 sqrt(sz^2/2 + sdl^2 sin^2/4) (App. B)
-    double t_max = ((double)g.L + 8.0 * sg.sigma_z) / (2.0 * g.R);
+    double t_max = ((double)g.L + 8.0 * szm) / (2.0 * g.R);
     double sin2 = t_max * t_max / (1.0 + t_max * t_max);
     double hy = 1.5 * sg.sigma_dl / px;
-    double hz = 3.0 * std::sqrt(0.5 * (double)sg.sigma_z * sg.sigma_z + 0.25 * (double)sg.sigma_dl * sg.sigma_dl * sin2) / px;
-    double chord = 6.0 * sg.sigma_z / std::sqrt(2.0) / px;
-    int rows_max = std::min<int>(gr.n_y, (int)std::floor(2.0 * hy) + 2);
-    int chord_max = std::min<int>(gr.n_z, (int)std::floor(chord) + 2);
+    double hz = 3.0 * std::sqrt(0.5 * szm * szm + 0.25 * (double)sg.sigma_dl * sg.sigma_dl * sin2) / px;
+    const double H0p_max = 9.0 * 0.5 * szm * szm / (px * px);       // half chord^2 at the centre row, widest event
     p.Hy = (int)std::ceil(hy) + 1;
     p.Hz = (int)std::ceil(hz) + 1;
     p.t_max = (float)t_max;
     // ellipse row counts a regular event can have (unclipped): hy_px * cos(theta) for |tan theta| <= t_max, +- rounding
     const int nr_hi = std::min(255, (int)std::floor(2.0 * hy) + 2);
     const int nr_lo = std::max(1, (int)std::floor(2.0 * hy / std::sqrt(1.0 + t_max * t_max)) - 1);
-    // variant: smallest shape that holds rows_max rows, chord_max pixels per row, and the region's rows
-    auto fits = [&](const Variant& c) {
-        if (c.NA > 0) return rows_max + 1 <= 32 * (c.NA + c.NBW) && chord_max + 1 <= c.NJ * c.NH && 2 * p.Hy + 4 <= c.HS;
-        return rows_max + 1 <= c.NW * 32 / c.NH * c.NR && chord_max <= c.NJ * c.NH && 2 * p.Hy + 4 <= c.HS;
-    };
     std::vector<uint32_t> tab;
-    auto fits3 = [&](const Variant3& c) {
-        return 2 * p.Hy + 4 <= c.HS && jpet_host::build_task_table(nr_lo, nr_hi, (double)p.H0p, c.NWE, c.NJA, c.NJB, &tab);
+    auto fits = [&](const Shape& c) {
+        return 2 * p.Hy + 4 <= c.HS && jpet_host::build_task_table(nr_lo, nr_hi, H0p_max, c.NWE, c.NJA, c.NJB, &tab);
     };
     int v = -1;
-    if (g_opt_variant >= 0) v = (int)g_opt_variant;
+    if (g_opt.variant >= 0) v = (int)g_opt.variant;
     else {
-        // third-generation shapes first; degree of the exponent polynomial from the truncation bound (mlem_rows3.cuh,
-        // poly_coeffs2): |x| = |eps u / delta| <= xb, ba^2 / D <= eb inside the ellipse and the image
-        const double y_max = 0.5 * gr.n_y * px, u_max = 3.0 * sg.sigma_z / std::sqrt(2.0), R2 = (double)g.R * g.R;
+        // degree of the exponent polynomial from the truncation bound (mlem_rows.cuh, poly_coeffs2):
+        // |x| = |eps u / delta| <= xb, ba^2 / D <= eb inside the ellipse and the image.  A position-dependent sigma_z
+        // adds the term Dl R to S y in alpha and eps (common.cuh): |Dl| / S <= dls, i.e. y grows by at most dls R.
+        const double dls = ((1.0 + eta) * (1.0 + eta) - 1.0) / ((1.0 + eta) * (1.0 + eta) + 1.0);
+        const double y_max = 0.5 * gr.n_y * px + dls * g.R, u_max = 3.0 * szm / std::sqrt(2.0), R2 = (double)g.R * g.R;
         // gamma (Eq. 12): delta changes by at most g_rel of itself, |b.C^-1.a| / sqrt(D) grows by at most g_ba
         const double ag = std::fabs((double)gamma);
-        const double g_rel = 2.0 * ag * std::fabs((double)a3) * y_max * sg.sigma_z * sg.sigma_z * (t_max / std::sqrt(1.0 + t_max * t_max)) / g.R;
-        const double g_ba = 6.0 / std::sqrt(2.0) * ag * sg.sigma_z * sg.sigma_dl;
-        const double xb = 2.0 * (t_max / (1.0 + t_max * t_max)) * y_max * u_max / (R2 + y_max * y_max) / (0.95 - g_rel);
+        const double g_rel = 2.0 * ag * std::fabs((double)a3) * y_max * szm * szm * (t_max / std::sqrt(1.0 + t_max * t_max)) / g.R;
+        const double g_ba = 6.0 / std::sqrt(2.0) * ag * szm * sg.sigma_dl;
+        const double xb = 2.0 * (t_max / (1.0 + t_max * t_max)) * y_max * u_max / (R2 + y_max * y_max) / (0.95 - g_rel - 2.0 * dls * y_max * g.R / (R2 + y_max * y_max));
         const double eb = 1.1 * std::pow(3.0 * y_max / std::sqrt(R2 + y_max * y_max) + g_ba, 2.0);
         auto trunc_err = [&](int deg) {      // log2 units
             return 1.4427 * (0.5 * eb * std::pow(xb, deg - 1) / (1.0 - xb) + 0.5 * std::pow(xb, deg + 1) / (deg + 1));
         };
-        const int deg_sel = g_opt_poly_off ? 0 : (trunc_err(4) <= 2e-5 ? 1 : (trunc_err(5) <= 2e-5 ? 2 : 0));
+        const int deg = g_opt.poly_off || !(xb > 0.0 && xb < 0.5) ? 0 : (trunc_err(4) <= 2e-5 ? 4 : (trunc_err(5) <= 2e-5 ? 5 : 0));
         // ellipses of at most ~100 rows on three warps instead of four (config 4: 91 rows on 128 lanes leave a quarter of
         // the lanes idle; 14.60 -> 14.02 ms per 5x10^6 events), the few rows beyond 96 as B pieces
-        if (deg_sel == 2 && nr_hi > 64 && nr_hi <= 104 && fits3(kVariants3[37])) v = kNumVariants2 + 37;
-        for (int sh = 0; sh < 4 && v < 0; ++sh)
-            if (fits3(kVariants3[kShape3[sh][deg_sel]])) v = kNumVariants2 + kShape3[sh][deg_sel];
-        const int order[] = {14, 12, 15, 16, 0, 8, 9, 10, 5};
-        for (int cand : order)
-            if (v < 0 && fits(kVariants[cand])) { v = cand; break; }
-        if (v < 0) v = 5;
+        if (deg == 5 && nr_hi > 64 && nr_hi <= 104 && fits(kShapes[jpet_host::k_wide3_deg5])) v = jpet_host::k_wide3_deg5;
+        for (int s = 0; s < kNumShapes && v < 0; ++s)           // the list is ordered by size within each degree
+            if (kShapes[s].DEG == deg && kShapes[s].NWE != 3 && fits(kShapes[s])) v = s;
     }
-    const bool gen3 = v >= kNumVariants2;
-    // else: every event takes the direct path (the later generations have no overflow loops)
-    bool tiles_ok;
-    int v_HS, v_NJ, n_regions = 2;
-    if (gen3) {
-        const Variant3& c = kVariants3[v - kNumVariants2];
-        tiles_ok = fits3(c);
-        v_HS = c.HS; v_NJ = c.NJA; n_regions = 1 + c.NG;
-        p.nr_min = nr_lo; p.nr_max = nr_hi;
-    } else {
-        tiles_ok = 2 * p.Hy + 4 <= kVariants[v].HS && (kVariants[v].NA == 0 || fits(kVariants[v]));
-        v_HS = kVariants[v].HS; v_NJ = kVariants[v].NJ;
-        p.nr_min = 0; p.nr_max = 0;
-        tab.clear();
-    }
-    p.HS = v_HS;
+    // no shape fits (or a forced shape does not): every event takes the direct path
+    bool tiles_ok = v >= 0 && fits(kShapes[v]);
+    if (v < 0) v = 0;
+    const Shape& c = kShapes[v];
+    const int n_regions = 1 + c.NG;
+    p.nr_min = nr_lo; p.nr_max = nr_hi;
+    p.HS = c.HS;
     p.Sy = std::max(1, p.HS - 2 * p.Hy);
-    // shared memory: w region + accumulator region(s) (+ task table).  The sub-tile width Sz (8 or 4 columns) is the
+    // shared memory: w region + accumulator regions + task table.  The sub-tile width Sz (8 or 4 columns) is the
     // one that lets most warps live on an SM (228 KB per SM, 1 KB reserved per CTA, 227 KB per CTA); 8 on a tie.
     const size_t budget = 225 * 1024, sm_bytes = 228 * 1024, tab_bytes = tab.size() * sizeof(uint32_t);
-    const int cta_warps = gen3 ? kVariants3[v - kNumVariants2].NWE * kVariants3[v - kNumVariants2].NG : kVariants[v].NW;
+    const int cta_warps = c.NWE * c.NG;
     size_t smem = 0;
     {
         int best_sz = 4;
         size_t best_warps = 0;
         for (int sz : {8, 4}) {
-            if (g_opt_sz > 0) sz = (int)g_opt_sz;
+            if (g_opt.sz > 0) sz = (int)g_opt.sz;
             const size_t need = n_regions * sizeof(float) * (size_t)p.HS * (sz + 2 * p.Hz) + tab_bytes;
             const size_t ctas = need <= budget ? std::min<size_t>(sm_bytes / (need + 2048), 2048 / (32 * cta_warps)) : 0;
             if (ctas * cta_warps > best_warps) { best_warps = ctas * cta_warps; best_sz = sz; }
@@ -562,42 +402,32 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
         p.WZ = p.Sz + 2 * p.Hz;
         smem = n_regions * sizeof(float) * (size_t)p.HS * p.WZ + tab_bytes;
     }
-    if (smem > budget || !tiles_ok || p.WZ < v_NJ + 4 || g_opt_force_direct) { p.t_max = -1.f; smem = 0; p.nr_min = p.nr_max = 0; tab.clear(); }
+    if (smem > budget || !tiles_ok || p.WZ < c.NJA + 4 || g_opt.force_direct || g_opt.exact_kernel > 0) {
+        p.t_max = -1.f; smem = 0; p.nr_min = p.nr_max = 0; tab.clear();
+    }
     p.nby = (gr.n_y + 2 * p.Hy + p.Sy - 1) / p.Sy;
     p.nbz = (gr.n_z + 2 * p.Hz + p.Sz - 1) / p.Sz;
     // events per work item (one staging of w and one flush of the accumulator regions per item): measured optimum on B200
-    // 128 events per group for the one-warp groups (config 2: 0.740 -> 0.734 ms), 256 for the four-warp groups
+    // 128 events per group for the one-warp groups (config 2: 0.740 -> 0.734 ms), 256 for the multi-warp groups
     // (configs 4, 5: +5-8 %)
-    p.chunk = g_opt_chunk > 0 ? (int)g_opt_chunk
-                              : (gen3 ? (kVariants3[v - kNumVariants2].NWE > 1 ? 256 : 128) * kVariants3[v - kNumVariants2].NG : 64);
-    *out = p;
-    *variant = v;
-    *smem_out = smem;
+    p.chunk = g_opt.chunk > 0 ? (int)g_opt.chunk : (c.NWE > 1 ? 256 : 128) * c.NG;
+    out->dp = p;
+    out->shape = v;
+    out->smem = smem;
+    out->vs = eta != 0.0;
     if (tab_out) tab_out->swap(tab);
 }
 
-bool same_problem(const jpet_geometry& g, const jpet_grid& gr) {
-    return g_ws.s_valid && g_ws.geom.R == g.R && g_ws.geom.L == g.L && g_ws.grid.n_y == gr.n_y &&
-           g_ws.grid.n_z == gr.n_z && g_ws.grid.pixel == gr.pixel;
+bool same_problem(const Workspace& w, const jpet_geometry& g, const jpet_grid& gr) {
+    return w.s_valid && w.geom.R == g.R && w.geom.L == g.L && w.grid.n_y == gr.n_y && w.grid.n_z == gr.n_z && w.grid.pixel == gr.pixel;
 }
 
 int grid_for(int64_t M) { return (int)((M + 255) / 256); }
 
-int plan_stride() { return (g_ws.variant >= kNumVariants2 || kVariants[g_ws.variant].NA > 0) ? 16 : 3; }
-
-// Events per work item for a batch of n events: the plan's size, halved (not below 64) while the batch would give fewer
-// than four items per SM - small batches are launch- and tail-bound.
-int batch_chunk(int64_t n, const DevParams& dp) {
-    int chunk = dp.chunk;
-    if (g_opt_chunk > 0) return chunk;
-    while (chunk > 64 && n / chunk < 4 * (int64_t)g_ws.sm_count) chunk /= 2;
-    return chunk;
-}
-
-int ensure_binset(BinSet& bs, int64_t n, const DevParams& dp, bool need_sorted) {
-    size_t items_cap = (size_t)(n / batch_chunk(n, dp)) + (size_t)dp.nby * dp.nbz + 2;
-    bs.stride = plan_stride();
-    const size_t need_floats = (size_t)bs.stride * (size_t)std::max<int64_t>(n, 1);
+int ensure_binset(Workspace& w, BinSet& bs, int64_t n, bool need_sorted) {
+    const DevParams& dp = w.plan.dp;
+    size_t items_cap = (size_t)(n / batch_chunk(w, n)) + (size_t)dp.nby * dp.nbz + 2;
+    const size_t need_floats = 16 * (size_t)std::max<int64_t>(n, 1);
     if (need_sorted && need_floats > bs.cap_events) {          // cap_events counts floats
         if (bs.owns_sorted) cudaFree(bs.sorted);
         bs.sorted = nullptr; bs.cap_events = 0;
@@ -622,45 +452,58 @@ void free_binset(BinSet& bs) {
     bs = BinSet{};
 }
 
+constexpr size_t kTileBytes = sizeof(float) * 3 * jpet::kBinTile;
+
+int ensure_sort_attr(Workspace& w) {
+    if (w.sort_attr_set) return JPET_OK;
+    const int bytes = (int)(kTileBytes + sizeof(int) * jpet::kBinSmemMax);
+    CUDA_TRY(cudaFuncSetAttribute(jpet::bin_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CUDA_TRY(cudaFuncSetAttribute(jpet::bin_scatter_rec_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    w.sort_attr_set = true;
+    return JPET_OK;
+}
+
 // Counting sort of one batch (<= kMaxBatch events) by sub-tile into bs.sorted, and its work items.
-int bin_batch(const float* events, int64_t n, BinSet& bs, const DevParams& dp, cudaStream_t st) {
+int bin_batch(Workspace& w, const float* events, int64_t n, BinSet& bs, cudaStream_t st) {
+    const DevParams& dp = w.plan.dp;
     const int nb = dp.nby * dp.nbz;
-    if ((size_t)n > g_ws.cap_bin_of) {
-        cudaFree(g_ws.bin_of);
-        g_ws.bin_of = nullptr; g_ws.cap_bin_of = 0;
-        CUDA_TRY(cudaMalloc(&g_ws.bin_of, sizeof(int) * (size_t)n));
-        g_ws.cap_bin_of = (size_t)n;
+    int rc = ensure_sort_attr(w);
+    if (rc) return rc;
+    if ((size_t)n > w.cap_place) {
+        cudaFree(w.place);
+        w.place = nullptr; w.cap_place = 0;
+        CUDA_TRY(cudaMalloc(&w.place, sizeof(int2) * (size_t)n));
+        w.cap_place = (size_t)n;
     }
-    if ((size_t)(2 * (nb + 1)) > g_ws.cap_counts) {
-        cudaFree(g_ws.counts);
-        g_ws.counts = nullptr; g_ws.cap_counts = 0;
-        CUDA_TRY(cudaMalloc(&g_ws.counts, sizeof(int) * 2 * (size_t)(nb + 1)));
-        g_ws.cap_counts = (size_t)(2 * (nb + 1));
-        g_ws.counts_clean_nb = -1;
+    if ((size_t)(2 * (nb + 1)) > w.cap_counts) {
+        cudaFree(w.counts);
+        w.counts = nullptr; w.cap_counts = 0;
+        CUDA_TRY(cudaMalloc(&w.counts, sizeof(int) * 2 * (size_t)(nb + 1)));
+        w.cap_counts = (size_t)(2 * (nb + 1));
+        w.counts_clean_nb = -1;
     }
-    int* counts = g_ws.counts;
-    int* cursors = g_ws.counts + (nb + 1);
-    if (g_ws.counts_clean_nb != nb) {        // bin_scan_kernel leaves the counts zeroed: a memset only when the layout changes
+    int* counts = w.counts;
+    int* cursors = w.counts + (nb + 1);
+    if (w.counts_clean_nb != nb) {        // bin_scan_kernel leaves the counts zeroed: a memset only when the layout changes
         CUDA_TRY(cudaMemsetAsync(counts, 0, sizeof(int) * (nb + 1), st));
-        g_ws.counts_clean_nb = nb;
+        w.counts_clean_nb = nb;
     }
-    const int per_block = jpet::kBinBlock * jpet::kBinPer;
-    const int blocks = (int)((n + per_block - 1) / per_block);
+    const int blocks = (int)((n + jpet::kBinTile - 1) / jpet::kBinTile);
     const int use_smem = nb + 1 <= jpet::kBinSmemMax;
-    const size_t hist_bytes = use_smem ? sizeof(int) * (size_t)(nb + 1) : 0;
+    const size_t smem_bytes = kTileBytes + (use_smem ? sizeof(int) * (size_t)(nb + 1) : 0);
+    const int saved_clean = w.counts_clean_nb;
+    w.counts_clean_nb = -1;                 // dirty until bin_scan_kernel has been queued (an error in between leaves it so)
     if (n > 0) {
-        CUDA_TRY(launch_pdl(jpet::bin_count_kernel, dim3(blocks), dim3(jpet::kBinBlock), hist_bytes, st, events, (int)n, dp, g_ws.bin_of,
+        CUDA_TRY(launch_pdl(jpet::bin_count_kernel, dim3(blocks), dim3(jpet::kBinBlock), smem_bytes, st, events, (int)n, dp, w.place,
                             counts, nb + 1, use_smem));
         g_launches++;
     }
-    CUDA_TRY(launch_pdl(jpet::bin_scan_kernel, dim3(1), dim3(1024), 0, st, counts, cursors, bs.items, bs.meta, nb, batch_chunk(n, dp)));
+    CUDA_TRY(launch_pdl(jpet::bin_scan_kernel, dim3(1), dim3(1024), 0, st, counts, cursors, bs.items, bs.meta, nb, batch_chunk(w, n)));
     g_launches++;
+    w.counts_clean_nb = saved_clean;
     if (n > 0) {
-        if (bs.stride == 16)
-            CUDA_TRY(launch_pdl(jpet::bin_scatter_rec_kernel, dim3(blocks), dim3(jpet::kBinBlock), hist_bytes, st, events, (int)n,
-                                g_ws.bin_of, cursors, reinterpret_cast<jpet::EventRec*>(bs.sorted), dp, nb + 1, use_smem));
-        else
-            jpet::bin_scatter_kernel<<<blocks, jpet::kBinBlock, hist_bytes, st>>>(events, (int)n, g_ws.bin_of, cursors, bs.sorted, nb + 1, use_smem);
+        CUDA_TRY(launch_pdl(jpet::bin_scatter_rec_kernel, dim3(blocks), dim3(jpet::kBinBlock), smem_bytes, st, events, (int)n,
+                            (const int2*)w.place, cursors, reinterpret_cast<jpet::EventRec*>(bs.sorted), dp, nb + 1, use_smem));
         g_launches++;
     }
     CUDA_TRY(cudaGetLastError());
@@ -668,186 +511,198 @@ int bin_batch(const float* events, int64_t n, BinSet& bs, const DevParams& dp, c
     return JPET_OK;
 }
 
-int run_binset(BinSet& bs, cudaStream_t st) {
-    // the work counter meta[3] is zero here: bin_scan_kernel zeroes it and mlem_rows_direct_kernel, the last kernel of every
-    // run over a sorted set, zeroes it again
-    return dispatch_rows(g_ws.variant, bs, g_ws.dp, g_ws.smem, st);
-}
-
-int do_begin(const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr, const float* rho_in, cudaStream_t st) {
+int do_begin(Workspace& w, const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr, const float* rho_in, cudaStream_t st) {
     int rc = validate(g, sg, gr);
     if (rc) return rc;
     if (!sg) return fail(JPET_E_INVAL, "NULL sigmas");
     if (!rho_in) return fail(JPET_E_INVAL, "NULL rho_in");
-    if ((rc = ensure_device())) return rc;
     const int M = gr->n_y * gr->n_z;
-    if ((rc = ensure_images(M))) return rc;
-    if (!same_problem(*g, *gr)) {
-        jpet::sensitivity_kernel<<<grid_for(M), 256, 0, st>>>(g_ws.s, gr->n_y, gr->n_z, gr->pixel, g->R, g->L);
+    if ((rc = ensure_images(w, M))) return rc;
+    w.open = false;
+    if (!same_problem(w, *g, *gr)) {
+        jpet::sensitivity_kernel<<<grid_for(M), 256, 0, st>>>(w.s, gr->n_y, gr->n_z, gr->pixel, g->R, g->L);
         g_launches++;
         CUDA_TRY(cudaGetLastError());
-        g_ws.geom = *g; g_ws.grid = *gr; g_ws.s_valid = true;
+        w.geom = *g; w.grid = *gr; w.s_valid = true;
     }
-    g_ws.sig = *sg; g_ws.M = M;
+    w.sig = *sg; w.M = M;
     {   // the plan depends only on these inputs: rebuild it (and the task table) when one of them changes
-        const PlanKey key{*g, *sg, *gr, g_a3_coef, g_gamma, g_opt_variant, g_opt_sz, g_opt_chunk, g_opt_force_direct + 2 * g_opt_poly_off};
-        if (!g_ws.plan_valid || memcmp(&key, &g_ws.plan_key, sizeof key) != 0) {
-            make_plan(*g, *sg, *gr, g_a3_coef, g_gamma, &g_ws.dp, &g_ws.variant, &g_ws.smem, &g_ws.tab_host);
-            g_ws.plan_key = key;
-            g_ws.plan_valid = true;
+        PlanKey key;
+        key.g = *g; key.sg = *sg; key.gr = *gr; key.a3 = g_opt.a3_coef; key.gamma = g_opt.gamma; key.sz_eta = g_opt.sz_eta;
+        key.variant = g_opt.variant; key.sz = g_opt.sz; key.chunk = g_opt.chunk; key.force_direct = g_opt.force_direct;
+        key.poly_off = g_opt.poly_off; key.exact = g_opt.exact_kernel;
+        if (!w.plan_valid || !(key == w.plan_key)) {
+            make_plan(*g, *sg, *gr, &w.plan, &w.tab_host);
+            w.plan_key = key;
+            w.plan_valid = true;
         }
     }
-    if (g_ws.variant < 0 || g_ws.variant >= kNumVariants) return fail(JPET_E_INVAL, "unknown kernel variant");
-    if (!g_ws.tab_host.empty() && g_ws.tab_host != g_ws.tab_uploaded) {        // task table of the third-generation kernel
-        if (g_ws.tab_host.size() > g_ws.cap_tab) {
-            cudaFree(g_ws.tab);
-            g_ws.tab = nullptr; g_ws.cap_tab = 0;
-            CUDA_TRY(cudaMalloc(&g_ws.tab, sizeof(uint32_t) * g_ws.tab_host.size()));
-            g_ws.cap_tab = g_ws.tab_host.size();
+    if (w.plan.shape < 0 || w.plan.shape >= kNumShapes) return fail(JPET_E_INVAL, "unknown kernel shape");
+    if (!w.tab_host.empty() && w.tab_host != w.tab_uploaded) {        // task table of the tiled event kernel
+        if (w.tab_host.size() > w.cap_tab) {
+            cudaFree(w.tab);
+            w.tab = nullptr; w.cap_tab = 0;
+            CUDA_TRY(cudaMalloc(&w.tab, sizeof(uint32_t) * w.tab_host.size()));
+            w.cap_tab = w.tab_host.size();
         }
-        g_ws.tab_uploaded = g_ws.tab_host;      // the copy below reads tab_uploaded, which stays put until the next change
-        CUDA_TRY(cudaMemcpyAsync(g_ws.tab, g_ws.tab_uploaded.data(), sizeof(uint32_t) * g_ws.tab_uploaded.size(),
-                                 cudaMemcpyHostToDevice, st));
+        w.tab_uploaded = w.tab_host;      // the copy below reads tab_uploaded, which stays put until the next change
+        CUDA_TRY(cudaMemcpyAsync(w.tab, w.tab_uploaded.data(), sizeof(uint32_t) * w.tab_uploaded.size(), cudaMemcpyHostToDevice, st));
     }
-    g_tk_used = 0;                 // last_kernel_ns covers the event-kernel launches of one iteration
-    CUDA_TRY(launch_pdl(jpet::prepass_kernel, dim3(grid_for(M)), dim3(256), 0, st, (const float*)g_ws.s, rho_in, g_ws.wT, g_ws.accT,
-                        gr->n_y, gr->n_z, g_ws.counters));
+    w.tk_used = 0;                 // last_kernel_ns covers the event-kernel launches of one iteration
+    CUDA_TRY(launch_pdl(jpet::prepass_kernel, dim3(grid_for(M)), dim3(256), 0, st, (const float*)w.s, rho_in, w.wT, w.accT, gr->n_y,
+                        gr->n_z, w.counters));
     g_launches++;
     CUDA_TRY(cudaGetLastError());
-    g_ws.open = true;
+    w.open = true;
     return JPET_OK;
 }
 
-int do_accumulate(const float* events, int64_t n, cudaStream_t st) {
-    if (!g_ws.open) return fail(JPET_E_INVAL, "jpet_mlem_accumulate without jpet_mlem_begin");
+int do_accumulate(Workspace& w, const float* events, int64_t n, cudaStream_t st) {
+    if (!w.open) return fail(JPET_E_INVAL, "jpet_mlem_accumulate without jpet_mlem_begin");
     if (n < 0) return fail(JPET_E_INVAL, "n < 0");
     if (n > 0 && !events) return fail(JPET_E_INVAL, "NULL events");
     for (int64_t off = 0; off < n; off += kMaxBatch) {
         int64_t nb = std::min(kMaxBatch, n - off);
-        int rc = ensure_binset(g_ws.scratch, nb, g_ws.dp, true);
-        if (rc) return rc;
-        if ((rc = bin_batch(events + 3 * off, nb, g_ws.scratch, g_ws.dp, st))) return rc;
-        if ((rc = run_binset(g_ws.scratch, st))) return rc;
+        int rc = ensure_binset(w, w.scratch, nb, true);
+        if (!rc) rc = bin_batch(w, events + 3 * off, nb, w.scratch, st);
+        if (!rc) rc = run_binset(w, w.scratch, st);
+        if (rc) { w.open = false; return rc; }
     }
     return JPET_OK;
 }
 
-int do_end(const float* rho_in, float* rho_out, cudaStream_t st) {
-    if (!g_ws.open) return fail(JPET_E_INVAL, "jpet_mlem_end without jpet_mlem_begin");
+int do_end(Workspace& w, const float* rho_in, float* rho_out, const float* const* peers, int n_peers, cudaStream_t st) {
+    if (!w.open) return fail(JPET_E_INVAL, "jpet_mlem_end without jpet_mlem_begin");
     if (!rho_in || !rho_out) return fail(JPET_E_INVAL, "NULL image pointer");
-    CUDA_TRY(launch_pdl(jpet::finalise_kernel, dim3(grid_for(g_ws.M)), dim3(256), 0, st, (const float*)g_ws.s, rho_in,
-                        (const float*)g_ws.accT, rho_out, g_ws.grid.n_y, g_ws.grid.n_z));
+    jpet::PeerAcc pa{};
+    if (peers) {
+        if (n_peers < 1 || n_peers > jpet::kMaxPeers) return fail(JPET_E_INVAL, "n_peers must be 1 .. %d", jpet::kMaxPeers);
+        for (int q = 0; q < n_peers; ++q) {
+            if (!peers[q]) return fail(JPET_E_INVAL, "NULL peer accumulator");
+            pa.acc[q] = peers[q];
+        }
+        pa.n = n_peers;
+    } else {
+        pa.acc[0] = w.accT;
+        pa.n = 1;
+    }
+    w.open = false;
+    CUDA_TRY(launch_pdl(jpet::finalise_kernel, dim3(grid_for(w.M)), dim3(256), 0, st, (const float*)w.s, rho_in, pa, rho_out, w.grid.n_y,
+                        w.grid.n_z));
     g_launches++;
     CUDA_TRY(cudaGetLastError());
-    g_ws.open = false;
     return JPET_OK;
 }
 
 // n_iter iterations over device-resident events; the events are binned once (first iteration) and the
 // sorted copy is reused by the others (events never change between iterations).
-int iterate_many(const float* events, int64_t n, const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr,
+int iterate_many(Workspace& w, const float* events, int64_t n, const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr,
                  const float* rho_start, float* rho_out, int n_iter, cudaStream_t st) {
-    const int M = gr->n_y * gr->n_z;
     const float* cur = rho_start;
     const int64_t n_batches = (n + kMaxBatch - 1) / kMaxBatch;
     const bool keep = n_iter > 1;
-    if (keep) while ((int64_t)g_ws.kept.size() < n_batches) g_ws.kept.emplace_back();
+    if (keep) while ((int64_t)w.kept.size() < n_batches) w.kept.emplace_back();
     for (int it = 0; it < n_iter; ++it) {
-        float* nxt = (it == n_iter - 1) ? rho_out : (cur == g_ws.rho_a ? g_ws.rho_b : g_ws.rho_a);
-        int rc = do_begin(g, sg, gr, cur, st);        // fixes the plan (kernel variant, record stride) for this problem
+        float* nxt = (it == n_iter - 1) ? rho_out : (cur == w.rho_a ? w.rho_b : w.rho_a);
+        int rc = do_begin(w, g, sg, gr, cur, st);        // fixes the plan (kernel shape, tiling) for this problem
         if (rc) return rc;
-        const size_t stride = (size_t)plan_stride();
-        if (keep && it == 0 && stride * (size_t)n > g_ws.cap_kept_sorted) {      // capacity counts floats
-            cudaFree(g_ws.kept_sorted);
-            g_ws.kept_sorted = nullptr; g_ws.cap_kept_sorted = 0;
-            CUDA_TRY(cudaMalloc(&g_ws.kept_sorted, sizeof(float) * stride * (size_t)n));
-            g_ws.cap_kept_sorted = stride * (size_t)n;
+        if (keep && it == 0 && 16 * (size_t)n > w.cap_kept_sorted) {      // capacity counts floats
+            cudaFree(w.kept_sorted);
+            w.kept_sorted = nullptr; w.cap_kept_sorted = 0;
+            cudaError_t e = cudaMalloc(&w.kept_sorted, sizeof(float) * 16 * (size_t)n);
+            if (e != cudaSuccess) { w.open = false; return fail(JPET_E_CUDA, "cudaMalloc of the kept records failed: %s", cudaGetErrorString(e)); }
+            w.cap_kept_sorted = 16 * (size_t)n;
         }
         if (!keep) {
-            if ((rc = do_accumulate(events, n, st))) { g_ws.open = false; return rc; }
+            if ((rc = do_accumulate(w, events, n, st))) return rc;
         } else {
             for (int64_t b = 0; b < n_batches; ++b) {
-                BinSet& bs = g_ws.kept[b];
+                BinSet& bs = w.kept[b];
                 int64_t off = b * kMaxBatch, nb = std::min(kMaxBatch, n - off);
                 if (it == 0) {
+                    if (bs.owns_sorted) cudaFree(bs.sorted);
                     bs.owns_sorted = false;
-                    bs.sorted = g_ws.kept_sorted + stride * (size_t)off;
-                    if ((rc = ensure_binset(bs, nb, g_ws.dp, false))) return rc;
-                    if ((rc = bin_batch(events + 3 * off, nb, bs, g_ws.dp, st))) return rc;
+                    bs.sorted = w.kept_sorted + 16 * (size_t)off;
+                    rc = ensure_binset(w, bs, nb, false);
+                    if (!rc) rc = bin_batch(w, events + 3 * off, nb, bs, st);
                 }
-                if ((rc = run_binset(bs, st))) { g_ws.open = false; return rc; }
+                if (!rc) rc = run_binset(w, bs, st);
+                if (rc) { w.open = false; return rc; }
             }
         }
-        if ((rc = do_end(cur, nxt, st))) return rc;
+        if ((rc = do_end(w, cur, nxt, nullptr, 0, st))) return rc;
         cur = nxt;
     }
-    (void)M;
     return JPET_OK;
 }
 
-int ensure_host_path(size_t stage_bytes) {
-    if (!g_ws.copy_stream) {
-        CUDA_TRY(cudaStreamCreateWithFlags(&g_ws.copy_stream, cudaStreamNonBlocking));
-        CUDA_TRY(cudaStreamCreateWithFlags(&g_ws.compute_stream, cudaStreamNonBlocking));
+int ensure_host_path(Workspace& w, size_t stage_bytes) {
+    if (!w.copy_stream) {
+        CUDA_TRY(cudaStreamCreateWithFlags(&w.copy_stream, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamCreateWithFlags(&w.compute_stream, cudaStreamNonBlocking));
         for (int i = 0; i < 2; ++i) {
-            CUDA_TRY(cudaEventCreateWithFlags(&g_ws.ev_copy[i], cudaEventDisableTiming));
-            CUDA_TRY(cudaEventCreateWithFlags(&g_ws.ev_done[i], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&w.ev_copy[i], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&w.ev_done[i], cudaEventDisableTiming));
         }
     }
-    if (stage_bytes > g_ws.cap_stage) {
-        cudaFree(g_ws.stage);
-        g_ws.stage = nullptr;
-        g_ws.cap_stage = 0;
-        CUDA_TRY(cudaMalloc(&g_ws.stage, stage_bytes));
-        g_ws.cap_stage = stage_bytes;
+    if (stage_bytes > w.cap_stage) {
+        cudaFree(w.stage);
+        w.stage = nullptr;
+        w.cap_stage = 0;
+        CUDA_TRY(cudaMalloc(&w.stage, stage_bytes));
+        w.cap_stage = stage_bytes;
     }
     return JPET_OK;
 }
 
-// One iteration's accumulate phase from host events.  resident_in: events already in stage[0..n).
-// If everything fits the staging buffer it is filled chunk by chunk (copy of chunk c+1 overlaps compute of chunk c)
-// and left resident; otherwise two chunk-sized slots are used as a ring.
-int accumulate_from_host(const float* events_host, int64_t n, int64_t chunk, bool fits, bool resident_in) {
-    cudaStream_t cs = g_ws.copy_stream, ks = g_ws.compute_stream;
-    if (resident_in) return do_accumulate(g_ws.stage, n, ks);
+// One iteration's accumulate phase from host events.  If everything fits the staging buffer it is filled chunk by chunk
+// (copy of chunk c+1 overlaps compute of chunk c) and left resident; otherwise two chunk-sized slots are used as a
+// ring: before a slot is overwritten the copy stream waits for the kernels that read its previous content - also across
+// iterations (slot_used lives in the workspace, not in this call).
+int accumulate_from_host(Workspace& w, const float* events_host, int64_t n, int64_t chunk, bool fits) {
+    cudaStream_t cs = w.copy_stream, ks = w.compute_stream;
     int c = 0;
     for (int64_t off = 0; off < n; off += chunk, ++c) {
         int64_t nb = std::min(chunk, n - off);
         int slot = c & 1;
-        float* dst = fits ? g_ws.stage + 3 * off : g_ws.stage + 3 * (int64_t)slot * chunk;
-        if (!fits && c >= 2) CUDA_TRY(cudaStreamWaitEvent(cs, g_ws.ev_done[slot], 0));   // slot free again
+        float* dst = fits ? w.stage + 3 * off : w.stage + 3 * (int64_t)slot * chunk;
+        if (!fits && w.slot_used[slot]) CUDA_TRY(cudaStreamWaitEvent(cs, w.ev_done[slot], 0));   // slot free again
         CUDA_TRY(cudaMemcpyAsync(dst, events_host + 3 * off, sizeof(float) * 3 * nb, cudaMemcpyHostToDevice, cs));
-        CUDA_TRY(cudaEventRecord(g_ws.ev_copy[slot], cs));
-        CUDA_TRY(cudaStreamWaitEvent(ks, g_ws.ev_copy[slot], 0));
-        int rc = do_accumulate(dst, nb, ks);
+        CUDA_TRY(cudaEventRecord(w.ev_copy[slot], cs));
+        CUDA_TRY(cudaStreamWaitEvent(ks, w.ev_copy[slot], 0));
+        int rc = do_accumulate(w, dst, nb, ks);
         if (rc) return rc;
-        if (!fits) CUDA_TRY(cudaEventRecord(g_ws.ev_done[slot], ks));
+        if (!fits) { CUDA_TRY(cudaEventRecord(w.ev_done[slot], ks)); w.slot_used[slot] = true; }
     }
     return JPET_OK;
 }
 
 int reconstruct_host_impl(const float* events_host, int64_t n, const jpet_geometry* g, const jpet_sigmas* sg,
-                          const jpet_grid* gr, const float* rho_init_host, float* rho_out_host, int32_t n_iter,
-                          int64_t chunk) {
+                          const jpet_grid* gr, const float* rho_init_host, float* rho_out_host, int32_t n_iter, int64_t chunk) {
     int rc = validate(g, sg, gr);
     if (rc) return rc;
     if (!sg) return fail(JPET_E_INVAL, "NULL sigmas");
     if (n < 0 || n_iter < 0) return fail(JPET_E_INVAL, "n < 0 or n_iter < 0");
     if ((n > 0 && !events_host) || !rho_out_host) return fail(JPET_E_INVAL, "NULL host pointer");
-    if ((rc = ensure_device())) return rc;
+    Workspace* wp = nullptr;
+    if ((rc = current_ws(&wp))) return rc;
+    Workspace& w = *wp;
     const int M = gr->n_y * gr->n_z;
-    if ((rc = ensure_images(M))) return rc;
+    if ((rc = ensure_images(w, M))) return rc;
     // upload chunk: a quarter of the events, between 5x10^5 and 2x10^6, so that the copy of chunk c+1 overlaps the sort
     // and the event kernel of chunk c also for one-batch problems (config 2 on a box with a 12 GB/s host link:
     // 1.6 ms with one chunk, 1.07 ms with two; no difference on a 50 GB/s link)
     if (chunk <= 0) chunk = std::min<int64_t>(2000000, std::max<int64_t>(500000, (n + 3) / 4));
     chunk = std::min<int64_t>(chunk, std::max<int64_t>(n, 1));
-    const bool fits = (int64_t)sizeof(float) * 3 * n <= kStageBytes;
+    const int64_t budget = g_opt.stage_bytes > 0 ? g_opt.stage_bytes : kStageDefault;
+    const bool fits = (int64_t)sizeof(float) * 3 * n <= budget;
     size_t stage_bytes = fits ? sizeof(float) * 3 * (size_t)std::max<int64_t>(n, 1) : sizeof(float) * 3 * 2 * (size_t)chunk;
-    if ((rc = ensure_host_path(stage_bytes))) return rc;
-    cudaStream_t ks = g_ws.compute_stream;
-    float* cur = g_ws.rho_a;
-    float* nxt = g_ws.rho_b;
+    if ((rc = ensure_host_path(w, stage_bytes))) return rc;
+    cudaStream_t ks = w.compute_stream;
+    if ((rc = enter(w, ks))) return rc;
+    w.slot_used[0] = w.slot_used[1] = false;       // nothing of an earlier call is in flight: every host call ends synchronised
+    float* cur = w.rho_a;
+    float* nxt = w.rho_b;
     if (rho_init_host) {
         CUDA_TRY(cudaMemcpyAsync(cur, rho_init_host, sizeof(float) * M, cudaMemcpyHostToDevice, ks));
     } else {
@@ -857,28 +712,46 @@ int reconstruct_host_impl(const float* events_host, int64_t n, const jpet_geomet
     }
     if (n_iter > 0) {
         // first iteration: the upload of chunk c+1 overlaps the binning + event kernels of chunk c
-        if ((rc = do_begin(g, sg, gr, cur, ks))) return rc;
-        if ((rc = accumulate_from_host(events_host, n, chunk, fits, false))) return rc;
-        if ((rc = do_end(cur, nxt, ks))) return rc;
+        if ((rc = do_begin(w, g, sg, gr, cur, ks))) return rc;
+        if ((rc = accumulate_from_host(w, events_host, n, chunk, fits))) return rc;
+        if ((rc = do_end(w, cur, nxt, nullptr, 0, ks))) return rc;
         std::swap(cur, nxt);
         if (n_iter > 1) {
             if (fits) {         // events are now resident in the staging buffer: bin once, iterate
-                if ((rc = iterate_many(g_ws.stage, n, g, sg, gr, cur, nxt, n_iter - 1, ks))) return rc;
+                if ((rc = iterate_many(w, w.stage, n, g, sg, gr, cur, nxt, n_iter - 1, ks))) return rc;
                 std::swap(cur, nxt);
             } else {
                 for (int it = 1; it < n_iter; ++it) {
-                    if ((rc = do_begin(g, sg, gr, cur, ks))) return rc;
-                    if ((rc = accumulate_from_host(events_host, n, chunk, false, false))) return rc;
-                    if ((rc = do_end(cur, nxt, ks))) return rc;
+                    if ((rc = do_begin(w, g, sg, gr, cur, ks))) return rc;
+                    if ((rc = accumulate_from_host(w, events_host, n, chunk, false))) return rc;
+                    if ((rc = do_end(w, cur, nxt, nullptr, 0, ks))) return rc;
                     std::swap(cur, nxt);
                 }
             }
         }
     }
     CUDA_TRY(cudaMemcpyAsync(rho_out_host, cur, sizeof(float) * M, cudaMemcpyDeviceToHost, ks));
+    if ((rc = leave(w, ks))) return rc;
     CUDA_TRY(cudaStreamSynchronize(ks));
-    CUDA_TRY(cudaStreamSynchronize(g_ws.copy_stream));
+    CUDA_TRY(cudaStreamSynchronize(w.copy_stream));
     return JPET_OK;
+}
+
+void release_ws(Workspace& w) {
+    cudaFree(w.s); cudaFree(w.wT); cudaFree(w.accT); cudaFree(w.rho_a); cudaFree(w.rho_b);
+    cudaFree(w.counters); cudaFree(w.stage); cudaFree(w.place); cudaFree(w.counts); cudaFree(w.kept_sorted);
+    cudaFree(w.tab);
+    free_binset(w.scratch);
+    for (auto& bs : w.kept) free_binset(bs);
+    for (int i = 0; i < 2; ++i) {
+        if (w.ev_copy[i]) cudaEventDestroy(w.ev_copy[i]);
+        if (w.ev_done[i]) cudaEventDestroy(w.ev_done[i]);
+    }
+    if (w.ev_last) cudaEventDestroy(w.ev_last);
+    for (cudaEvent_t e : w.tk)
+        if (e) cudaEventDestroy(e);
+    if (w.copy_stream) cudaStreamDestroy(w.copy_stream);
+    if (w.compute_stream) cudaStreamDestroy(w.compute_stream);
 }
 
 }  // namespace
@@ -902,17 +775,84 @@ int jpet_sensitivity(const jpet_geometry* geometry, const jpet_grid* grid, float
 int jpet_mlem_begin(const jpet_geometry* geometry, const jpet_sigmas* sigmas, const jpet_grid* grid,
                     const float* rho_in_dev, void* cuda_stream) {
     g_err.clear();
-    return do_begin(geometry, sigmas, grid, rho_in_dev, (cudaStream_t)cuda_stream);
+    int rc = validate(geometry, sigmas, grid);
+    if (rc) return rc;
+    Workspace* w = nullptr;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = current_ws(&w)) || (rc = enter(*w, st))) return rc;
+    if ((rc = do_begin(*w, geometry, sigmas, grid, rho_in_dev, st))) return rc;
+    return leave(*w, st);
 }
 
 int jpet_mlem_accumulate(const float* events_dev, int64_t n_batch, void* cuda_stream) {
     g_err.clear();
-    return do_accumulate(events_dev, n_batch, (cudaStream_t)cuda_stream);
+    Workspace* w = device_ws();
+    if (!w || !w->open) return fail(JPET_E_INVAL, "jpet_mlem_accumulate without jpet_mlem_begin");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = enter(*w, st);
+    if (rc) return rc;
+    if ((rc = do_accumulate(*w, events_dev, n_batch, st))) return rc;
+    return leave(*w, st);
 }
 
 int jpet_mlem_end(const float* rho_in_dev, float* rho_out_dev, void* cuda_stream) {
     g_err.clear();
-    return do_end(rho_in_dev, rho_out_dev, (cudaStream_t)cuda_stream);
+    Workspace* w = device_ws();
+    if (!w || !w->open) return fail(JPET_E_INVAL, "jpet_mlem_end without jpet_mlem_begin");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = enter(*w, st);
+    if (rc) return rc;
+    if ((rc = do_end(*w, rho_in_dev, rho_out_dev, nullptr, 0, st))) return rc;
+    return leave(*w, st);
+}
+
+int jpet_mlem_end_peers(const float* rho_in_dev, float* rho_out_dev, const float* const* peer_acc_dev, int32_t n_peers,
+                        void* cuda_stream) {
+    g_err.clear();
+    Workspace* w = device_ws();
+    if (!w || !w->open) return fail(JPET_E_INVAL, "jpet_mlem_end_peers without jpet_mlem_begin");
+    if (!peer_acc_dev) return fail(JPET_E_INVAL, "NULL peer list");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = enter(*w, st);
+    if (rc) return rc;
+    if ((rc = do_end(*w, rho_in_dev, rho_out_dev, peer_acc_dev, n_peers, st))) return rc;
+    return leave(*w, st);
+}
+
+int jpet_mlem_accumulator(float** acc_dev, int64_t* n_floats) {
+    g_err.clear();
+    Workspace* w = device_ws();
+    if (!w || !w->open) return fail(JPET_E_INVAL, "jpet_mlem_accumulator without an open iteration (jpet_mlem_begin)");
+    if (!acc_dev || !n_floats) return fail(JPET_E_INVAL, "NULL output pointer");
+    *acc_dev = w->accT;
+    *n_floats = w->M;
+    return JPET_OK;
+}
+
+int jpet_ipc_export(const void* dev_ptr, void* handle64_out) {
+    g_err.clear();
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "cudaIpcMemHandle_t is 64 bytes");
+    if (!dev_ptr || !handle64_out) return fail(JPET_E_INVAL, "NULL pointer");
+    cudaIpcMemHandle_t h;
+    CUDA_TRY(cudaIpcGetMemHandle(&h, const_cast<void*>(dev_ptr)));
+    memcpy(handle64_out, &h, sizeof h);
+    return JPET_OK;
+}
+
+int jpet_ipc_open(const void* handle64, void** dev_ptr_out) {
+    g_err.clear();
+    if (!handle64 || !dev_ptr_out) return fail(JPET_E_INVAL, "NULL pointer");
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle64, sizeof h);
+    CUDA_TRY(cudaIpcOpenMemHandle(dev_ptr_out, h, cudaIpcMemLazyEnablePeerAccess));
+    return JPET_OK;
+}
+
+int jpet_ipc_close(void* dev_ptr) {
+    g_err.clear();
+    if (!dev_ptr) return fail(JPET_E_INVAL, "NULL pointer");
+    CUDA_TRY(cudaIpcCloseMemHandle(dev_ptr));
+    return JPET_OK;
 }
 
 int jpet_mlem_iterate(const float* events_dev, int64_t n, const jpet_geometry* geometry, const jpet_sigmas* sigmas,
@@ -924,9 +864,12 @@ int jpet_mlem_iterate(const float* events_dev, int64_t n, const jpet_geometry* g
     if (n > 0 && !events_dev) return fail(JPET_E_INVAL, "NULL events");
     if (!rho_in_dev || !rho_out_dev) return fail(JPET_E_INVAL, "NULL image pointer");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if ((rc = do_begin(geometry, sigmas, grid, rho_in_dev, st))) return rc;
-    if ((rc = do_accumulate(events_dev, n, st))) { g_ws.open = false; return rc; }
-    return do_end(rho_in_dev, rho_out_dev, st);
+    Workspace* w = nullptr;
+    if ((rc = current_ws(&w)) || (rc = enter(*w, st))) return rc;
+    if ((rc = do_begin(*w, geometry, sigmas, grid, rho_in_dev, st))) return rc;
+    if ((rc = do_accumulate(*w, events_dev, n, st))) return rc;
+    if ((rc = do_end(*w, rho_in_dev, rho_out_dev, nullptr, 0, st))) return rc;
+    return leave(*w, st);
 }
 
 int jpet_reconstruct(const float* events_dev, int64_t n, const jpet_geometry* geometry, const jpet_sigmas* sigmas,
@@ -938,23 +881,25 @@ int jpet_reconstruct(const float* events_dev, int64_t n, const jpet_geometry* ge
     if (!sigmas) return fail(JPET_E_INVAL, "NULL sigmas");
     if (n < 0 || n_iter < 0) return fail(JPET_E_INVAL, "n < 0 or n_iter < 0");
     if ((n > 0 && !events_dev) || !rho_out_dev) return fail(JPET_E_INVAL, "NULL pointer");
-    if ((rc = ensure_device())) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    Workspace* w = nullptr;
+    if ((rc = current_ws(&w)) || (rc = enter(*w, st))) return rc;
     const int M = grid->n_y * grid->n_z;
-    if ((rc = ensure_images(M))) return rc;
+    if ((rc = ensure_images(*w, M))) return rc;
     // ping-pong through the workspace so that rho_out may alias rho_init and is written once per iteration
     const float* cur = rho_init_dev;
     if (!cur) {
-        jpet::ones_kernel<<<grid_for(M), 256, 0, st>>>(g_ws.rho_a, M);
+        jpet::ones_kernel<<<grid_for(M), 256, 0, st>>>(w->rho_a, M);
         g_launches++;
         CUDA_TRY(cudaGetLastError());
-        cur = g_ws.rho_a;
+        cur = w->rho_a;
     }
     if (n_iter == 0) {
         if (cur != rho_out_dev) CUDA_TRY(cudaMemcpyAsync(rho_out_dev, cur, sizeof(float) * M, cudaMemcpyDeviceToDevice, st));
-        return JPET_OK;
+        return leave(*w, st);
     }
-    return iterate_many(events_dev, n, geometry, sigmas, grid, cur, rho_out_dev, n_iter, st);
+    if ((rc = iterate_many(*w, events_dev, n, geometry, sigmas, grid, cur, rho_out_dev, n_iter, st))) return rc;
+    return leave(*w, st);
 }
 
 int jpet_mlem_iterate_host(const float* events_host, int64_t n, const jpet_geometry* geometry, const jpet_sigmas* sigmas,
@@ -973,12 +918,18 @@ int jpet_reconstruct_host(const float* events_host, int64_t n, const jpet_geomet
 
 int jpet_get_counters(uint64_t* n_evals_host, uint64_t* n_skipped_host, void* cuda_stream) {
     g_err.clear();
-    if (!g_ws.counters) return fail(JPET_E_INVAL, "no iteration has been run");
-    unsigned long long h[2];
-    CUDA_TRY(cudaMemcpyAsync(h, g_ws.counters, sizeof h, cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
-    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+    Workspace* w = device_ws();
+    if (!w || !w->counters) return fail(JPET_E_INVAL, "no iteration has been run");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = enter(*w, st);
+    if (rc) return rc;
+    unsigned long long h[3];
+    CUDA_TRY(cudaMemcpyAsync(h, w->counters, sizeof h, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
     if (n_evals_host) *n_evals_host = h[0];
     if (n_skipped_host) *n_skipped_host = h[1];
+    if (h[2]) return fail(JPET_E_INTERNAL, "the event kernel met %llu records it could not hold (piece longer than its register slot or "
+                          "row count outside the task table): the image of this iteration is incomplete", h[2]);
     return JPET_OK;
 }
 
@@ -989,22 +940,21 @@ int jpet_count_evals(const float* events_dev, int64_t n, const jpet_geometry* ge
     if (rc) return rc;
     if (!sigmas) return fail(JPET_E_INVAL, "NULL sigmas");
     if (n < 0 || (n > 0 && !events_dev)) return fail(JPET_E_INVAL, "bad events");
-    if ((rc = ensure_device())) return rc;
+    Workspace* w = nullptr;
+    if ((rc = current_ws(&w))) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     unsigned long long* d = nullptr;
     CUDA_TRY(cudaMalloc(&d, 2 * sizeof(unsigned long long)));
-    CUDA_TRY(cudaMemsetAsync(d, 0, 2 * sizeof(unsigned long long), st));
-    DevParams dp;
-    int variant = 0;
-    size_t smem = 0;
-    make_plan(*geometry, *sigmas, *grid, g_a3_coef, g_gamma, &dp, &variant, &smem);
-    if (n > 0) {
-        int blocks = (int)std::min<int64_t>((n + 255) / 256, (int64_t)g_ws.sm_count * 8);
-        jpet::count_evals_kernel<<<blocks, 256, 0, st>>>(events_dev, (long long)n, dp, d);
+    cudaError_t e = cudaMemsetAsync(d, 0, 2 * sizeof(unsigned long long), st);
+    jpet_host::RowsPlan plan;
+    make_plan(*geometry, *sigmas, *grid, &plan);
+    if (e == cudaSuccess && n > 0) {
+        int blocks = (int)std::min<int64_t>((n + 255) / 256, (int64_t)w->sm_count * 8);
+        jpet::count_evals_kernel<<<blocks, 256, 0, st>>>(events_dev, (long long)n, plan.dp, d);
         g_launches++;
     }
     unsigned long long h[2] = {0, 0};
-    cudaError_t e = cudaMemcpyAsync(h, d, sizeof h, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h, d, sizeof h, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     cudaFree(d);
     if (e != cudaSuccess) return fail(JPET_E_CUDA, "count_evals: %s", cudaGetErrorString(e));
@@ -1013,50 +963,153 @@ int jpet_count_evals(const float* events_dev, int64_t n, const jpet_geometry* ge
     return JPET_OK;
 }
 
-int jpet_set_a3_coef(float k) {
+int jpet_direct_histogram(const float* events_dev, int64_t n, const jpet_geometry* geometry, const jpet_grid* grid,
+                          uint32_t* hist_dev, uint64_t* n_outside_host, void* cuda_stream) {
     g_err.clear();
-    if (!std::isfinite(k)) return fail(JPET_E_INVAL, "a3 coefficient must be finite");
-    g_a3_coef = k;
+    int rc = validate(geometry, nullptr, grid);
+    if (rc) return rc;
+    if (n < 0 || (n > 0 && !events_dev)) return fail(JPET_E_INVAL, "bad events");
+    if (n > 0x7fffffffll) return fail(JPET_E_INVAL, "at most 2^31 - 1 events per call");
+    if (!hist_dev) return fail(JPET_E_INVAL, "NULL hist_dev");
+    Workspace* w = nullptr;
+    if ((rc = current_ws(&w))) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = enter(*w, st))) return rc;
+    if (!w->counters) CUDA_TRY(cudaMalloc(&w->counters, 4 * sizeof(unsigned long long)));
+    CUDA_TRY(cudaMemsetAsync(w->counters + 3, 0, sizeof(unsigned long long), st));
+    jpet::HistParams h;
+    h.n_y = grid->n_y; h.n_z = grid->n_z;
+    h.inv2R = (float)(1.0 / (2.0 * (double)geometry->R));
+    h.inv_px = (float)(1.0 / (double)grid->pixel);
+    h.oy = (float)(0.5 * (grid->n_y - 1) + 0.5);
+    h.oz = (float)(0.5 * (grid->n_z - 1) + 0.5);
+    if (n > 0) {
+        const int M = grid->n_y * grid->n_z;
+        const int use_smem = M <= jpet::kHistSmemMax;
+        const size_t smem = kTileBytes + (use_smem ? sizeof(unsigned int) * (size_t)M : 0);
+        const int tiles = (int)((n + jpet::kBinTile - 1) / jpet::kBinTile);
+        // shared-memory histograms: a persistent grid (one flush per block); global atomics: one tile per block
+        const int blocks = use_smem ? std::min(tiles, w->sm_count * 4) : tiles;
+        jpet::direct_histogram_kernel<<<blocks, jpet::kBinBlock, smem, st>>>(events_dev, (int)n, h, hist_dev, w->counters + 3, use_smem);
+        g_launches++;
+        CUDA_TRY(cudaGetLastError());
+    }
+    if ((rc = leave(*w, st))) return rc;
+    if (n_outside_host) {
+        unsigned long long out = 0;
+        CUDA_TRY(cudaMemcpyAsync(&out, w->counters + 3, sizeof out, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        *n_outside_host = out;
+    }
     return JPET_OK;
 }
 
-float jpet_get_a3_coef(void) { return g_a3_coef; }
+int jpet_generate_events(const jpet_primitive* phantom_host, int32_t n_primitives, int64_t n, int64_t first,
+                         const jpet_geometry* geometry, const jpet_sigmas* sigmas, uint64_t seed, float* events_dev,
+                         void* cuda_stream) {
+    g_err.clear();
+    if (!geometry || !sigmas) return fail(JPET_E_INVAL, "NULL geometry or sigmas");
+    if (!(geometry->R > 0.f) || !(geometry->L > 0.f) || !std::isfinite(geometry->R) || !std::isfinite(geometry->L))
+        return fail(JPET_E_INVAL, "R and L must be positive and finite");
+    if (!(sigmas->sigma_z >= 0.f) || !(sigmas->sigma_dl >= 0.f) || !std::isfinite(sigmas->sigma_z) || !std::isfinite(sigmas->sigma_dl))
+        return fail(JPET_E_INVAL, "sigmas must be non-negative and finite");
+    if (!phantom_host || n_primitives < 1 || n_primitives > jpet::kMaxPrimitives)
+        return fail(JPET_E_INVAL, "the phantom must hold 1 .. %d primitives", jpet::kMaxPrimitives);
+    if (n < 0 || first < 0 || (n > 0 && !events_dev)) return fail(JPET_E_INVAL, "bad n, first or events_dev");
+    jpet::PhantomDev ph{};
+    ph.n = n_primitives;
+    double y0 = 1e300, y1 = -1e300, z0 = 1e300, z1 = -1e300, rho_max = 0.0;
+    for (int k = 0; k < n_primitives; ++k) {
+        const jpet_primitive& q = phantom_host[k];
+        if ((q.kind != 0 && q.kind != 1) || !(q.hy > 0.f) || !(q.hz > 0.f) || !(q.intensity >= 0.f) || !std::isfinite(q.cy) ||
+            !std::isfinite(q.cz) || !std::isfinite(q.hy) || !std::isfinite(q.hz) || !std::isfinite(q.phi_deg) || !std::isfinite(q.intensity))
+            return fail(JPET_E_INVAL, "primitive %d: kind must be 0 or 1, half sizes positive, intensity >= 0, all finite", k);
+        const double phi = (double)q.phi_deg * 3.14159265358979323846 / 180.0, c = std::cos(phi), s = std::sin(phi);
+        double ey, ez;
+        if (q.kind == 0) { ez = std::hypot(q.hz * c, q.hy * s); ey = std::hypot(q.hz * s, q.hy * c); }
+        else { ez = q.hz * std::fabs(c) + q.hy * std::fabs(s); ey = q.hz * std::fabs(s) + q.hy * std::fabs(c); }
+        y0 = std::min(y0, q.cy - ey); y1 = std::max(y1, q.cy + ey);
+        z0 = std::min(z0, q.cz - ez); z1 = std::max(z1, q.cz + ez);
+        rho_max = std::max(rho_max, (double)q.intensity);
+        ph.kind[k] = q.kind; ph.cy[k] = q.cy; ph.cz[k] = q.cz;
+        ph.inv_hy[k] = (float)(1.0 / q.hy); ph.inv_hz[k] = (float)(1.0 / q.hz);
+        ph.cphi[k] = (float)c; ph.sphi[k] = (float)s;
+    }
+    if (!(rho_max > 0.0)) return fail(JPET_E_INVAL, "the phantom has no primitive with positive intensity");
+    for (int k = 0; k < n_primitives; ++k) ph.rel[k] = (float)(phantom_host[k].intensity / rho_max);
+    ph.y0 = (float)y0; ph.y1 = (float)y1; ph.z0 = (float)z0; ph.z1 = (float)z1;
+    ph.R = geometry->R; ph.half_L = 0.5f * geometry->L; ph.sigma_z = sigmas->sigma_z; ph.sigma_dl = sigmas->sigma_dl;
+    if (n == 0) return JPET_OK;
+    Workspace* w = nullptr;
+    int rc = current_ws(&w);
+    if (rc) return rc;
+    const int blocks = (int)std::min<int64_t>((n + 255) / 256, (int64_t)w->sm_count * 16);
+    jpet::generate_events_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>(events_dev, (long long)n, (unsigned long long)first,
+                                                                              (unsigned long long)seed, ph);
+    g_launches++;
+    CUDA_TRY(cudaGetLastError());
+    return JPET_OK;
+}
+
+int jpet_set_a3_coef(float k) {
+    g_err.clear();
+    if (!std::isfinite(k)) return fail(JPET_E_INVAL, "a3 coefficient must be finite");
+    g_opt.a3_coef = k;
+    return JPET_OK;
+}
+
+float jpet_get_a3_coef(void) { return g_opt.a3_coef; }
 
 int jpet_set_gamma(float gamma) {
     g_err.clear();
     if (!std::isfinite(gamma)) return fail(JPET_E_INVAL, "gamma must be finite");
-    g_gamma = gamma;
+    g_opt.gamma = gamma;
     return JPET_OK;
 }
 
-float jpet_get_gamma(void) { return g_gamma; }
+float jpet_get_gamma(void) { return g_opt.gamma; }
+
+int jpet_set_sigma_z_edge(float eta) {
+    g_err.clear();
+    if (!(eta >= 0.f && eta <= 1.f)) return fail(JPET_E_INVAL, "the sigma_z edge coefficient must lie in [0, 1]");
+    g_opt.sz_eta = eta;
+    return JPET_OK;
+}
+
+float jpet_get_sigma_z_edge(void) { return g_opt.sz_eta; }
 
 int jpet_set_option(const char* name, int64_t value) {
     g_err.clear();
     if (!name) return fail(JPET_E_INVAL, "NULL option name");
     if (!strcmp(name, "force_direct")) {
         if (value < 0 || value > 1) return fail(JPET_E_INVAL, "force_direct must be 0 or 1");
-        g_opt_force_direct = value;
+        g_opt.force_direct = value;
     } else if (!strcmp(name, "time_kernel")) {
         if (value < 0 || value > 1) return fail(JPET_E_INVAL, "time_kernel must be 0 or 1");
-        g_opt_time_kernel = value;
-        g_tk_used = 0;
+        g_opt.time_kernel = value;
+        for (auto& kv : g_ctx) kv.second->tk_used = 0;
     } else if (!strcmp(name, "sub_tile_z")) {
         if (value < 0 || value > 256) return fail(JPET_E_INVAL, "sub_tile_z must be 0 (auto) .. 256");
-        g_opt_sz = value;
+        g_opt.sz = value;
     } else if (!strcmp(name, "chunk")) {
         if (value < 0 || value > (1 << 20)) return fail(JPET_E_INVAL, "chunk must be 0 (auto) .. 2^20");
-        g_opt_chunk = value;
+        g_opt.chunk = value;
     } else if (!strcmp(name, "variant")) {
-        if (value < -1 || value >= kNumVariants) return fail(JPET_E_INVAL, "variant must be -1 (auto) .. %d", kNumVariants - 1);
-        g_opt_variant = value;
+        if (value < -1 || value >= kNumShapes) return fail(JPET_E_INVAL, "variant must be -1 (auto) .. %d", kNumShapes - 1);
+        g_opt.variant = value;
     } else if (!strcmp(name, "poly_off")) {
-        g_opt_poly_off = value != 0;
+        g_opt.poly_off = value != 0;
     } else if (!strcmp(name, "pdl")) {
-        g_opt_pdl = value != 0;
+        g_opt.pdl = value != 0;
     } else if (!strcmp(name, "ctas_per_sm")) {
         if (value < 0 || value > 32) return fail(JPET_E_INVAL, "ctas_per_sm must be 0 (auto) .. 32");
-        g_opt_ctas_per_sm = value;
+        g_opt.ctas_per_sm = value;
+    } else if (!strcmp(name, "stage_bytes")) {
+        if (value < 0) return fail(JPET_E_INVAL, "stage_bytes must be >= 0 (0 = default)");
+        g_opt.stage_bytes = value;
+    } else if (!strcmp(name, "exact_kernel")) {
+        if (value < 0 || value > 4096) return fail(JPET_E_INVAL, "exact_kernel must be 0 (off) .. 4096 quadrature nodes");
+        g_opt.exact_kernel = value;
     } else {
         return fail(JPET_E_INVAL, "unknown option '%s'", name);
     }
@@ -1065,31 +1118,35 @@ int jpet_set_option(const char* name, int64_t value) {
 
 int64_t jpet_get_option(const char* name) {
     if (!name) return -1;
-    if (!strcmp(name, "force_direct")) return g_opt_force_direct;
-    if (!strcmp(name, "chunk")) return g_opt_chunk;
-    if (!strcmp(name, "sub_tile_z")) return g_opt_sz;
-    if (!strcmp(name, "time_kernel")) return g_opt_time_kernel;
+    if (!strcmp(name, "force_direct")) return g_opt.force_direct;
+    if (!strcmp(name, "chunk")) return g_opt.chunk;
+    if (!strcmp(name, "sub_tile_z")) return g_opt.sz;
+    if (!strcmp(name, "time_kernel")) return g_opt.time_kernel;
+    if (!strcmp(name, "variant")) return g_opt.variant;
+    if (!strcmp(name, "poly_off")) return g_opt.poly_off;
+    if (!strcmp(name, "pdl")) return g_opt.pdl;
+    if (!strcmp(name, "ctas_per_sm")) return g_opt.ctas_per_sm;
+    if (!strcmp(name, "stage_bytes")) return g_opt.stage_bytes;
+    if (!strcmp(name, "exact_kernel")) return g_opt.exact_kernel;
+    Workspace* w = last_ws();
+    if (!w) return -1;
     if (!strcmp(name, "last_kernel_ns")) {      // summed duration of the tiled event-kernel launches of the last iteration
-        if (g_tk_used == 0) return -1;          // (one launch per batch of events; synchronises on the last one)
+        if (w->tk_used == 0) return -1;         // (one launch per batch of events; synchronises on the last one)
         double total = 0.0;
-        for (size_t i = 0; i + 1 < g_tk_used; i += 2) {
+        for (size_t i = 0; i + 1 < w->tk_used; i += 2) {
             float ms = 0.f;
-            if (cudaEventSynchronize(g_tk[i + 1]) != cudaSuccess || cudaEventElapsedTime(&ms, g_tk[i], g_tk[i + 1]) != cudaSuccess) return -1;
+            if (cudaEventSynchronize(w->tk[i + 1]) != cudaSuccess || cudaEventElapsedTime(&ms, w->tk[i], w->tk[i + 1]) != cudaSuccess) return -1;
             total += ms;
         }
         return (int64_t)(total * 1e6);
     }
-    if (!strcmp(name, "last_kernel_launches")) return (int64_t)(g_tk_used / 2);
-    if (!strcmp(name, "variant")) return g_opt_variant;
-    if (!strcmp(name, "poly_off")) return g_opt_poly_off;
-    if (!strcmp(name, "pdl")) return g_opt_pdl;
-    if (!strcmp(name, "ctas_per_sm")) return g_opt_ctas_per_sm;
-    if (!strcmp(name, "last_variant")) return g_ws.variant;
-    if (!strcmp(name, "last_smem_bytes")) return (int64_t)g_ws.smem;
-    if (!strcmp(name, "last_tiled")) return g_ws.dp.t_max >= 0.f;
-    if (!strcmp(name, "last_overflow")) {       // pieces that exceeded their slot (0 by construction; synchronises the device)
+    if (!strcmp(name, "last_kernel_launches")) return (int64_t)(w->tk_used / 2);
+    if (!strcmp(name, "last_variant")) return w->plan.shape;
+    if (!strcmp(name, "last_smem_bytes")) return (int64_t)w->plan.smem;
+    if (!strcmp(name, "last_tiled")) return w->plan.dp.t_max >= 0.f;
+    if (!strcmp(name, "last_overflow")) {       // records the event kernel could not hold (0 by construction; synchronises the device)
         unsigned long long h = 0;
-        if (!g_ws.counters || cudaMemcpy(&h, g_ws.counters + 2, sizeof h, cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+        if (!w->counters || cudaMemcpy(&h, w->counters + 2, sizeof h, cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
         return (int64_t)h;
     }
     return -1;
@@ -1098,22 +1155,13 @@ int64_t jpet_get_option(const char* name) {
 uint64_t jpet_launch_count(void) { return g_launches.load(); }
 
 void jpet_release(void) {
-    cudaFree(g_ws.s); cudaFree(g_ws.wT); cudaFree(g_ws.accT); cudaFree(g_ws.rho_a); cudaFree(g_ws.rho_b);
-    cudaFree(g_ws.counters); cudaFree(g_ws.stage); cudaFree(g_ws.bin_of); cudaFree(g_ws.counts); cudaFree(g_ws.kept_sorted);
-    g_ws.counts_clean_nb = -1;
-    cudaFree(g_ws.tab);
-    free_binset(g_ws.scratch);
-    for (auto& bs : g_ws.kept) free_binset(bs);
-    for (int i = 0; i < 2; ++i) {
-        if (g_ws.ev_copy[i]) cudaEventDestroy(g_ws.ev_copy[i]);
-        if (g_ws.ev_done[i]) cudaEventDestroy(g_ws.ev_done[i]);
+    int cur = -1;
+    cudaGetDevice(&cur);
+    for (auto& kv : g_ctx) {
+        if (cudaSetDevice(kv.first) == cudaSuccess) release_ws(*kv.second);
     }
-    if (g_ws.copy_stream) cudaStreamDestroy(g_ws.copy_stream);
-    if (g_ws.compute_stream) cudaStreamDestroy(g_ws.compute_stream);
-    int dev = g_ws.device, sms = g_ws.sm_count;
-    g_ws = Workspace{};
-    g_ws.device = dev;
-    g_ws.sm_count = sms;
+    g_ctx.clear();
+    if (cur >= 0) cudaSetDevice(cur);
 }
 
 const char* jpet_last_error(void) { return g_err.c_str(); }
@@ -1125,21 +1173,21 @@ int64_t jpet_plan_describe(const jpet_geometry* geometry, const jpet_sigmas* sig
     if (rc) return rc;
     if (!sigmas) return fail(JPET_E_INVAL, "NULL sigmas");
     if (!out || n_out < 17) return fail(JPET_E_INVAL, "out must hold at least 17 values");
-    DevParams dp;
-    int variant = 0;
-    size_t smem = 0;
+    jpet_host::RowsPlan plan;
     std::vector<uint32_t> tab;
-    make_plan(*geometry, *sigmas, *grid, g_a3_coef, g_gamma, &dp, &variant, &smem, &tab);
-    const bool gen3 = variant >= kNumVariants2;
-    const Variant3 v3 = gen3 ? kVariants3[variant - kNumVariants2] : Variant3{0, 0, 0, 0, 0, 0, 0, 0};
-    const int64_t vals[17] = {variant, gen3 ? v3.DEG : 0, gen3 ? v3.NWE : 0, gen3 ? v3.NG : 0, gen3 ? v3.NJA : 0,
-                              gen3 ? v3.NJB : 0, dp.HS, dp.WZ, dp.Sy, dp.Sz, dp.Hy, dp.Hz, dp.chunk, (int64_t)smem,
-                              dp.t_max >= 0.f, dp.nr_min, dp.nr_max};
+    make_plan(*geometry, *sigmas, *grid, &plan, &tab);
+    const DevParams& dp = plan.dp;
+    const bool tiled = dp.t_max >= 0.f;
+    const Shape v = tiled ? kShapes[plan.shape] : Shape{"none", 0, 0, 0, 0, 0, 0, 0, 0};
+    const int64_t vals[17] = {plan.shape, v.DEG, v.NWE, v.NG, v.NJA, v.NJB, dp.HS, dp.WZ, dp.Sy, dp.Sz, dp.Hy, dp.Hz, dp.chunk,
+                              (int64_t)plan.smem, tiled, dp.nr_min, dp.nr_max};
     for (int i = 0; i < 17; ++i) out[i] = vals[i];
     if (task_table_host)
         for (int64_t i = 0; i < std::min<int64_t>(table_cap, (int64_t)tab.size()); ++i) task_table_host[i] = tab[(size_t)i];
     return (int64_t)tab.size();
 }
+
+const char* jpet_shape_name(int32_t shape) { return shape >= 0 && shape < kNumShapes ? kShapes[shape].name : ""; }
 
 int jpet_abi_version(void) { return JPET_ABI_VERSION; }
 

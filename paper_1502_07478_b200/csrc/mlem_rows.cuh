@@ -1,31 +1,37 @@
-// mlem_rows3.cuh - third-generation event kernel of the list-mode MLEM hot path (sm_100a).
+// mlem_rows.cuh - the tiled event kernel of the list-mode MLEM hot path (sm_100a): steps 1-3 of an iteration for the
+// events of the regular bins - ellipse rows and spans (App. B :251-267), the kernel of Eq. 7-12
+// with the denominator of Eq. 3, and the back-projection (Listing 1 line 10).
 //
-// Same mathematics, the same sorted 64-byte event records and the same tiling as mlem_rows2_kernel (events sorted
-// by image sub-tile, w = s*rho region and private accumulator regions in shared memory, LANE <-> ELLIPSE ROW,
-// kernel values cached in registers between the denominator pass and the back-projection pass).  ncu on the
-// second generation showed the bound to be issue slots spent outside the per-pixel arithmetic: 772 warp
-// instructions per config-2 event of which about 320 are the two pixel passes; the rest is the lane -> row map,
-// row set-up repeated by two warps, the CTA barrier of the denominator and region staging.  Changes:
-//
-//   * an event is handled by a GROUP of NWE warps (1 for ellipses of up to 64 rows), several groups per CTA
-//     share one staged w region and own one accumulator region each; with NWE = 1 the event loop has no
-//     barrier at all (the denominator is a warp shuffle reduction);
+// Design (B200, not the paper's warp-per-event / texture scheme):
+//   * events are pre-sorted by image sub-tile (sort_kernels.cuh) and carry a 64-byte record of per-event constants; a
+//     CTA takes a work item (sub-tile, chunk of events), stages the w = s*rho region (sub-tile + halo) in shared
+//     memory, accumulates P / denominator into PRIVATE shared-memory regions with plain (non-atomic) read-modify-
+//     writes, and flushes them once with red.global.add.f32 (measured: global red.add tops out at ~2.8e10 warp
+//     requests/s, a factor 5-10 below what the SFU/FP32 pipes produce, so the scatter has to stay on chip);
+//   * regions are stored transposed (y fastest, row stride HS a multiple of 32): lanes are consecutive image rows, so
+//     whole-row pieces of a warp never share a bank whatever the ellipse tilt (split cap rows do: see piece B);
+//   * an event is handled by a GROUP of NWE warps (1 for ellipses of up to 64 rows), several groups per CTA share one
+//     staged w region and own one accumulator region each; with NWE = 1 the event loop has no barrier at all (the
+//     denominator is a warp shuffle reduction);
 //   * every lane owns up to two PIECES of ellipse rows per event: piece A, a whole row of the central block
 //     (capacity NJA pixels), and piece B, a row or a half / quarter of a row of the caps (capacity NJB).  Which
 //     (row, part) a lane takes is read from a table indexed by the number of rows of the ellipse, built on
 //     the host from the ellipse geometry (task_table.h) and kept in shared memory - no index arithmetic;
-//   * the row constants of the two pieces are evaluated together in packed fp32x2 arithmetic;
-//   * pixel walks are nested (each block of pixels is entered only if the previous one was), pairs of pixels
-//     per fp32x2 operation, warp-uniform bounds from redux; the ragged ends of the rows are masked per pair;
+//   * the row constants of the two pieces are evaluated together in packed fp32x2 arithmetic; the kernel values of a
+//     piece stay in registers between the denominator pass and the back-projection pass;
+//   * pixel walks are cut into blocks of BW pixels entered through one warp-uniform switch, pairs of pixels per fp32x2
+//     operation; the ragged ends of the rows are masked per pixel;
 //   * DEG > 0: the exponent of Eq. 7 as a degree-DEG polynomial in u along a piece (poly_coeffs2): one ex2 per kernel
-//     value instead of rsqrt + ex2, the Horner steps of all pairs of a block (BW = 16 pixels: 8 chains) in lockstep;
+//     value instead of rsqrt + ex2, the Horner steps of all pairs of a block in lockstep;
 //   * the back-projection pass issues its shared-memory read-modify-writes eight at a time; when every lane of a
 //     one-warp group owns at least 8 pixels of its central row, the first 8 run without masks and predicates;
+//   * VS: sigma_z depends on the hit positions (common.cuh): the Gaussian coefficient GS and the chord H0p / GS are
+//     per event;
 //   * every kernel of an iteration starts with pdl_wait() and is launched with programmatic stream serialisation.
 //
 // Citations are /root/reference/PAPER.md lines.  Nothing here is shared with oracle/.
 #pragma once
-#include "mlem_rows2.cuh"
+#include "common.cuh"
 
 namespace jpet {
 
@@ -40,6 +46,7 @@ struct Piece {
     RowWalk rc;          // rc.lo / rc.len: first column and pixel count of the piece
     uint32_t off;        // byte offset of its first pixel inside a region
     float c[6];          // DEG > 0: log2 P = c[0] + c[1] v + ... + c[DEG] v^DEG along the piece (see poly_coeffs2)
+    float ngs;           // DEG = 0: -GS, the coefficient of the Gaussian term (-1 for a constant sigma_z)
 };
 
 __device__ __forceinline__ float rcp_approx(float x) {
@@ -53,7 +60,7 @@ __device__ __forceinline__ float lg2_approx(float x) {
     return y;
 }
 
-// One MUFU per kernel value instead of two.  Along a row (v = scaled u, mlem_kernels.cuh) Eq. 7 reads
+// One MUFU per kernel value instead of two.  Along a row (v = scaled u, common.cuh) Eq. 7 reads
 //     log2 P = c2s - v^2 + ba(v)^2 / D(v) - 1/2 log2 D(v),     ba = alphas v + betas,   D = delta + eps v,
 // and x = eps v / delta is small inside the 3-sigma ellipse: |x| <= 2 |t| |y| |u| / (sec^2 (R^2 + y^2)), a few
 // per cent at most (the host plan bounds it and picks DEG, or falls back to DEG = 0, the closed form).  With
@@ -63,8 +70,9 @@ __device__ __forceinline__ float lg2_approx(float x) {
 //     -1/2 log2 D = -1/2 log2 delta - LH (kappa v - kappa^2 v^2 / 2 + kappa^3 v^3 / 3 - ...),   LH = log2(e) / 2.
 // The series is cut after v^DEG; the neglected terms are bounded by (ba^2/D) |x|^(DEG-1) + |x|^(DEG+1).
 // Two pieces (A in the low half, B in the high half) at a time.
+// NGS = -GS: coefficient of the Gaussian term (-1 for a constant sigma_z).
 template <int DEG>
-__device__ __forceinline__ void poly_coeffs2(f32x2 C2S, f32x2 BET, f32x2 ALP, f32x2 EPS, f32x2 DEL, f32x2 (&C)[6]) {
+__device__ __forceinline__ void poly_coeffs2(f32x2 C2S, f32x2 BET, f32x2 ALP, f32x2 EPS, f32x2 DEL, float NGS, f32x2 (&C)[6]) {
     float d0, d1;
     unpack2(DEL, d0, d1);
     const f32x2 G = pack2(rcp_approx(d0), rcp_approx(d1));
@@ -82,7 +90,7 @@ __device__ __forceinline__ void poly_coeffs2(f32x2 C2S, f32x2 BET, f32x2 ALP, f3
     for (int n = 3; n <= DEG; ++n) E[n] = mul2(NK, E[n - 1]);
     C[0] = fma2(L2, bc2(-0.5f), add2(C2S, E[0]));
     C[1] = fma2(K[1], bc2(kLH), E[1]);                                  // -LH kappa
-    C[2] = fma2(K[2], bc2(0.5f * kLH), add2(E[2], bc2(-1.f)));          // +LH kappa^2 / 2, and the Gaussian -v^2
+    C[2] = fma2(K[2], bc2(0.5f * kLH), add2(E[2], bc2(NGS)));           // +LH kappa^2 / 2, and the Gaussian -GS v^2
 #pragma unroll
     for (int n = 3; n <= DEG; ++n) C[n] = fma2(K[n], bc2(kLH / (float)n), E[n]);      // (-1)^n LH kappa^n / n
 }
@@ -112,12 +120,14 @@ __device__ __forceinline__ void piece_span(uint32_t te, int iy, float hw2, float
     pc.off = 4u * (uint32_t)((lo - rz0) * HS + (iy - ry0));
 }
 
-// Row constants of pieces A and B (polynomials in dy, see mlem_rows2.cuh) in packed arithmetic, then their spans.
-template <int NJA, int NJB, int HS, int DEG>
+// Row constants of pieces A and B (polynomials in dy, see EventRec in common.cuh) in packed arithmetic, then their spans.
+template <int NJA, int NJB, int HS, int DEG, bool VS>
 __device__ __forceinline__ void pieces_setup(uint32_t te, const float4 r0, const float4 r1, const float4 r2,
                                              const float4 r3, const DevParams& p, int ry0, int rz0, int col_lo, int col_hi,
                                              Piece& A, Piece& B, int& overflow) {
-    const int iy0 = __float_as_int(r3.z);
+    const int iy0 = rows_first(__float_as_int(r3.w));
+    const float ngs = VS ? -r3.z : -1.f;                               // -GS
+    const float H0e = VS ? p.H0p * rcp_approx(r3.z) : p.H0p;            // half chord^2 at the centre row [px^2]
     const uint32_t teA = te, teB = te >> 16;
     const int iyA = iy0 + (int)(teA & 0xffu), iyB = iy0 + (int)(teB & 0xffu);
     if constexpr (NJB > 0) {
@@ -128,7 +138,7 @@ __device__ __forceinline__ void pieces_setup(uint32_t te, const float4 r0, const
         const f32x2 ALP = fma2(bc2(r1.y), DY, bc2(r1.x));
         const f32x2 EPS = fma2(bc2(r1.w), DY, bc2(r1.z));
         const f32x2 DEL = fma2(DY, fma2(bc2(r2.z), DY, bc2(r2.y)), bc2(r2.x));
-        const f32x2 HW2 = fma2(bc2(r2.w), DY2, bc2(p.H0p));
+        const f32x2 HW2 = fma2(bc2(r2.w), DY2, bc2(H0e));
         const f32x2 ZCP = fma2(bc2(r3.y), DY, bc2(r3.x));
         float hwA, hwB, zcA, zcB;
         unpack2(C2S, A.rc.c2s, B.rc.c2s);
@@ -138,9 +148,10 @@ __device__ __forceinline__ void pieces_setup(uint32_t te, const float4 r0, const
         unpack2(DEL, A.rc.delta, B.rc.delta);
         unpack2(HW2, hwA, hwB);
         unpack2(ZCP, zcA, zcB);
+        A.ngs = B.ngs = ngs;
         if constexpr (DEG > 0) {
             f32x2 C[6];
-            poly_coeffs2<DEG>(C2S, BET, ALP, EPS, DEL, C);
+            poly_coeffs2<DEG>(C2S, BET, ALP, EPS, DEL, ngs, C);
 #pragma unroll
             for (int n = 0; n <= DEG; ++n) unpack2(C[n], A.c[n], B.c[n]);
         }
@@ -154,27 +165,28 @@ __device__ __forceinline__ void pieces_setup(uint32_t te, const float4 r0, const
         A.rc.alphas = fmaf(r1.y, dy, r1.x);
         A.rc.eps = fmaf(r1.w, dy, r1.z);
         A.rc.delta = fmaf(dy, fmaf(r2.z, dy, r2.y), r2.x);
+        A.ngs = ngs;
         if constexpr (DEG > 0) {
             f32x2 C[6];
-            poly_coeffs2<DEG>(bc2(A.rc.c2s), bc2(A.rc.betas), bc2(A.rc.alphas), bc2(A.rc.eps), bc2(A.rc.delta), C);
+            poly_coeffs2<DEG>(bc2(A.rc.c2s), bc2(A.rc.betas), bc2(A.rc.alphas), bc2(A.rc.eps), bc2(A.rc.delta), ngs, C);
             float dummy;
 #pragma unroll
             for (int n = 0; n <= DEG; ++n) unpack2(C[n], A.c[n], dummy);
         }
-        piece_span<NJA, HS, false>(teA, iyA, fmaf(r2.w, dy2, p.H0p), fmaf(r3.y, dy, r3.x), p.pxs, p, ry0, rz0, col_lo, col_hi, A, overflow);
+        piece_span<NJA, HS, false>(teA, iyA, fmaf(r2.w, dy2, H0e), fmaf(r3.y, dy, r3.x), p.pxs, p, ry0, rz0, col_lo, col_hi, A, overflow);
     }
 }
 
 // State of one pixel walk (pass 1): packed row constants, running u' pair and denominator pair.
 struct Walk {
-    f32x2 EPS2, DEL2, ALP2, BET2, C2S2, STEP2, V2, DEN2;
+    f32x2 EPS2, DEL2, ALP2, BET2, C2S2, NGS2, STEP2, V2, DEN2;
     f32x2 C[6];          // DEG > 0: broadcast polynomial coefficients (EPS2 ... C2S2 unused)
     uint32_t wa;
     int len;
 };
 
 // Two adjacent pixels j, j+1 of the piece: Eq. 7 (up to the constant K) and the denominator term.
-template <int J, int HS, bool MASK, int DEG>
+template <int J, int HS, bool MASK, int DEG, bool VS>
 __device__ __forceinline__ void walk_pair(Walk& s, float& p0, float& p1) {
     if constexpr (DEG > 0) {
         f32x2 E2 = fma2(s.C[DEG], s.V2, s.C[DEG - 1]);
@@ -198,7 +210,9 @@ __device__ __forceinline__ void walk_pair(Walk& s, float& p0, float& p1) {
     unpack2(D2, d0, d1);
     const f32x2 RS2 = pack2(rsqrt_approx(d0), rsqrt_approx(d1));
     const f32x2 BAR2 = mul2(BA2, RS2);
-    const f32x2 E2 = fma2(add2(BAR2, s.V2), sub2(BAR2, s.V2), s.C2S2);     // c2s - v^2 + bar^2
+    f32x2 E2;
+    if constexpr (VS) E2 = fma2(mul2(s.NGS2, s.V2), s.V2, fma2(BAR2, BAR2, s.C2S2));     // c2s - GS v^2 + bar^2
+    else E2 = fma2(add2(BAR2, s.V2), sub2(BAR2, s.V2), s.C2S2);                           // c2s - v^2 + bar^2
     float e0, e1;
     unpack2(E2, e0, e1);
     float x0 = ex2_approx(e0), x1 = ex2_approx(e1);
@@ -261,7 +275,7 @@ __device__ __forceinline__ void walk_block_lockstep(Walk& s, float u0s, float px
     if constexpr (NPAIR > 1) s.DEN2 = add2(s.DEN2, DENB);
 }
 
-template <int JB, int NJ, int HS, int DEG, int BW, int NFULL = 0>
+template <int JB, int NJ, int HS, int DEG, int BW, bool VS, int NFULL = 0>
 __device__ __forceinline__ void walk_block(Walk& s, float u0s, float pxs, float (&preg)[NJ]) {
     if constexpr (DEG > 0) {
         if constexpr (JB < NJ) walk_block_lockstep<JB, NJ, HS, DEG, BW, NFULL>(s, u0s, pxs, preg);
@@ -270,7 +284,7 @@ __device__ __forceinline__ void walk_block(Walk& s, float u0s, float pxs, float 
         s.V2 = pack2(vb, vb + pxs);
         static_for<0, BW / 2>([&](auto kc) {
             constexpr int J = JB + 2 * decltype(kc)::value;
-            if constexpr (J < NJ) walk_pair<J, HS, true, DEG>(s, preg[J], preg[J + 1]);
+            if constexpr (J < NJ) walk_pair<J, HS, true, DEG, VS>(s, preg[J], preg[J + 1]);
         });
     }
 }
@@ -294,7 +308,7 @@ __device__ __forceinline__ void walk_block(Walk& s, float u0s, float pxs, float 
     }
 
 // full8 (warp-uniform): every lane of the warp has at least 8 pixels, so block 0 runs its first 8 pixels without masks.
-template <int NJ, int HS, int DEG, int BW>
+template <int NJ, int HS, int DEG, int BW, bool VS>
 __device__ __forceinline__ float piece_pass1(const Piece& pc, uint32_t w_addr, float pxs, int nblk, float (&preg)[NJ],
                                              bool full8 = false) {
     static_assert(NJ % 2 == 0 && NJ <= 12 * BW && (BW == 4 || BW == 8 || BW == 16 || BW == 32), "pixel capacity must be even and at most 12 blocks");
@@ -306,6 +320,7 @@ __device__ __forceinline__ float piece_pass1(const Piece& pc, uint32_t w_addr, f
     } else {
         s.EPS2 = bc2(pc.rc.eps); s.DEL2 = bc2(pc.rc.delta); s.ALP2 = bc2(pc.rc.alphas); s.BET2 = bc2(pc.rc.betas);
         s.C2S2 = bc2(pc.rc.c2s);
+        s.NGS2 = bc2(pc.ngs);
     }
     s.STEP2 = bc2(2.f * pxs);
     s.DEN2 = pack2(0.f, 0.f);
@@ -314,8 +329,8 @@ __device__ __forceinline__ float piece_pass1(const Piece& pc, uint32_t w_addr, f
     const float u0s = pc.rc.u0s;
 #define JPET_WALK(B)                                                                          \
     do {                                                                                      \
-        if ((B) == 0 && DEG > 0 && BW >= 8 && NJ >= 8 && full8) walk_block<0, NJ, HS, DEG, BW, 8>(s, u0s, pxs, preg); \
-        else walk_block<(B) * BW, NJ, HS, DEG, BW>(s, u0s, pxs, preg);                        \
+        if ((B) == 0 && DEG > 0 && BW >= 8 && NJ >= 8 && full8) walk_block<0, NJ, HS, DEG, BW, VS, 8>(s, u0s, pxs, preg); \
+        else walk_block<(B) * BW, NJ, HS, DEG, BW, VS>(s, u0s, pxs, preg);                    \
     } while (0)
     JPET_BLOCK_CASES(JPET_WALK)
 #undef JPET_WALK
@@ -474,26 +489,26 @@ __device__ __forceinline__ void named_barrier(int id, int nthreads) {
 }
 
 // One event on one group of NWE warps.  tab_n: table row of this event's row count ([lane of the group]).
-template <int NWE, int NJA, int NJB, int HS, int DEG, int BW>
-__device__ __forceinline__ void process_event_rows3(const float4 r0, const float4 r1, const float4 r2, const float4 r3,
+template <int NWE, int NJA, int NJB, int HS, int DEG, int BW, bool VS>
+__device__ __forceinline__ void process_event(const float4 r0, const float4 r1, const float4 r2, const float4 r3,
                                                     const DevParams& p, const uint32_t* tab_n, uint32_t w_addr, uint32_t a_addr,
                                                     int ry0, int rz0, int col_lo, int col_hi, float* red_s, int group, int glane,
                                                     int& my_evals, int& my_skipped, int& overflow) {
     constexpr int GL = NWE * 32;
     Piece A, B;
-    pieces_setup<NJA, NJB, HS, DEG>(tab_n[glane], r0, r1, r2, r3, p, ry0, rz0, col_lo, col_hi, A, B, overflow);
+    pieces_setup<NJA, NJB, HS, DEG, VS>(tab_n[glane], r0, r1, r2, r3, p, ry0, rz0, col_lo, col_hi, A, B, overflow);
     const int nbA = (__reduce_max_sync(0xffffffffu, A.rc.len) + BW - 1) / BW;
     float pregA[NJA];
     // (one-warp groups only: in the 512-thread CTAs of the four-warp groups the second copy of block 0 costs more than it saves)
     const bool fullA = NWE == 1 && DEG > 0 && BW >= 8 && NJA >= 8 && __reduce_min_sync(0xffffffffu, A.rc.len) >= 8;
-    float denom = piece_pass1<NJA, HS, DEG, BW>(A, w_addr, p.pxs, nbA, pregA, fullA);
+    float denom = piece_pass1<NJA, HS, DEG, BW, VS>(A, w_addr, p.pxs, nbA, pregA, fullA);
     my_evals += A.rc.len;
     constexpr int NJB1 = NJB > 0 ? NJB : 2;
     float pregB[NJB1];
     int nbB = 0;
     if constexpr (NJB > 0) {
         nbB = (__reduce_max_sync(0xffffffffu, B.rc.len) + BW - 1) / BW;
-        denom += piece_pass1<NJB, HS, DEG, BW>(B, w_addr, p.pxs, nbB, pregB);
+        denom += piece_pass1<NJB, HS, DEG, BW, VS>(B, w_addr, p.pxs, nbB, pregB);
         my_evals += B.rc.len;
     }
     // ---- denominator: sum over the group -----------------------------------------------------------------------
@@ -515,9 +530,9 @@ __device__ __forceinline__ void process_event_rows3(const float4 r0, const float
 
 // CTA = NG groups of NWE warps.  Work item = (sub-tile, chunk of sorted events): the CTA stages w once, group g
 // takes events g, g + NG, ... of the chunk into its own accumulator region and flushes it with red.global.add.
-template <int NWE, int NG, int NJA, int NJB, int HS, int MINB, int DEG, int BW>
+template <int NWE, int NG, int NJA, int NJB, int HS, int MINB, int DEG, int BW, bool VS>
 __global__ void __launch_bounds__(NWE * NG * 32, MINB)
-mlem_rows3_kernel(const EventRec* __restrict__ sorted, const WorkItem* __restrict__ items, int* __restrict__ meta,
+mlem_rows_kernel(const EventRec* __restrict__ sorted, const WorkItem* __restrict__ items, int* __restrict__ meta,
                   const __grid_constant__ DevParams p, const float* __restrict__ wT, float* __restrict__ accT,
                   const uint32_t* __restrict__ tab, unsigned long long* __restrict__ counters) {
     pdl_wait();
@@ -583,9 +598,13 @@ mlem_rows3_kernel(const EventRec* __restrict__ sorted, const WorkItem* __restric
             slot ^= 64u;
             if (q + NG < wi.count && lane < 4) cp_async16(rec_addr + slot + 16 * lane, rec + 4 * (q + NG) + lane);
             cp_async_commit();
-            const int nrows = __float_as_int(r3.w);
-            const uint32_t* tab_n = tab_s + (nrows - p.nr_min) * GL;
-            process_event_rows3<NWE, NJA, NJB, HS, DEG, BW>(r0, r1, r2, r3, p, tab_n, w_addr, a_addr, ry0, rz0, col_lo, col_hi,
+            // the sort admitted the event to a regular bin because its row count is one the table holds (event_place);
+            // the clamp keeps a corrupted record inside the table and reports it like an overflowing piece
+            const int nrows = rows_count(__float_as_int(r3.w));
+            const int tn = min(max(nrows - p.nr_min, 0), p.nr_max - p.nr_min);
+            overflow |= tn != nrows - p.nr_min;
+            const uint32_t* tab_n = tab_s + tn * GL;
+            process_event<NWE, NJA, NJB, HS, DEG, BW, VS>(r0, r1, r2, r3, p, tab_n, w_addr, a_addr, ry0, rz0, col_lo, col_hi,
                                                    red_s[group][parity], group, glane, my_evals, my_skipped, overflow);
             parity ^= 1;
         }

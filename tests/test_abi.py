@@ -29,7 +29,7 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
     for name in declared_symbols():
         assert hasattr(lib, name), f"{name} declared in include/jpet.h but not exported by libjpet.so"
     assert sorted(binding.EXPORTS) == declared_symbols()
-    assert lib.jpet_abi_version() == 1
+    assert lib.jpet_abi_version() == 2
 
 
 def test_library_is_sm100a_native():
@@ -73,6 +73,19 @@ def test_argument_validation_needs_no_gpu():
     assert lib.jpet_mlem_iterate(None, 0, g, s, gr, None, None, None) == binding.JPET_E_INVAL
     assert b"gamma" in lib.jpet_last_error()
     assert lib.jpet_set_gamma(ctypes.c_float(0.0)) == binding.JPET_OK
+    # the calls added in round 2 validate before touching CUDA as well
+    assert lib.jpet_set_sigma_z_edge(ctypes.c_float(-0.1)) == binding.JPET_E_INVAL
+    assert lib.jpet_set_sigma_z_edge(ctypes.c_float(float("nan"))) == binding.JPET_E_INVAL
+    assert lib.jpet_get_sigma_z_edge() == 0.0
+    assert lib.jpet_direct_histogram(None, 5, g, gr, None, None, None) == binding.JPET_E_INVAL
+    assert lib.jpet_direct_histogram(None, 0, g, gr, None, None, None) == binding.JPET_E_INVAL          # NULL histogram
+    prim = (binding.Primitive * 1)(binding.Primitive(0, 0, 0, 10, 10, 0, 0.0))
+    assert lib.jpet_generate_events(prim, 1, 0, 0, g, s, 1, None, None) == binding.JPET_E_INVAL            # no positive intensity
+    assert lib.jpet_generate_events(prim, 0, 0, 0, g, s, 1, None, None) == binding.JPET_E_INVAL
+    assert lib.jpet_mlem_end_peers(None, None, None, 2, None) == binding.JPET_E_INVAL
+    assert lib.jpet_ipc_export(None, None) == binding.JPET_E_INVAL
+    assert lib.jpet_set_option(b"exact_kernel", 5000) == binding.JPET_E_INVAL
+    assert lib.jpet_shape_name(0) == b"small_closed" and lib.jpet_shape_name(99) == b""
 
 
 def test_product_does_not_reach_into_the_oracle():

@@ -20,13 +20,13 @@ def decode(entry):
     return {"row": entry & 0xFF, "part": (entry >> 8) & 3, "sh": (entry >> 10) & 3} if entry & VALID else None
 
 
-@pytest.mark.parametrize("name,variant,degree,warps", [("cfg1", 40, 4, 1), ("cfg2", 56, 4, 1), ("cfg3", 56, 4, 1),
-                                                       ("cfg4", 58, 5, 3), ("cfg5", 52, 4, 4), ("fig4", 60, 0, 1)])
-def test_plan_of_every_workload(name, variant, degree, warps):
+@pytest.mark.parametrize("name,shape,degree,warps", [("cfg1", "small_deg4", 4, 1), ("cfg2", "mid_deg4", 4, 1), ("cfg3", "mid_deg4", 4, 1),
+                                                     ("cfg4", "wide3_deg5", 5, 3), ("cfg5", "xl_deg4", 4, 4), ("fig4", "small_closed", 0, 1)])
+def test_plan_of_every_workload(name, shape, degree, warps):
     """Shape and degree per workload, and the tiling identities the kernels rely on."""
     cfg = synth.CONFIGS[name]
     p = plan_of(cfg)
-    assert (p["variant"], p["degree"], p["warps_per_event"], p["tiled"]) == (variant, degree, warps, 1)
+    assert (jp.jpet_shape_name(p["variant"]), p["degree"], p["warps_per_event"], p["tiled"]) == (shape, degree, warps, 1)
     assert p["HS"] % 32 == 0 and p["HS"] >= 2 * p["Hy"] + 4          # region rows: bank-conflict-free stride, whole ellipse
     assert p["Sy"] == p["HS"] - 2 * p["Hy"] and p["WZ"] == p["Sz"] + 2 * p["Hz"]
     hy = 1.5 * cfg.sigma_dl / cfg.pixel
