@@ -85,6 +85,10 @@ def _load():
     lib.jo_direct_histogram.argtypes = [p, i64, d, i, i, d, p]
     lib.jo_generate_events.restype = i
     lib.jo_generate_events.argtypes = [p, i, i64, i64, d, d, d, d, ctypes.c_uint64, p]
+    lib.jo_kernel_exact_events.restype = None
+    lib.jo_kernel_exact_events.argtypes = [p, i64, d, d, d, d, d, d, i, p]
+    lib.jo_philox4x32_10_block.restype = None
+    lib.jo_philox4x32_10_block.argtypes = [p, p, p]
     _lib = lib
     return lib
 
@@ -138,6 +142,20 @@ def kernel_exact(y, z, event, R, Cinv, n_theta=20001) -> float:
     return float(_load().jo_kernel_exact(y, z, e.ctypes.data, R, C.ctypes.data, int(n_theta)))
 
 
+def kernel_exact_events(events, y, z, R, L, sigma_z, sigma_dl, n_theta=2001) -> np.ndarray:
+    """kernel_exact for events float64 [n, 3] at one pixel, each event with its own matrix (cinv)."""
+    ev = np.ascontiguousarray(events, dtype=np.float64)
+    P = np.empty(ev.shape[0], dtype=np.float64)
+    _load().jo_kernel_exact_events(ev.ctypes.data, ev.shape[0], y, z, R, L, sigma_z, sigma_dl, int(n_theta), P.ctypes.data)
+    return P
+
+
+def philox4x32_10(counter, key):
+    c, k, o = (np.ascontiguousarray(v, dtype=np.uint32) for v in (counter, key, np.zeros(4)))
+    _load().jo_philox4x32_10_block(c.ctypes.data, k.ctypes.data, o.ctypes.data)
+    return [int(v) for v in o]
+
+
 def bbox_half_extents_c(tan_t, Cinv):
     C = np.ascontiguousarray(Cinv, dtype=np.float64)
     out = (ctypes.c_double * 2)()
@@ -162,8 +180,8 @@ def direct_histogram(events, R, n_y, n_z, pixel, hist=None):
 def generate_events(phantom, n, R, L, sigma_z, sigma_dl, seed, first=0) -> np.ndarray:
     """Counter-based event simulation (same generator as the CUDA path, fp64). phantom: objects with kind ('E'/'B'),
     cy, cz, hy, hz, phi_deg, intensity. Returns float32 [n, 3]."""
-    prims = np.array([[{"E": 0.0, "B": 1.0}.get(q.kind, float(q.kind)), q.cy, q.cz, q.hy, q.hz, q.phi_deg, q.intensity]
-                      for q in phantom], dtype=np.float64)
+    kinds = {"E": 0.0, "B": 1.0, 0: 0.0, 1: 1.0}
+    prims = np.array([[kinds[q.kind], q.cy, q.cz, q.hy, q.hz, q.phi_deg, q.intensity] for q in phantom], dtype=np.float64)
     out = np.empty((n, 3), dtype=np.float32)
     rc = _load().jo_generate_events(prims.ctypes.data, len(phantom), int(n), int(first), R, L, sigma_z, sigma_dl,
                                     int(seed), out.ctypes.data)

@@ -518,3 +518,25 @@ int jo_generate_events(const double *prims, int n_prim, int64_t n, int64_t first
     }
     return 0;
 }
+
+/* ---- conveniences for the tests: the exact integral for many events (double [n][3]) at one pixel, each with its own
+ * matrix (jo_cinv); and the Philox block function on its own (known-answer test)                                 */
+void jo_kernel_exact_events(const double *events, int64_t n, double y, double z, double R, double L, double sigma_z,
+                            double sigma_dl, int n_theta, double *P_out)
+{
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int64_t j = 0; j < n; ++j) {
+        double Cinv[3][3];
+        jo_cinv(events[3 * j + 0], events[3 * j + 1], L, sigma_z, sigma_dl, Cinv);
+        P_out[j] = jo_kernel_exact(y, z, events + 3 * j, R, Cinv, n_theta);
+    }
+}
+
+void jo_philox4x32_10_block(const uint32_t counter[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c[4] = { counter[0], counter[1], counter[2], counter[3] };
+    jo_philox4x32_10(c, key[0], key[1]);
+    for (int k = 0; k < 4; ++k) out[k] = c[k];
+}
