@@ -83,8 +83,10 @@ constexpr int64_t kStageDefault = 4ll << 30;
 #define CUDA_TRY(expr)                                                                              \
     do {                                                                                            \
         cudaError_t _e = (expr);                                                                    \
-        if (_e != cudaSuccess)                                                                      \
+        if (_e != cudaSuccess) {                                                                    \
+            (void)cudaGetLastError(); /* reported here: do not leave it for an unrelated later call */ \
             return fail(JPET_E_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+        }                                                                                           \
     } while (0)
 
 // Everything the plan depends on; compared field by field (no padding bytes involved).

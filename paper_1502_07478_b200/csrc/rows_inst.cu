@@ -14,8 +14,10 @@ namespace {
 #define CUDA_TRY(expr)                                                                              \
     do {                                                                                            \
         cudaError_t _e = (expr);                                                                    \
-        if (_e != cudaSuccess)                                                                      \
+        if (_e != cudaSuccess) {                                                                    \
+            (void)cudaGetLastError(); /* reported here: do not leave it for an unrelated later call */ \
             return fail(JPET_E_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+        }                                                                                           \
     } while (0)
 
 // Persistent grid: resident CTAs per SM x SMs (capped by the number of work items); launched with programmatic stream
