@@ -368,15 +368,19 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
         const double g_ba = 6.0 / std::sqrt(2.0) * ag * szm * sg.sigma_dl;
         const double xb = 2.0 * (t_max / (1.0 + t_max * t_max)) * y_max * u_max / (R2 + y_max * y_max) / (0.95 - g_rel - 2.0 * dls * y_max * g.R / (R2 + y_max * y_max));
         const double eb = 1.1 * std::pow(3.0 * y_max / std::sqrt(R2 + y_max * y_max) + g_ba, 2.0);
-        auto trunc_err = [&](int deg) {      // log2 units
-            return 1.4427 * (0.5 * eb * std::pow(xb, deg - 1) / (1.0 - xb) + 0.5 * std::pow(xb, deg + 1) / (deg + 1));
+        // What has to be small is the error of a kernel value against the event's largest one (the image tolerance is
+        // relative to the image maximum).  At the fraction s = |u| / u_max of the central half chord |x| <= xb s, so the two
+        // neglected tails scale with s^(deg-1) and s^(deg+1); the kernel value there is at most exp(-q (1 - eb/9) / 2) of
+        // the peak (b.C^-1.a is linear in b, so ba^2 / D <= (eb / 9) q, and q = b.C^-1.b >= 9 s^2), times <= 1.05 for
+        // the D^-1/2 factor.  max over s in [0, 1] of s^n exp(-g s^2) is (n / (2 g e))^(n/2) when n <= 2 g, else exp(-g).
+        const double gw = 4.5 * std::max(0.0, 1.0 - eb / 9.0);
+        auto wmax = [&](int n) { return 1.05 * (n < 2.0 * gw ? std::pow(n / (2.0 * gw * std::exp(1.0)), 0.5 * n) : std::exp(-gw)); };
+        auto trunc_err = [&](int deg) {      // log2 units, weighted by the kernel value relative to the event's peak
+            return 1.4427 * (0.5 * eb * std::pow(xb, deg - 1) / (1.0 - xb) * wmax(deg - 1) + 0.5 * std::pow(xb, deg + 1) / (deg + 1) * wmax(deg + 1));
         };
         const int deg = g_opt.poly_off || !(xb > 0.0 && xb < 0.5) ? 0 : (trunc_err(4) <= 2e-5 ? 4 : (trunc_err(5) <= 2e-5 ? 5 : 0));
-        // ellipses of at most ~100 rows on three warps instead of four (config 4: 91 rows on 128 lanes leave a quarter of
-        // the lanes idle; 14.60 -> 14.02 ms per 5x10^6 events), the few rows beyond 96 as B pieces
-        if (deg == 5 && nr_hi > 64 && nr_hi <= 104 && fits(kShapes[jpet_host::k_wide3_deg5])) v = jpet_host::k_wide3_deg5;
         for (int s = 0; s < kNumShapes && v < 0; ++s)           // the list is ordered by size within each degree
-            if (kShapes[s].DEG == deg && kShapes[s].NWE != 3 && fits(kShapes[s])) v = s;
+            if (kShapes[s].DEG == deg && fits(kShapes[s])) v = s;
     }
     // no shape fits (or a forced shape does not): every event takes the direct path
     bool tiles_ok = v >= 0 && fits(kShapes[v]);

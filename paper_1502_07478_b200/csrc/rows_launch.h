@@ -26,15 +26,14 @@ namespace jpet_host {
     X(xxl_closed,        4, 3, 52,  0, 128, 1,  0,  8,  0) /* <= 128 rows, chords <= 52 px, three groups (168 registers) */ \
     X(small_deg4,        1, 4, 12,  0,  64, 4,  4,  8,  1) /*                                       (config 1)    */ \
     X(mid_deg4,          1, 4, 20,  8,  64, 4,  4, 32,  1) /* one block per piece                   (configs 2, 3) */ \
-    X(large_deg4,        4, 4, 36,  0, 128, 1,  4,  8,  1)                                                          \
+    X(large_deg4,        4, 4, 36,  0, 128, 1,  4,  8,  1) /*                                       (config 4)    */ \
     X(xl_deg4,           4, 4, 44,  0, 128, 1,  4, 16,  1) /*                                       (config 5)    */ \
     X(xxl_deg4,          4, 3, 52,  0, 128, 1,  4, 16,  1) /* (config 5 with a position-dependent sigma_z)        */ \
     X(small_deg5,        1, 4, 12,  0,  64, 4,  5,  8,  2)                                                          \
     X(mid_deg5,          1, 4, 20,  8,  64, 4,  5,  8,  2)                                                          \
     X(large_deg5,        4, 4, 36,  0, 128, 1,  5, 16,  2)                                                          \
     X(xl_deg5,           4, 4, 44,  0, 128, 1,  5,  8,  3)                                                          \
-    X(xxl_deg5,          4, 3, 52,  0, 128, 1,  5, 16,  3)                                                          \
-    X(wide3_deg5,        3, 4, 36,  8, 128, 1,  5, 32,  3) /* three warps per event: 96 central rows + caps (config 4) */
+    X(xxl_deg5,          4, 3, 52,  0, 128, 1,  5, 16,  3)
 
 struct Shape { const char* name; int NWE, NG, NJA, NJB, HS, MINB, DEG, BW; };
 

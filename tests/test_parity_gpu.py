@@ -156,7 +156,11 @@ def test_cfg1_ten_iterations(jp, oracle):
 
 
 # every shape of the list in csrc/rows_launch.h: the automatic plan can reach each of them
-N_SHAPES = 16
+N_SHAPES = 15
+
+
+def test_the_variant_tests_cover_the_whole_shape_list(jp):
+    assert jp.jpet_shape_name(N_SHAPES - 1) != "" and jp.jpet_shape_name(N_SHAPES) == ""
 
 
 @pytest.mark.parametrize("variant", range(N_SHAPES))
