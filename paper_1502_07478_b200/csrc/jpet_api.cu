@@ -264,11 +264,13 @@ cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t sme
 }
 
 // Events per work item for a batch of n events: the plan's size, halved (not below 64) while the batch would give fewer
-// than four items per SM - small batches are launch- and tail-bound.
+// than three items per resident CTA (MINB CTAs per SM for the shape) - small batches are launch- and tail-bound
+// (config 2, 10^6 events on 592 CTAs: 0.683 ms with 512 events per item, 0.716 ms with 1024).
 int batch_chunk(const Workspace& w, int64_t n) {
     int chunk = w.plan.dp.chunk;
     if (g_opt.chunk > 0) return chunk;
-    while (chunk > 64 && n / chunk < 4 * (int64_t)w.sm_count) chunk /= 2;
+    const int64_t ctas = (int64_t)w.sm_count * std::max(1, kShapes[std::min(std::max(w.plan.shape, 0), kNumShapes - 1)].MINB);
+    while (chunk > 64 && n / chunk < 3 * ctas) chunk /= 2;
     return chunk;
 }
 
@@ -413,10 +415,11 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     }
     p.nby = (gr.n_y + 2 * p.Hy + p.Sy - 1) / p.Sy;
     p.nbz = (gr.n_z + 2 * p.Hz + p.Sz - 1) / p.Sz;
-    // events per work item (one staging of w and one flush of the accumulator regions per item): measured optimum on B200
-    // 128 events per group for the one-warp groups (config 2: 0.740 -> 0.734 ms), 256 for the multi-warp groups
-    // (configs 4, 5: +5-8 %)
-    p.chunk = g_opt.chunk > 0 ? (int)g_opt.chunk : (c.NWE > 1 ? 256 : 128) * c.NG;
+    // events per work item (one staging of w and one flush of the accumulator regions per item): measured on B200 with 10^7
+    // events per launch - 256 events per group for the one-warp groups (config 3: 6.28 -> 6.21 ms against 128), 512 for the
+    // multi-warp groups (config 5: 34.36 -> 33.99 ms, config 4: 24.64 -> 24.34 ms against 256); batch_chunk halves it for
+    // small batches
+    p.chunk = g_opt.chunk > 0 ? (int)g_opt.chunk : (c.NWE > 1 ? 512 : 256) * c.NG;
     out->dp = p;
     out->shape = v;
     out->smem = smem;

@@ -3,6 +3,8 @@ seeded inputs: per-event sigma_z (f1), the direct-reconstruction histogram (f2, 
 accumulator sum fused into the finalise kernel (f3), the device event generator and the exact-kernel mode (f4); plus the
 host ring path and the stream ordering of the workspace.  Run on the B200 box with  pytest -m gpu."""
 import math
+import os
+import sys
 
 import numpy as np
 import pytest
@@ -294,3 +296,56 @@ def test_calls_on_different_streams_are_ordered(jp, oracle):
     ne, _ = jp.jpet_get_counters(stream=s2)
     torch.cuda.synchronize()
     assert ne > 0 and float((b2 - b).abs().max() / b.max()) <= 1e-5
+
+
+# ---- (f3) the sharded iteration across two PROCESSES (one GPU: the ranks' kernels never wait on one another) ------------
+def _p2p_worker(rank, world, port, n_events, n_iter, q):
+    os.environ.update(RANK=str(rank), LOCAL_RANK="0", WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import torch
+    import torch.distributed as dist
+
+    from paper_1502_07478_b200.sharding import ShardedMlem, shard_range
+
+    torch.cuda.set_device(0)
+    dist.init_process_group("gloo")                                 # host plumbing only: handles, barriers
+    cfg = synth.CONFIGS["cfg2"]
+    events = synth.config_events(cfg, n=n_events)                   # every rank draws the same list and takes its shard
+    lo, hi = shard_range(len(events), rank, world)
+    sm = ShardedMlem(dist, mode="p2p")                              # accumulators mapped with cudaIpc, summed in the finalise kernel
+    rho = torch.ones(cfg.n_y * cfg.n_z, device="cuda")
+    out = torch.empty_like(rho)
+    sm.reconstruct(torch.from_numpy(events[lo:hi]).cuda(), geom(cfg), rho, out, n_iter)
+    torch.cuda.synchronize()
+    img = out.cpu().numpy().reshape(cfg.n_y, cfg.n_z)
+    sm.close()
+    dist.destroy_process_group()
+    q.put((rank, lo, hi, img))
+
+
+def test_two_processes_share_accumulators_through_cuda_ipc(jp, oracle):
+    """ShardedMlem(mode="p2p") as bench.py --gpus N runs it, with two processes on this one GPU and gloo for the handle exchange
+    and the barriers: each rank accumulates its half of the events, maps the other rank's accumulator with cudaIpc and
+    finalises over both - every rank must hold the image one process computes from all events (and the oracle's)."""
+    import socket
+
+    import torch.multiprocessing as mp
+
+    n_events, n_iter = 60_001, 2
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_p2p_worker, args=(r, 2, port, n_events, n_iter, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted((q.get(timeout=600) for _ in procs), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    assert (got[0][1], got[0][2], got[1][1], got[1][2]) == (0, n_events // 2, n_events // 2, n_events)
+    assert (got[0][3] == got[1][3]).all()                           # peers are read in rank order: identical bits on every rank
+    cfg = synth.CONFIGS["cfg2"]
+    want, _, _ = oracle.reconstruct(synth.config_events(cfg, n=n_events), *geom(cfg), n_iter)
+    assert rel_err(got[0][3].astype(np.float64), want) <= 1e-4
