@@ -25,8 +25,9 @@ namespace jpet_host {
     X(xl_closed,         4, 4, 44,  0, 128, 1,  0,  8,  0) /* <= 128 rows, chords <= 44 px                        */ \
     X(xxl_closed,        4, 3, 52,  0, 128, 1,  0,  8,  0) /* <= 128 rows, chords <= 52 px, three groups (168 registers) */ \
     X(small_deg4,        1, 4, 12,  0,  64, 4,  4,  8,  1) /*                                       (config 1)    */ \
-    X(mid_deg4,          1, 4, 20,  8,  64, 4,  4, 32,  1) /* one block per piece                   (configs 2, 3) */ \
-    X(large_deg4,        4, 4, 36,  0, 128, 1,  4,  8,  1) /*                                       (config 4)    */ \
+    X(mid18_deg4,        1, 4, 18,  8,  64, 4,  4, 32,  3) /* one block per piece, chords <= 18 px   (configs 2, 3) */ \
+    X(mid_deg4,          1, 4, 20,  8,  64, 4,  4, 32,  1) /* one block per piece                                  */ \
+    X(large_deg4,        4, 4, 36,  0, 128, 1,  4, 16,  1) /*                                       (config 4)    */ \
     X(xl_deg4,           4, 4, 44,  0, 128, 1,  4, 16,  1) /*                                       (config 5)    */ \
     X(xxl_deg4,          4, 3, 52,  0, 128, 1,  4, 16,  1) /* (config 5 with a position-dependent sigma_z)        */ \
     X(small_deg5,        1, 4, 12,  0,  64, 4,  5,  8,  2)                                                          \

@@ -20,7 +20,7 @@ def decode(entry):
     return {"row": entry & 0xFF, "part": (entry >> 8) & 3, "sh": (entry >> 10) & 3} if entry & VALID else None
 
 
-@pytest.mark.parametrize("name,shape,degree,warps", [("cfg1", "small_deg4", 4, 1), ("cfg2", "mid_deg4", 4, 1), ("cfg3", "mid_deg4", 4, 1),
+@pytest.mark.parametrize("name,shape,degree,warps", [("cfg1", "small_deg4", 4, 1), ("cfg2", "mid18_deg4", 4, 1), ("cfg3", "mid18_deg4", 4, 1),
                                                      ("cfg4", "large_deg4", 4, 4), ("cfg5", "xl_deg4", 4, 4), ("fig4", "small_closed", 0, 1)])
 def test_plan_of_every_workload(name, shape, degree, warps):
     """Shape and degree per workload, and the tiling identities the kernels rely on."""
