@@ -286,7 +286,7 @@ def measure(dev: Device, ranks: Ranks, cfg, ev_d, steps, warmup, sharded=None):
     plan = jp.jpet_plan_describe(*g)
     return {"step_ms_sum": sum(step_ms), "step_ms": statistics.mean(step_ms), "kern_ms": statistics.mean(kern_ms),
             "n_evals": n_evals, "n_skipped": n_skipped, "launches": int(launches), "kernel_launches": int(kernel_launches),
-            "plan": plan, "shape": jp.jpet_shape_name(jp.jpet_get_option("last_variant")),
+            "plan": plan, "shape": shape_names(jp),
             "tiled": bool(jp.jpet_get_option("last_tiled")), "smem": jp.jpet_get_option("last_smem_bytes")}
 
 
@@ -328,6 +328,14 @@ def roofline_of(dev: Device, cfg, n_events, m, peaks, peak_kind):
             "kernel_ms": m["kern_ms"], "kernel_share_of_step": m["kern_ms"] / m["step_ms"],
             "kernel_launches_per_step": m["kernel_launches"],
             "hbm_gbs_algorithmic": algorithmic * batches / kern_s / 1e9, "hbm_peak_gbs": peaks.get("hbm_gbs")}
+
+
+def shape_names(jp):
+    """Shape of the last iteration's event kernel; "a + b" when the sort made two degree classes (b walks the events whose own
+    truncation bound allows the degree-3 exponent polynomial)."""
+    name = jp.jpet_shape_name(jp.jpet_get_option("last_variant"))
+    low = jp.jpet_get_option("last_variant_low")
+    return name + (" + " + jp.jpet_shape_name(low) if low >= 0 else "")
 
 
 def ncu_traffic(name, n_events, batches):

@@ -182,7 +182,10 @@ int jpet_ipc_close(void *dev_ptr);
  *   "sub_tile_z"   width in pixels of the image sub-tiles the events are sorted by; 0 = automatic
  *   "ctas_per_sm"  cap on resident CTAs per SM for the persistent grid; 0 = automatic
  *   "poly_off"     1 = never evaluate the exponent of Eq. 7 as a polynomial in u (always rsqrt + ex2); 0 = automatic:
- *                  the plan bounds the truncation error and picks degree 4, 5 or the closed form
+ *                  the plan bounds the truncation error and picks degree 3, 4, 5 or the closed form
+ *   "degree_classes_off"  1 = one degree for all events; 0 (default) = when the plan's degree is 4 or 5, the sort tests every
+ *                  event against its own truncation bound and the events that pass are walked with the degree-3
+ *                  polynomial (a second launch of the same kernel shape; gamma = 0 and constant sigma_z only)
  *   "pdl"          1 (default) = launch the kernels of an iteration with programmatic stream serialisation (each starts
  *                  with griddepcontrol.wait: only launch latency overlaps the previous kernel); 0 = plain launches
  *   "time_kernel"  1 = bracket each tiled event-kernel launch with CUDA events on its stream; the summed duration of
@@ -195,7 +198,8 @@ int jpet_ipc_close(void *dev_ptr);
  *                  over (-pi/2, pi/2)) evaluated with that many trapezoid nodes in tan(theta) over +-8 sigma around the
  *                  integrand's peak, on the same 3-sigma pixel set; every event takes the direct kernel (a diagnostic mode,
  *                  ~50x slower); 0 (default) = Eq. 7
- * jpet_get_option also answers "last_variant", "last_tiled", "last_smem_bytes" (what the last iteration used) and
+ * jpet_get_option also answers "last_variant", "last_variant_low" (the degree-3 shape of the second degree class, -1 if
+ * there is one class), "last_tiled", "last_smem_bytes" (what the last iteration used) and
  * "last_overflow" (row pieces that did not fit their register slot: 0 by construction; synchronises the device).
  * Returns JPET_E_INVAL for an unknown name or a value out of range. */
 int jpet_set_option(const char *name, int64_t value);
@@ -218,6 +222,7 @@ const char *jpet_last_error(void);
  *   out[10] / out[11] halo Hy / Hz                                 out[12] events per work item
  *   out[13] dynamic shared memory per CTA [bytes]                  out[14] 1 = tiled (0: every event on the direct kernel)
  *   out[15] / out[16] smallest / largest ellipse row count of the task table (0, 0: no table)
+ *   out[17] (when n_out >= 18) shape id of the degree-3 instance for the events of the second degree class, -1 if none
  * n_out = number of int64 slots the caller provides (>= 17).  task_table_host (may be NULL) receives up to
  * table_cap 32-bit words of the task table [(row count - out[15]) * 32 * out[2] + lane]: piece A in bits 0-15, piece B
  * in bits 16-31; a 16-bit entry: bits 0-7 row, 8-9 part, 10-11 log2(parts), bit 15 valid (csrc/task_table.h).

@@ -240,14 +240,15 @@ def jpet_plan_describe(R, L, sigma_z, sigma_dl, n_y, n_z, pixel):
     import numpy as np
 
     g, s, gr = _structs(R, L, sigma_z, sigma_dl, n_y, n_z, pixel)
-    out = (ctypes.c_int64 * 17)()
-    n = load().jpet_plan_describe(g, s, gr, out, 17, None, 0)
+    out = (ctypes.c_int64 * 18)()
+    n = load().jpet_plan_describe(g, s, gr, out, 18, None, 0)
     if n < 0:
         _check(int(n))
     tab = np.zeros(int(n), dtype=np.uint32)
     if n:
-        load().jpet_plan_describe(g, s, gr, out, 17, tab.ctypes.data, int(n))
+        load().jpet_plan_describe(g, s, gr, out, 18, tab.ctypes.data, int(n))
     plan = dict(zip(PLAN_FIELDS, [int(v) for v in out]))
+    plan["variant_low"] = int(out[17])     # degree-3 instance for the events of degree class 1 (-1: one class)
     lanes = 32 * max(plan["warps_per_event"], 1)
     plan["table"] = tab.reshape(-1, lanes) if n else tab
     return plan

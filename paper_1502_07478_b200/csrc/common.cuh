@@ -64,7 +64,16 @@ struct DevParams {
     int chunk;                         // events per work item
     int nr_min, nr_max;                // ellipse row counts covered by the task table of the tiled event kernel;
                                        // nr_max > 0 makes the records carry the UNCLIPPED row range of the ellipse
+    // degree classes (n_cls = 2): the sort puts the events whose OWN truncation bound allows the degree-3 exponent
+    // polynomial (low_degree_ok) into a second set of bins, walked by the degree-3 instance of the kernel shape
+    int n_cls;                         // 1: one class
+    float cls_xk, cls_ylim, cls_tol;   // 2 u_max / 0.95 [mm], half image height [mm], bound in log2 units
 };
+
+// meta words of a sorted batch (BinSet::meta): the work-item list holds the full items (chunk events) of all bins in bin
+// order, then the partly filled last items in bin order; the bins of degree class 0 come first.
+enum MetaWord { kMetaItems = 0, kMetaDirectStart = 1, kMetaDirectCount = 2, kMetaCounter0 = 3, kMetaFull0 = 4, kMetaPart0 = 5,
+                kMetaCounter1 = 6, kMetaFull = 7, kMetaWords = 8 };
 
 struct WorkItem { int bin, start, count; };
 
@@ -134,6 +143,26 @@ __device__ __forceinline__ EventConsts event_setup(float zu, float zd, float dl,
         e.S = iu + id; e.Dl = id - iu; e.inv_S = 1.f / e.S;
     }
     return e;
+}
+
+// Per-event form of the plan's truncation bound (jpet_api.cu make_plan) for the degree-3 exponent
+// polynomial, gamma = 0 and constant sigma_z: with y_m the largest |y| the event's ellipse reaches inside the image,
+//   x_e = 2 |t| / sec2 * y_m u_max / (R^2 + y_m^2) / 0.95,      e_e = 1.1 (3 y_m / sqrt(R^2 + y_m^2))^2,
+// the neglected terms at the fraction s of the half chord are <= e_e (1 + x_e)^2 s^2 (x_e s)^2 / (2 (1 - x_e)) and
+// (x_e s)^4 / 8, a kernel value there is <= 1.05 exp(-g s^2) of the event's peak, g = 4.5 (1 - e_e / 9), and
+// max_s s^4 exp(-g s^2) = (2 / (g e))^2 for g > 2.  Evaluated in fp32 against 0.9 of the bound.
+__device__ __forceinline__ bool low_degree_ok(const EventConsts& e, const DevParams& p) {
+    const float ym = fminf(fabsf(e.y_t) + e.hy_px * p.px, p.cls_ylim);
+    const float r2 = fmaf(ym, ym, p.R2);
+    const float xe = p.cls_xk * fabsf(e.t) / e.sec2 * ym / r2;
+    const float ee = 1.1f * 9.f * ym * ym / r2;
+    const float g = 4.5f * (1.f - ee * (1.f / 9.f));
+    if (!(g > 2.2f) || !(xe < 0.25f)) return false;
+    const float m = 0.73575888f / g;                       // 2 / (g e)
+    const float w = 1.05f * m * m;
+    const float x2 = xe * xe, opx = 1.f + xe;
+    const float err = 1.4427f * w * (0.5f * ee * opx * opx * x2 / (1.f - xe) + 0.125f * x2 * x2);
+    return err <= 0.9f * p.cls_tol;
 }
 
 // Rows of the ellipse clipped to [row_lo, row_hi]: returns first row and count.

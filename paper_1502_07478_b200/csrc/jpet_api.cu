@@ -45,7 +45,7 @@ int launch_rows_shape(const RowsLaunch& rl) {
     if (rc == -100) rc = launch_rows_group1(rl);
     if (rc == -100) rc = launch_rows_group2(rl);
     if (rc == -100) rc = launch_rows_group3(rl);
-    if (rc == -100) rc = fail(JPET_E_INVAL, "unknown kernel shape %d", rl.plan->shape);
+    if (rc == -100) rc = fail(JPET_E_INVAL, "unknown kernel shape %d", rl.shape);
     return rc;
 }
 }  // namespace jpet_host
@@ -73,6 +73,7 @@ struct Options {
     int64_t variant = -1;         // shape id, -1 = automatic
     int64_t pdl = 1;              // 1 = launch the kernels of an iteration with programmatic stream serialisation
     int64_t poly_off = 0;         // 1 = never pick a polynomial-exponent shape automatically
+    int64_t cls_off = 0;          // 1 = no per-event degree classes
     int64_t ctas_per_sm = 0;      // 0 = automatic
     int64_t stage_bytes = 0;      // device staging budget of the host-buffer calls; 0 = default
     int64_t exact_kernel = 0;     // > 0: theta-quadrature nodes of the exact-kernel mode
@@ -95,12 +96,12 @@ struct PlanKey {
     jpet_sigmas sg{0, 0};
     jpet_grid gr{0, 0, 0};
     float a3 = 0, gamma = 0, sz_eta = 0;
-    int64_t variant = 0, sz = 0, chunk = 0, force_direct = 0, poly_off = 0, exact = 0;
+    int64_t variant = 0, sz = 0, chunk = 0, force_direct = 0, poly_off = 0, exact = 0, cls_off = 0;
     bool operator==(const PlanKey& o) const {
         return g.R == o.g.R && g.L == o.g.L && sg.sigma_z == o.sg.sigma_z && sg.sigma_dl == o.sg.sigma_dl && gr.n_y == o.gr.n_y &&
                gr.n_z == o.gr.n_z && gr.pixel == o.gr.pixel && a3 == o.a3 && gamma == o.gamma && sz_eta == o.sz_eta &&
                variant == o.variant && sz == o.sz && chunk == o.chunk && force_direct == o.force_direct && poly_off == o.poly_off &&
-               exact == o.exact;
+               exact == o.exact && cls_off == o.cls_off;
     }
 };
 
@@ -290,13 +291,18 @@ int run_binset(Workspace& w, BinSet& bs, cudaStream_t st) {
         rl.bs = &bs; rl.plan = &w.plan; rl.wT = w.wT; rl.accT = w.accT; rl.tab = w.tab; rl.counters = w.counters;
         rl.sm_count = w.sm_count; rl.device = w.device; rl.stream = st; rl.pdl = g_opt.pdl != 0;
         rl.ctas_per_sm = (int)g_opt.ctas_per_sm;
-        rl.max_items = bs.n / batch_chunk(w, bs.n) + (int64_t)dp.nby * dp.nbz + 1;
+        rl.max_items = bs.n / batch_chunk(w, bs.n) + (int64_t)dp.nby * dp.nbz * dp.n_cls + 1;
+        rl.shape = w.plan.shape; rl.cls = 0;
         int rc = jpet_host::launch_rows_shape(rl);
         if (rc) return rc;
+        if (dp.n_cls == 2) {                 // the events of degree class 1 on the degree-3 instance of the shape
+            rl.shape = w.plan.shape_lo; rl.cls = 1;
+            if ((rc = jpet_host::launch_rows_shape(rl))) return rc;
+        }
         if (g_opt.time_kernel) { CUDA_TRY(cudaEventRecord(w.tk[w.tk_used + 1], st)); w.tk_used += 2; }
     }
-    // the work counter meta[3] is zero before the tiled kernel: bin_scan_kernel zeroes it and the direct kernel, the last
-    // kernel of every run over a sorted set, zeroes it again (jpet_reconstruct sorts once and iterates)
+    // the work counters are zero before the tiled kernels: bin_scan_kernel zeroes them and the direct kernel, the last
+    // kernel of every run over a sorted set, zeroes them again (jpet_reconstruct sorts once and iterates)
     const int dgrid = dp.t_max >= 0.f ? w.sm_count : w.sm_count * 16;
     if (g_opt.exact_kernel > 0)
         CUDA_TRY(launch_pdl(jpet::mlem_rows_direct_kernel<true>, dim3(dgrid), dim3(128), 0, st, (const float*)bs.sorted, 16, bs.meta, dp,
@@ -380,13 +386,40 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
         auto trunc_err = [&](int deg) {      // log2 units, weighted by the kernel value relative to the event's peak
             return 1.4427 * (0.5 * eb * std::pow(xb, deg - 1) / (1.0 - xb) * wmax(deg - 1) + 0.5 * std::pow(xb, deg + 1) / (deg + 1) * wmax(deg + 1));
         };
-        const int deg = g_opt.poly_off || !(xb > 0.0 && xb < 0.5) ? 0 : (trunc_err(4) <= 2e-5 ? 4 : (trunc_err(5) <= 2e-5 ? 5 : 0));
-        for (int s = 0; s < kNumShapes && v < 0; ++s)           // the list is ordered by size within each degree
-            if (kShapes[s].DEG == deg && fits(kShapes[s])) v = s;
+        // among the degrees that meet the bound (a higher degree is only more accurate): the first shape of each degree
+        // that holds the workload's ellipses (the list is ordered by size within a degree), then the one with the fewest
+        // pixel slots per event, the lowest degree on a tie; no polynomial degree: the closed form
+        const bool poly_ok = !g_opt.poly_off && xb > 0.0 && xb < 0.5;
+        int best_slots = 0;
+        for (int deg = 3; deg <= 5 && poly_ok; ++deg) {
+            if (!(trunc_err(deg) <= 2e-5)) continue;
+            for (int s = 0; s < kNumShapes; ++s) {
+                if (kShapes[s].DEG != deg || !fits(kShapes[s])) continue;
+                const int slots = 32 * kShapes[s].NWE * (kShapes[s].NJA + kShapes[s].NJB);
+                if (v < 0 || slots < best_slots) { v = s; best_slots = slots; }
+                break;
+            }
+        }
+        for (int s = 0; s < kNumShapes && v < 0; ++s)
+            if (kShapes[s].DEG == 0 && fits(kShapes[s])) v = s;
     }
     // no shape fits (or a forced shape does not): every event takes the direct path
     bool tiles_ok = v >= 0 && fits(kShapes[v]);
     if (v < 0) v = 0;
+    // Degree classes: the bound above holds for the worst event the image can hold (largest |y|, largest tilt); most
+    // events are far from it.  When the plan's degree is 4 or 5 and the shape has a degree-3 instance, the sort tests
+    // every event against its OWN bound (low_degree_ok, common.cuh; gamma = 0 and constant sigma_z only) and the events
+    // that pass are walked by the degree-3 instance (configs 2 and 4: 100 % / 77 % of the events, -6 % / -5 % time).
+    int v_lo = -1;
+    if (g_opt.variant < 0 && !g_opt.cls_off && tiles_ok && kShapes[v].DEG > 3 && kShapes[v].CLS && gamma == 0.f && eta == 0.0)
+        for (int s = 0; s < kNumShapes && v_lo < 0; ++s)
+            if (kShapes[s].DEG == 3 && kShapes[s].CLS && kShapes[s].NWE == kShapes[v].NWE && kShapes[s].NG == kShapes[v].NG && kShapes[s].NJA == kShapes[v].NJA &&
+                kShapes[s].NJB == kShapes[v].NJB && kShapes[s].HS == kShapes[v].HS)
+                v_lo = s;
+    p.n_cls = v_lo >= 0 ? 2 : 1;
+    p.cls_xk = (float)(2.0 * 3.0 * szm / std::sqrt(2.0) / 0.95);
+    p.cls_ylim = (float)(0.5 * gr.n_y * px);
+    p.cls_tol = 2e-5f;
     const Shape& c = kShapes[v];
     const int n_regions = 1 + c.NG;
     p.nr_min = nr_lo; p.nr_max = nr_hi;
@@ -412,6 +445,7 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     }
     if (smem > budget || !tiles_ok || p.WZ < c.NJA + 4 || g_opt.force_direct || g_opt.exact_kernel > 0) {
         p.t_max = -1.f; smem = 0; p.nr_min = p.nr_max = 0; tab.clear();
+        p.n_cls = 1; v_lo = -1;
     }
     p.nby = (gr.n_y + 2 * p.Hy + p.Sy - 1) / p.Sy;
     p.nbz = (gr.n_z + 2 * p.Hz + p.Sz - 1) / p.Sz;
@@ -422,6 +456,7 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     p.chunk = g_opt.chunk > 0 ? (int)g_opt.chunk : (c.NWE > 1 ? 512 : 256) * c.NG;
     out->dp = p;
     out->shape = v;
+    out->shape_lo = v_lo;
     out->smem = smem;
     out->vs = eta != 0.0;
     if (tab_out) tab_out->swap(tab);
@@ -435,7 +470,7 @@ int grid_for(int64_t M) { return (int)((M + 255) / 256); }
 
 int ensure_binset(Workspace& w, BinSet& bs, int64_t n, bool need_sorted) {
     const DevParams& dp = w.plan.dp;
-    size_t items_cap = (size_t)(n / batch_chunk(w, n)) + (size_t)dp.nby * dp.nbz + 2;
+    size_t items_cap = (size_t)(n / batch_chunk(w, n)) + (size_t)dp.nby * dp.nbz * dp.n_cls + 2;
     const size_t need_floats = 16 * (size_t)std::max<int64_t>(n, 1);
     if (need_sorted && need_floats > bs.cap_events) {          // cap_events counts floats
         if (bs.owns_sorted) cudaFree(bs.sorted);
@@ -450,7 +485,7 @@ int ensure_binset(Workspace& w, BinSet& bs, int64_t n, bool need_sorted) {
         CUDA_TRY(cudaMalloc(&bs.items, sizeof(jpet::WorkItem) * items_cap));
         bs.cap_items = items_cap;
     }
-    if (!bs.meta) CUDA_TRY(cudaMalloc(&bs.meta, 4 * sizeof(int)));
+    if (!bs.meta) CUDA_TRY(cudaMalloc(&bs.meta, jpet::kMetaWords * sizeof(int)));
     return JPET_OK;
 }
 
@@ -475,7 +510,7 @@ int ensure_sort_attr(Workspace& w) {
 // Counting sort of one batch (<= kMaxBatch events) by sub-tile into bs.sorted, and its work items.
 int bin_batch(Workspace& w, const float* events, int64_t n, BinSet& bs, cudaStream_t st) {
     const DevParams& dp = w.plan.dp;
-    const int nb = dp.nby * dp.nbz;
+    const int nb0 = dp.nby * dp.nbz, nb = nb0 * dp.n_cls;      // regular bins: of degree class 0, of all classes
     int rc = ensure_sort_attr(w);
     if (rc) return rc;
     if ((size_t)n > w.cap_place) {
@@ -507,7 +542,7 @@ int bin_batch(Workspace& w, const float* events, int64_t n, BinSet& bs, cudaStre
                             counts, nb + 1, use_smem));
         g_launches++;
     }
-    CUDA_TRY(launch_pdl(jpet::bin_scan_kernel, dim3(1), dim3(1024), 0, st, counts, cursors, bs.items, bs.meta, nb, batch_chunk(w, n)));
+    CUDA_TRY(launch_pdl(jpet::bin_scan_kernel, dim3(1), dim3(1024), 0, st, counts, cursors, bs.items, bs.meta, nb, nb0, batch_chunk(w, n)));
     g_launches++;
     w.counts_clean_nb = saved_clean;
     if (n > 0) {
@@ -539,7 +574,7 @@ int do_begin(Workspace& w, const jpet_geometry* g, const jpet_sigmas* sg, const 
         PlanKey key;
         key.g = *g; key.sg = *sg; key.gr = *gr; key.a3 = g_opt.a3_coef; key.gamma = g_opt.gamma; key.sz_eta = g_opt.sz_eta;
         key.variant = g_opt.variant; key.sz = g_opt.sz; key.chunk = g_opt.chunk; key.force_direct = g_opt.force_direct;
-        key.poly_off = g_opt.poly_off; key.exact = g_opt.exact_kernel;
+        key.poly_off = g_opt.poly_off; key.exact = g_opt.exact_kernel; key.cls_off = g_opt.cls_off;
         if (!w.plan_valid || !(key == w.plan_key)) {
             make_plan(*g, *sg, *gr, &w.plan, &w.tab_host);
             w.plan_key = key;
@@ -1108,6 +1143,8 @@ int jpet_set_option(const char* name, int64_t value) {
         g_opt.variant = value;
     } else if (!strcmp(name, "poly_off")) {
         g_opt.poly_off = value != 0;
+    } else if (!strcmp(name, "degree_classes_off")) {
+        g_opt.cls_off = value != 0;
     } else if (!strcmp(name, "pdl")) {
         g_opt.pdl = value != 0;
     } else if (!strcmp(name, "ctas_per_sm")) {
@@ -1133,6 +1170,7 @@ int64_t jpet_get_option(const char* name) {
     if (!strcmp(name, "time_kernel")) return g_opt.time_kernel;
     if (!strcmp(name, "variant")) return g_opt.variant;
     if (!strcmp(name, "poly_off")) return g_opt.poly_off;
+    if (!strcmp(name, "degree_classes_off")) return g_opt.cls_off;
     if (!strcmp(name, "pdl")) return g_opt.pdl;
     if (!strcmp(name, "ctas_per_sm")) return g_opt.ctas_per_sm;
     if (!strcmp(name, "stage_bytes")) return g_opt.stage_bytes;
@@ -1151,6 +1189,7 @@ int64_t jpet_get_option(const char* name) {
     }
     if (!strcmp(name, "last_kernel_launches")) return (int64_t)(w->tk_used / 2);
     if (!strcmp(name, "last_variant")) return w->plan.shape;
+    if (!strcmp(name, "last_variant_low")) return w->plan.dp.n_cls == 2 ? w->plan.shape_lo : -1;
     if (!strcmp(name, "last_smem_bytes")) return (int64_t)w->plan.smem;
     if (!strcmp(name, "last_tiled")) return w->plan.dp.t_max >= 0.f;
     if (!strcmp(name, "last_overflow")) {       // records the event kernel could not hold (0 by construction; synchronises the device)
@@ -1187,10 +1226,11 @@ int64_t jpet_plan_describe(const jpet_geometry* geometry, const jpet_sigmas* sig
     make_plan(*geometry, *sigmas, *grid, &plan, &tab);
     const DevParams& dp = plan.dp;
     const bool tiled = dp.t_max >= 0.f;
-    const Shape v = tiled ? kShapes[plan.shape] : Shape{"none", 0, 0, 0, 0, 0, 0, 0, 0};
+    const Shape v = tiled ? kShapes[plan.shape] : Shape{"none", 0, 0, 0, 0, 0, 0, 0, 0, 0};
     const int64_t vals[17] = {plan.shape, v.DEG, v.NWE, v.NG, v.NJA, v.NJB, dp.HS, dp.WZ, dp.Sy, dp.Sz, dp.Hy, dp.Hz, dp.chunk,
                               (int64_t)plan.smem, tiled, dp.nr_min, dp.nr_max};
     for (int i = 0; i < 17; ++i) out[i] = vals[i];
+    if (n_out >= 18) out[17] = tiled ? plan.shape_lo : -1;
     if (task_table_host)
         for (int64_t i = 0; i < std::min<int64_t>(table_cap, (int64_t)tab.size()); ++i) task_table_host[i] = tab[(size_t)i];
     return (int64_t)tab.size();

@@ -59,7 +59,7 @@ mlem_rows_direct_kernel(const float* __restrict__ sorted, int stride, int* __res
     pdl_wait();
     const int lane = threadIdx.x & 31;
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
-    const int start = meta[1], count = meta[2];
+    const int start = meta[kMetaDirectStart], count = meta[kMetaDirectCount];
     unsigned long long my_evals = 0, my_skipped = 0;
     for (int q = warp; q < count; q += n_warps) {
         const float* ev = sorted + (size_t)stride * (size_t)(start + q);      // raw triple at the head of the slot
@@ -89,9 +89,9 @@ mlem_rows_direct_kernel(const float* __restrict__ sorted, int stride, int* __res
     for (int d = 16; d > 0; d >>= 1) my_evals += __shfl_xor_sync(0xffffffffu, my_evals, d);
     if (lane == 0 && my_evals) atomicAdd(counters + 0, my_evals);
     if (lane == 0 && my_skipped) atomicAdd(counters + 1, my_skipped);
-    // this kernel always follows the tiled event kernel in the stream: reset the work counter for the next run over
+    // this kernel always follows the tiled event kernel(s) in the stream: reset the work counters for the next run over
     // the same sorted events (jpet_reconstruct sorts once and iterates)
-    if (blockIdx.x == 0 && threadIdx.x == 0) meta[3] = 0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) { meta[kMetaCounter0] = 0; meta[kMetaCounter1] = 0; }
 }
 
 // |E_j| only (jpet_count_evals): thread per event, rows in a loop, no kernel values.

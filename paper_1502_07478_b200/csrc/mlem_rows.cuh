@@ -530,11 +530,11 @@ __device__ __forceinline__ void process_event(const float4 r0, const float4 r1, 
 
 // CTA = NG groups of NWE warps.  Work item = (sub-tile, chunk of sorted events): the CTA stages w once, group g
 // takes events g, g + NG, ... of the chunk into its own accumulator region and flushes it with red.global.add.
-template <int NWE, int NG, int NJA, int NJB, int HS, int MINB, int DEG, int BW, bool VS>
+template <int NWE, int NG, int NJA, int NJB, int HS, int MINB, int DEG, int BW, bool VS, bool CLS>
 __global__ void __launch_bounds__(NWE * NG * 32, MINB)
 mlem_rows_kernel(const EventRec* __restrict__ sorted, const WorkItem* __restrict__ items, int* __restrict__ meta,
                   const __grid_constant__ DevParams p, const float* __restrict__ wT, float* __restrict__ accT,
-                  const uint32_t* __restrict__ tab, unsigned long long* __restrict__ counters) {
+                  const uint32_t* __restrict__ tab, unsigned long long* __restrict__ counters, int cls) {
     pdl_wait();
     constexpr int GT = NWE * NG * 32, GL = NWE * 32;
     extern __shared__ __align__(16) float smem[];
@@ -557,19 +557,33 @@ mlem_rows_kernel(const EventRec* __restrict__ sorted, const WorkItem* __restrict
     const uint32_t rec_addr = (uint32_t)__cvta_generic_to_shared(&rec_s[tid >> 5][0][0]);
     const int n_tab = (p.nr_max - p.nr_min + 1) * GL;
     for (int i = tid; i < n_tab; i += GT) tab_s[i] = __ldg(tab + i);
-    const int n_items = meta[0];
+
+    const int n_items = meta[kMetaItems];              // (CLS: the item range of the degree class is read per item)
     int my_evals = 0, my_skipped = 0, overflow = 0;
     unsigned long long tot_evals = 0;
     int parity = 0, ip = 0;
 
     while (true) {
-        if (tid == 0) item_s[ip] = atomicAdd(meta + 3, 1);
+        if (tid == 0) {
+            if constexpr (CLS) {
+                // next item of this launch's degree class: a run of the full items, then a run of the partly filled ones
+                // (MetaWord, common.cuh); read from meta every time, nothing of it lives in registers across the event loop
+                const int k = atomicAdd(meta + (cls ? kMetaCounter1 : kMetaCounter0), 1);
+                const int n_full = meta[kMetaFull], f0 = meta[kMetaFull0], p0 = meta[kMetaPart0];
+                const int seg1_lo = cls ? f0 : 0, seg1_n = cls ? n_full - f0 : f0;
+                const int seg2_lo = n_full + (cls ? p0 : 0), seg2_n = cls ? meta[kMetaItems] - n_full - p0 : p0;
+                item_s[ip] = k < seg1_n ? seg1_lo + k : (k < seg1_n + seg2_n ? seg2_lo + (k - seg1_n) : -1);
+            } else {
+                item_s[ip] = atomicAdd(meta + kMetaCounter0, 1);
+            }
+        }
         __syncthreads();                                   // also: every group is done with the previous w region
         const int item = item_s[ip];
         ip ^= 1;
-        if (item >= n_items) break;
+        if (CLS ? item < 0 : item >= n_items) break;
         const WorkItem wi = items[item];
-        const int by = wi.bin / p.nbz, bz = wi.bin - by * p.nbz;
+        const int bin = CLS && wi.bin >= p.nby * p.nbz ? wi.bin - p.nby * p.nbz : wi.bin;
+        const int by = bin / p.nbz, bz = bin - by * p.nbz;
         const int ry0 = by * p.Sy - 2 * p.Hy, rz0 = bz * p.Sz - 2 * p.Hz;        // region origin (pixel indices)
         const int row_lo = max(0, ry0), row_hi = min(p.n_y - 1, ry0 + HS - 1);
         const int col_lo = max(0, rz0), col_hi = min(p.n_z - 1, rz0 + WZ - 1);

@@ -22,10 +22,11 @@ namespace {
 
 // Persistent grid: resident CTAs per SM x SMs (capped by the number of work items); launched with programmatic stream
 // serialisation (the kernel starts with pdl_wait()).
-template <int NWE, int NG, int NJA, int NJB, int HS, int MINB, int DEG, int BW, bool VS>
+template <int NWE, int NG, int NJA, int NJB, int HS, int MINB, int DEG, int BW, bool VS, bool CLS>
 int launch_rows(const RowsLaunch& rl) {
     constexpr int NT = NWE * NG * 32;
-    auto kern = jpet::mlem_rows_kernel<NWE, NG, NJA, NJB, HS, MINB, DEG, BW, VS>;
+    auto kern = jpet::mlem_rows_kernel<NWE, NG, NJA, NJB, HS, MINB, DEG, BW, VS, CLS>;
+    if (!CLS && (rl.cls != 0 || rl.plan->dp.n_cls != 1)) return fail(JPET_E_INVAL, "internal: shape without degree classes launched on a two-class sort");
     const jpet::DevParams& dp = rl.plan->dp;
     const size_t smem = rl.plan->smem;
     if (dp.HS != HS) return fail(JPET_E_INVAL, "internal: region stride %d does not match the kernel's %d", dp.HS, HS);
@@ -51,7 +52,7 @@ int launch_rows(const RowsLaunch& rl) {
     cfg.attrs = attr;
     cfg.numAttrs = rl.pdl ? 1 : 0;
     CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, reinterpret_cast<const jpet::EventRec*>(rl.bs->sorted), (const jpet::WorkItem*)rl.bs->items,
-                                rl.bs->meta, dp, rl.wT, rl.accT, rl.tab, rl.counters));
+                                rl.bs->meta, dp, rl.wT, rl.accT, rl.tab, rl.counters, rl.cls));
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     return JPET_OK;
@@ -63,12 +64,12 @@ int launch_rows(const RowsLaunch& rl) {
 #define JPET_CAT(a, b) JPET_CAT2(a, b)
 
 int JPET_CAT(launch_rows_group, JPET_GROUP)(const RowsLaunch& rl) {
-    switch (rl.plan->shape) {
-#define JPET_X(name, NWE, NG, NJA, NJB, HS, MINB, DEG, BW, GRP)                                              \
+    switch (rl.shape) {
+#define JPET_X(name, NWE, NG, NJA, NJB, HS, MINB, DEG, BW, CLS, GRP)                                         \
     case k_##name:                                                                                           \
         if constexpr (GRP == JPET_GROUP)                                                                     \
-            return rl.plan->vs ? launch_rows<NWE, NG, NJA, NJB, HS, MINB, DEG, BW, true>(rl)                 \
-                               : launch_rows<NWE, NG, NJA, NJB, HS, MINB, DEG, BW, false>(rl);               \
+            return rl.plan->vs ? launch_rows<NWE, NG, NJA, NJB, HS, MINB, DEG, BW, true, CLS != 0>(rl)       \
+                               : launch_rows<NWE, NG, NJA, NJB, HS, MINB, DEG, BW, false, CLS != 0>(rl);     \
         else return -100;
         JPET_SHAPES(JPET_X)
 #undef JPET_X

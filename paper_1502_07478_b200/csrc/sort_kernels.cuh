@@ -14,7 +14,8 @@
 namespace jpet {
 
 // Where an event goes in the sort, decided ONCE per event (bin_count_kernel) and carried to the scatter pass in one
-// word: the bin (sub-tile of the reconstructed point; nby * nbz = the "direct" bin for events that do not fit a region:
+// word: the bin (sub-tile of the reconstructed point, + nby * nbz for the events of degree class 1; n_cls * nby * nbz =
+// the "direct" bin for events that do not fit a region:
 // non-finite, |tan theta~| > t_max, centred outside the halo-extended image, or a row count the task table does not
 // hold) and the row range of the ellipse.  Not inlined: both sort kernels execute the same instructions, so the row
 // count that admitted an event to a regular bin is the one its record carries.
@@ -31,11 +32,13 @@ static __device__ __noinline__ Place event_place(float zu, float zd, float dl, c
     if (p.nr_max > 0) regular = regular && nrows >= p.nr_min && nrows <= p.nr_max;
     Place pl;
     pl.rows = pack_rows(iy_lo, min(nrows, 255));
-    pl.bin = p.nby * p.nbz;
+    const int nb = p.nby * p.nbz;
+    pl.bin = nb * p.n_cls;
     if (regular) {
         const int iyc = __float2int_rd(e.fy + 0.5f), izc = __float2int_rd(fz + 0.5f);
         const int by = min(max((iyc + p.Hy) / p.Sy, 0), p.nby - 1), bz = min(max((izc + p.Hz) / p.Sz, 0), p.nbz - 1);
         pl.bin = by * p.nbz + bz;
+        if (p.n_cls == 2 && low_degree_ok(e, p)) pl.bin += nb;       // degree class 1: the degree-3 instance
     }
     return pl;
 }
@@ -100,20 +103,26 @@ bin_count_kernel(const float* __restrict__ events, int n, const __grid_constant_
 // One block: exclusive prefix of counts -> starts (and cursors), work items for the regular bins.  Full items
 // (chunk events) come first in the list, the partly filled last item of every bin after them, so that the persistent
 // event kernel ends on small items.
-// meta[0] = number of items, meta[1] = start of the direct bin, meta[2] = its count, meta[3] = work counter (zeroed)
+// nb: regular bins of all degree classes, nb0: those of class 0 (the first nb0 bins).  meta: see MetaWord (common.cuh).
 __global__ void bin_scan_kernel(int* __restrict__ counts, int* __restrict__ cursors, WorkItem* __restrict__ items,
-                                int* __restrict__ meta, int nb, int chunk) {
+                                int* __restrict__ meta, int nb, int nb0, int chunk) {
     pdl_wait();
     __shared__ int s_ev[1024], s_it[1024], s_pt[1024];
+    __shared__ int s_full0, s_part0;
     const int tid = threadIdx.x, T = blockDim.x;
+    if (tid == 0) { s_full0 = 0; s_part0 = 0; }
+    __syncthreads();
     const int per = (nb + 1 + T - 1) / T;                  // bins per thread, contiguous
     const int b0 = tid * per, b1 = min(nb + 1, b0 + per);
-    int ev = 0, it = 0, pt = 0;
+    int ev = 0, it = 0, pt = 0, it0 = 0, pt0 = 0;
     for (int b = b0; b < b1; ++b) {
         int c = counts[b];
         ev += c;
         if (b < nb) { it += c / chunk; pt += (c % chunk) != 0; }
+        if (b < nb0) { it0 += c / chunk; pt0 += (c % chunk) != 0; }
     }
+    if (it0) atomicAdd(&s_full0, it0);
+    if (pt0) atomicAdd(&s_part0, pt0);
     s_ev[tid] = ev; s_it[tid] = it; s_pt[tid] = pt;
     __syncthreads();
     for (int d = 1; d < T; d <<= 1) {                      // Hillis-Steele inclusive scan
@@ -133,12 +142,19 @@ __global__ void bin_scan_kernel(int* __restrict__ counts, int* __restrict__ curs
             for (; k + chunk <= c; k += chunk) items[it_off++] = WorkItem{b, ev_off + k, chunk};
             if (k < c) items[pt_off++] = WorkItem{b, ev_off + k, c - k};
         } else {
-            meta[1] = ev_off;
-            meta[2] = c;
+            meta[kMetaDirectStart] = ev_off;
+            meta[kMetaDirectCount] = c;
         }
         ev_off += c;
     }
-    if (tid == T - 1) { meta[0] = s_it[tid] + s_pt[tid]; meta[3] = 0; }
+    if (tid == T - 1) {
+        meta[kMetaItems] = s_it[tid] + s_pt[tid];
+        meta[kMetaFull] = n_full;
+        meta[kMetaFull0] = s_full0;
+        meta[kMetaPart0] = s_part0;
+        meta[kMetaCounter0] = 0;
+        meta[kMetaCounter1] = 0;
+    }
 }
 
 // Scatter into bin order: ranks inside the block from a shared-memory histogram, one global cursor atomic per

@@ -156,7 +156,7 @@ def test_cfg1_ten_iterations(jp, oracle):
 
 
 # every shape of the list in csrc/rows_launch.h: the automatic plan can reach each of them
-N_SHAPES = 16
+N_SHAPES = 20
 
 
 def test_the_variant_tests_cover_the_whole_shape_list(jp):

@@ -20,13 +20,16 @@ def decode(entry):
     return {"row": entry & 0xFF, "part": (entry >> 8) & 3, "sh": (entry >> 10) & 3} if entry & VALID else None
 
 
-@pytest.mark.parametrize("name,shape,degree,warps", [("cfg1", "small_deg4", 4, 1), ("cfg2", "mid18_deg4", 4, 1), ("cfg3", "mid18_deg4", 4, 1),
-                                                     ("cfg4", "large_deg4", 4, 4), ("cfg5", "xl_deg4", 4, 4), ("fig4", "small_closed", 0, 1)])
-def test_plan_of_every_workload(name, shape, degree, warps):
-    """Shape and degree per workload, and the tiling identities the kernels rely on."""
+@pytest.mark.parametrize("name,shape,low,degree,warps", [("cfg1", "small_deg3", "", 3, 1), ("cfg2", "mid18_deg4", "mid18_deg3", 4, 1),
+                                                         ("cfg3", "mid18_deg3", "", 3, 1), ("cfg4", "large_deg4", "large_deg3", 4, 4),
+                                                         ("cfg5", "xl_deg4", "", 4, 4), ("fig4", "small_closed", "", 0, 1)])
+def test_plan_of_every_workload(name, shape, low, degree, warps):
+    """Shape and degree per workload - `low`: the degree-3 instance for the events whose own bound
+    allows it - and the tiling identities the kernels rely on."""
     cfg = synth.CONFIGS[name]
     p = plan_of(cfg)
     assert (jp.jpet_shape_name(p["variant"]), p["degree"], p["warps_per_event"], p["tiled"]) == (shape, degree, warps, 1)
+    assert jp.jpet_shape_name(p["variant_low"]) == low
     assert p["HS"] % 32 == 0 and p["HS"] >= 2 * p["Hy"] + 4          # region rows: bank-conflict-free stride, whole ellipse
     assert p["Sy"] == p["HS"] - 2 * p["Hy"] and p["WZ"] == p["Sz"] + 2 * p["Hz"]
     hy = 1.5 * cfg.sigma_dl / cfg.pixel
@@ -106,7 +109,7 @@ def test_degree_of_the_exponent_polynomial_keeps_the_truncation_small(name):
     Quadratic forms typed from Eq. 8-10 with the diagonal C^-1 (fp64)."""
     cfg = synth.CONFIGS[name]
     deg = plan_of(cfg)["degree"]
-    assert deg in (4, 5)
+    assert deg in (3, 4, 5)
     ev = synth.config_events(cfg, n=1500).astype(np.float64)
     R, iz2, il2, k = cfg.R, 1 / cfg.sigma_z**2, 1 / cfg.sigma_dl**2, 2.0
     y_lim = 0.5 * cfg.n_y * cfg.pixel
