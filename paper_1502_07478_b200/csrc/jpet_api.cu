@@ -377,14 +377,16 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
         const double xb = 2.0 * (t_max / (1.0 + t_max * t_max)) * y_max * u_max / (R2 + y_max * y_max) / (0.95 - g_rel - 2.0 * dls * y_max * g.R / (R2 + y_max * y_max));
         const double eb = 1.1 * std::pow(3.0 * y_max / std::sqrt(R2 + y_max * y_max) + g_ba, 2.0);
         // What has to be small is the error of a kernel value against the event's largest one (the image tolerance is
-        // relative to the image maximum).  At the fraction s = |u| / u_max of the central half chord |x| <= xb s, so the two
-        // neglected tails scale with s^(deg-1) and s^(deg+1); the kernel value there is at most exp(-q (1 - eb/9) / 2) of
-        // the peak (b.C^-1.a is linear in b, so ba^2 / D <= (eb / 9) q, and q = b.C^-1.b >= 9 s^2), times <= 1.05 for
-        // the D^-1/2 factor.  max over s in [0, 1] of s^n exp(-g s^2) is (n / (2 g e))^(n/2) when n <= 2 g, else exp(-g).
+        // relative to the image maximum).  At the fraction s = |u| / u_max of the central half chord |x| <= xb s; the tail
+        // of ba^2 / D is e_2 v^2 |x|^(deg-1) / (1 - |x|) with e_2 v^2 = (alpha v - x beta)^2 / delta <= eb s^2 (1 + xb)^2, the
+        // tail of ln D is |x|^(deg+1) / (deg + 1): both scale with s^(deg+1).  The kernel value there is at most
+        // exp(-q (1 - eb/9) / 2) of the peak (b.C^-1.a is linear in b, so ba^2 / D <= (eb / 9) q, and q = b.C^-1.b >= 9 s^2),
+        // times <= 1.05 for the D^-1/2 factor.  max over s in [0, 1] of s^n exp(-g s^2) is (n / (2 g e))^(n/2) when n <= 2 g,
+        // else exp(-g).  low_degree_ok (common.cuh) is the same bound for one event.
         const double gw = 4.5 * std::max(0.0, 1.0 - eb / 9.0);
         auto wmax = [&](int n) { return 1.05 * (n < 2.0 * gw ? std::pow(n / (2.0 * gw * std::exp(1.0)), 0.5 * n) : std::exp(-gw)); };
         auto trunc_err = [&](int deg) {      // log2 units, weighted by the kernel value relative to the event's peak
-            return 1.4427 * (0.5 * eb * std::pow(xb, deg - 1) / (1.0 - xb) * wmax(deg - 1) + 0.5 * std::pow(xb, deg + 1) / (deg + 1) * wmax(deg + 1));
+            return 1.4427 * wmax(deg + 1) * (0.5 * eb * (1.0 + xb) * (1.0 + xb) * std::pow(xb, deg - 1) / (1.0 - xb) + 0.5 * std::pow(xb, deg + 1) / (deg + 1));
         };
         // among the degrees that meet the bound (a higher degree is only more accurate): the first shape of each degree
         // that holds the workload's ellipses (the list is ordered by size within a degree), then the one with the fewest
