@@ -707,6 +707,26 @@ int ensure_host_path(Workspace& w, size_t stage_bytes) {
 // iterations (slot_used lives in the workspace, not in this call).
 int accumulate_from_host(Workspace& w, const float* events_host, int64_t n, int64_t chunk, bool fits) {
     cudaStream_t cs = w.copy_stream, ks = w.compute_stream;
+    if (fits) {
+        // resident events: upload and compute in batches that double from `chunk` up to the batch size of the device path -
+        // the first batch starts after one chunk has arrived, every later upload hides behind the previous batch's kernels,
+        // and most events are sorted and walked in full-size batches (config 5 through 2x10^6-event batches: 369 ms per
+        // iteration, 5 % over the device-resident 349 ms - five times as many partly filled work items)
+        int b = 0;
+        int64_t batch = chunk;
+        for (int64_t off = 0; off < n; ++b) {
+            const int64_t nb = std::min(batch, n - off);
+            float* dst = w.stage + 3 * off;
+            CUDA_TRY(cudaMemcpyAsync(dst, events_host + 3 * off, sizeof(float) * 3 * nb, cudaMemcpyHostToDevice, cs));
+            CUDA_TRY(cudaEventRecord(w.ev_copy[b & 1], cs));
+            CUDA_TRY(cudaStreamWaitEvent(ks, w.ev_copy[b & 1], 0));
+            int rc = do_accumulate(w, dst, nb, ks);
+            if (rc) return rc;
+            off += nb;
+            batch = std::min<int64_t>(2 * batch, kMaxBatch);
+        }
+        return JPET_OK;
+    }
     int c = 0;
     for (int64_t off = 0; off < n; off += chunk, ++c) {
         int64_t nb = std::min(chunk, n - off);
