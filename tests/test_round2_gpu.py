@@ -349,3 +349,26 @@ def test_two_processes_share_accumulators_through_cuda_ipc(jp, oracle):
     cfg = synth.CONFIGS["cfg2"]
     want, _, _ = oracle.reconstruct(synth.config_events(cfg, n=n_events), *geom(cfg), n_iter)
     assert rel_err(got[0][3].astype(np.float64), want) <= 1e-4
+
+
+# ---- degree classes: the events whose own truncation bound allows it are walked with the degree-3 exponent polynomial ----
+@pytest.mark.parametrize("name,n,low", [("cfg4", 120_000, "large_deg3"), ("cfg2", 150_000, "mid18_deg3"), ("cfg5", 60_000, "")])
+def test_degree_classes_do_not_change_the_image(jp, oracle, name, n, low):
+    """with a degree-4 plan the sort puts the events that pass low_degree_ok into a second set of bins and
+    the degree-3 instance of the kernel shape walks them.  Same image as with one class (the truncation error is far below
+    fp32 summation noise), same counters, and both match the oracle; config 5's shape has no degree-3 instance."""
+    cfg = synth.CONFIGS[name]
+    ev = synth.config_events(cfg, n=n)
+    rho = np.random.default_rng(7).uniform(0.5, 2.0, (cfg.n_y, cfg.n_z)).astype(np.float32)
+    got, (ne, ns) = gpu_iterate(jp, ev, cfg, rho)
+    assert jp.jpet_shape_name(jp.jpet_get_option("last_variant_low")) == low
+    jp.jpet_set_option("degree_classes_off", 1)
+    try:
+        one, (ne1, ns1) = gpu_iterate(jp, ev, cfg, rho)
+        assert jp.jpet_get_option("last_variant_low") == -1
+    finally:
+        jp.jpet_set_option("degree_classes_off", 0)
+    want, one_evals, one_skipped = oracle.mlem_iterate(ev, *geom(cfg), rho)
+    assert (ne, ns) == (ne1, ns1) and ns == one_skipped and abs(ne - one_evals) <= 1e-5 * one_evals + 2
+    assert np.max(np.abs(got - one)) <= 5e-6 * one.max()
+    assert rel_err(got, want) <= TOL_1 and rel_err(one, want) <= TOL_1
