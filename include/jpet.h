@@ -174,7 +174,7 @@ int jpet_ipc_open(const void *handle64, void **dev_ptr_out);
 int jpet_ipc_close(void *dev_ptr);
 
 /* Tuning knobs (do not change results beyond fp32 summation order).  name/value pairs:
- *   "variant"      event-kernel shape id (index into the shape list of csrc/jpet_api.cu, see DESIGN.md "Kernels";
+ *   "variant"      event-kernel shape id (index into the shape list JPET_SHAPES of csrc/rows_launch.h, see DESIGN.md section 6;
  *                  jpet_plan_describe reports it); -1 = automatic
  *   "force_direct" 1 = skip the shared-memory tiled path: every event goes through the direct kernel
  *                  (w from global memory, red.global.add into the image); 0 = automatic

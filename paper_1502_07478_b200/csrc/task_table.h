@@ -1,4 +1,4 @@
-// task_table.h - host side: which piece of which ellipse row each lane of an event group walks (mlem_rows3.cuh).
+// task_table.h - host side: which piece of which ellipse row each lane of an event group walks (mlem_rows.cuh).
 //
 // The 3-sigma ellipse of an event (App. B :251-267) has half height hy = 1.5 sigma_dl cos(theta~)
 // and, on the image row at signed distance d from its centre, a chord of half length sqrt(H0 (1 - (d/hy)^2)),
