@@ -78,6 +78,31 @@ int jpet_reconstruct(const float *events_dev, int64_t n, const jpet_geometry *ge
                      const jpet_grid *grid, const float *rho_init_dev, float *rho_out_dev, int32_t n_iter,
                      void *cuda_stream);
 
+/* jpet_mlem_iterate for callers that cannot allocate device memory when they need an iteration.
+ * Who that is: a loop with a latency budget (detector monitoring during acquisition) - cudaMalloc and cudaFree hold up
+ * every stream of the device while they run, and jpet_mlem_iterate grows its workspace on demand; a plug-in inside a
+ * program that has given all device memory to its own pool, where cudaMalloc just fails; a process that is not allowed
+ * driver allocations after start-up.  This call makes none: no cudaMalloc, cudaFree or allocating library routine, on
+ * any call.  Its scratch (s of Eq. 4, w = s rho, the accumulator, counters) is a fixed array of 3 MiB + 256 bytes compiled
+ * into the library; every GPU that loads the library holds that array until the process exits.
+ *   - Same arguments, result and skipping rules as jpet_mlem_iterate (Eq. 3, steps 1-4 above; a3 coefficient, gamma and
+ *     the sigma_z edge coefficient are honoured, tuning options and "exact_kernel" are not); the caller owns events and
+ *     both images, rho_out_dev may alias rho_in_dev; asynchronous on cuda_stream.
+ *   - Limits: n_y * n_z <= JPET_NOALLOC_MAX_PIXELS and n <= 2^31 - 1, else JPET_E_INVAL with the limit in the text.
+ *   - Every event takes the direct kernel (one warp per event, w read from global memory, red.global.add into the
+ *     accumulator) straight from events_dev, unsorted: the slow, simple path - expect a fraction of jpet_mlem_iterate's
+ *     rate.  The image differs from jpet_mlem_iterate's by fp32 summation order only.
+ *   - The first call on a device looks the array's device address up (cudaGetSymbolAddress) and reads the SM count; make
+ *     that first call on each device before any stream capture begins.
+ *   - All calls share the one array per device, and it keeps what the last call left in it; each call rewrites or zeroes
+ *     every part it reads, so calls one after another (same or different grids) are independent.  Two calls that overlap
+ *     on the GPU (different streams without an ordering between them, or two host threads) race on it: order them.
+ *     The array is separate from the workspace of the other calls, so those may run concurrently with this one;
+ *     jpet_get_counters does not see this call and jpet_release does not free the array. */
+#define JPET_NOALLOC_MAX_PIXELS (512 * 512)
+int jpet_mlem_iterate_noalloc(const float *events_dev, int64_t n, const jpet_geometry *geometry, const jpet_sigmas *sigmas,
+                              const jpet_grid *grid, const float *rho_in_dev, float *rho_out_dev, void *cuda_stream);
+
 /* The same iteration split in three so that a caller can stream event batches (BASELINE config 5):
  *   begin      : w = s * rho_in, accumulators and counters zeroed
  *   accumulate : steps 1-3 for one batch of events (device pointer); any number of calls

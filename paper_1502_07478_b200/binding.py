@@ -14,7 +14,7 @@ JPET_OK, JPET_E_INVAL, JPET_E_CUDA, JPET_E_INTERNAL = 0, -1, -2, -3
 JPET_MAX_PEERS = 16
 
 EXPORTS = (
-    "jpet_sensitivity", "jpet_mlem_iterate", "jpet_reconstruct", "jpet_mlem_begin", "jpet_mlem_accumulate",
+    "jpet_sensitivity", "jpet_mlem_iterate", "jpet_mlem_iterate_noalloc", "jpet_reconstruct", "jpet_mlem_begin", "jpet_mlem_accumulate",
     "jpet_mlem_end", "jpet_mlem_iterate_host", "jpet_reconstruct_host", "jpet_get_counters", "jpet_count_evals",
     "jpet_set_a3_coef", "jpet_get_a3_coef", "jpet_set_gamma", "jpet_get_gamma", "jpet_set_sigma_z_edge", "jpet_get_sigma_z_edge",
     "jpet_direct_histogram", "jpet_generate_events", "jpet_mlem_accumulator", "jpet_mlem_end_peers", "jpet_ipc_export",
@@ -69,6 +69,7 @@ def load(build_if_missing: bool = True) -> ctypes.CDLL:
     sigs = {
         "jpet_sensitivity": (ctypes.c_int, [G, Gr, p, p]),
         "jpet_mlem_iterate": (ctypes.c_int, [p, i64, G, S, Gr, p, p, p]),
+        "jpet_mlem_iterate_noalloc": (ctypes.c_int, [p, i64, G, S, Gr, p, p, p]),
         "jpet_reconstruct": (ctypes.c_int, [p, i64, G, S, Gr, p, p, i32, p]),
         "jpet_mlem_begin": (ctypes.c_int, [G, S, Gr, p, p]),
         "jpet_mlem_accumulate": (ctypes.c_int, [p, i64, p]),
@@ -161,6 +162,21 @@ def jpet_mlem_iterate(events_dev, R, L, sigma_z, sigma_dl, n_y, n_z, pixel, rho_
     ev, n = _events_ptr(events_dev, True)
     _check(load().jpet_mlem_iterate(ev, n, g, s, gr, _dev_f32(rho_in_dev, n_y * n_z, "rho_in_dev"),
                                     _dev_f32(rho_out_dev, n_y * n_z, "rho_out_dev"), _stream_handle(stream)))
+    return rho_out_dev
+
+
+NOALLOC_MAX_PIXELS = 512 * 512      # JPET_NOALLOC_MAX_PIXELS of include/jpet.h
+
+
+def jpet_mlem_iterate_noalloc(events_dev, R, L, sigma_z, sigma_dl, n_y, n_z, pixel, rho_in_dev, rho_out_dev, stream=None):
+    """jpet_mlem_iterate for callers that cannot allocate device memory when the iteration is due (a loop with a latency
+    budget, a host program whose pool owns all of HBM, a no-allocation-after-start-up rule): the library's scratch is a
+    fixed array compiled into it, so the call never reaches cudaMalloc. Images of up to NOALLOC_MAX_PIXELS pixels; the
+    slow direct kernel; calls share the scratch, so do not let two of them overlap on the GPU. See include/jpet.h."""
+    g, s, gr = _structs(R, L, sigma_z, sigma_dl, n_y, n_z, pixel)
+    ev, n = _events_ptr(events_dev, True)
+    _check(load().jpet_mlem_iterate_noalloc(ev, n, g, s, gr, _dev_f32(rho_in_dev, n_y * n_z, "rho_in_dev"),
+                                            _dev_f32(rho_out_dev, n_y * n_z, "rho_out_dev"), _stream_handle(stream)))
     return rho_out_dev
 
 

@@ -860,6 +860,50 @@ int jpet_mlem_accumulate(const float* events_dev, int64_t n_batch, void* cuda_st
     if ((rc = do_accumulate(*w, events_dev, n_batch, st))) return rc;
     return leave(*w, st);
 }
+// ---- jpet_mlem_iterate_noalloc: one iteration whose scratch is a fixed array inside the library image ------------------
+// Some users of this library must not, or cannot, allocate device memory at the moment they need an iteration: an
+// acquisition or monitoring loop with a latency budget (cudaMalloc / cudaFree stall every stream of the device while they
+// run), a plug-in inside a host program that has handed all of HBM to its own pool (cudaMalloc then simply fails), a
+// process whose rules forbid driver allocations after start-up.  For them the three scratch images of an iteration
+// (s of Eq. 4, w = s rho, the back-projection accumulator), the counters and the meta words of the direct event kernel
+// live in the array below.  It is part of the loaded library: every GPU on which the library's kernels get loaded keeps
+// its own 3 MiB copy until the process exits, whether or not the entry point is ever called.
+constexpr int kNoAllocMaxPixels = JPET_NOALLOC_MAX_PIXELS;
+constexpr size_t kNoAllocImageBytes = sizeof(float) * (size_t)kNoAllocMaxPixels;      // 1 MiB: keeps every part 256-aligned
+constexpr size_t kNoAllocCountersAt = 3 * kNoAllocImageBytes;                          // 4 x unsigned long long
+constexpr size_t kNoAllocMetaAt = kNoAllocCountersAt + 64;                             // kMetaWords x int
+constexpr size_t kNoAllocBytes = kNoAllocCountersAt + 256;
+static_assert(kNoAllocMetaAt + sizeof(int) * jpet::kMetaWords <= kNoAllocBytes, "scratch tail too small");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+// In host code `g_noalloc_scratch` is only a handle for the runtime, not an address a kernel could use: the device
+// address is asked for once per device, with that device current, and remembered.
+struct NoAllocDevice { unsigned char* base = nullptr; int sm_count = 0; };
+std::map<int, NoAllocDevice> g_noalloc_dev;
+
+int noalloc_device(NoAllocDevice* out) {
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    auto it = g_noalloc_dev.find(dev);
+    if (it == g_noalloc_dev.end()) {
+        NoAllocDevice d;
+        void* ptr = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&ptr, g_noalloc_scratch));
+        if (!ptr) return fail(JPET_E_CUDA, "cudaGetSymbolAddress gave no address for the static scratch on device %d", dev);
+        d.base = static_cast<unsigned char*>(ptr);
+        CUDA_TRY(cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev));
+        it = g_noalloc_dev.emplace(dev, d).first;
+    }
+    *out = it->second;
+    return JPET_OK;
+}
+
+// meta words of a "sorted batch" that is simply the caller's event array: the direct bin is all of it
+__global__ void noalloc_meta_kernel(int* __restrict__ meta, int n) {
+    const int i = threadIdx.x;
+    if (i < jpet::kMetaWords) meta[i] = i == jpet::kMetaDirectCount ? n : 0;
+}
+
 
 int jpet_mlem_end(const float* rho_in_dev, float* rho_out_dev, void* cuda_stream) {
     g_err.clear();
@@ -1263,3 +1307,43 @@ const char* jpet_shape_name(int32_t shape) { return shape >= 0 && shape < kNumSh
 int jpet_abi_version(void) { return JPET_ABI_VERSION; }
 
 }  // extern "C"
+int jpet_mlem_iterate_noalloc(const float* events_dev, int64_t n, const jpet_geometry* geometry, const jpet_sigmas* sigmas,
+                              const jpet_grid* grid, const float* rho_in_dev, float* rho_out_dev, void* cuda_stream) {
+    g_err.clear();
+    int rc = validate(geometry, sigmas, grid);
+    if (rc) return rc;
+    if (!sigmas) return fail(JPET_E_INVAL, "NULL sigmas");
+    if (n < 0 || (n > 0 && !events_dev)) return fail(JPET_E_INVAL, "bad events");
+    if (n > 0x7fffffffll) return fail(JPET_E_INVAL, "jpet_mlem_iterate_noalloc takes at most 2^31 - 1 events per call");
+    if (!rho_in_dev || !rho_out_dev) return fail(JPET_E_INVAL, "NULL image pointer");
+    const int64_t M64 = (int64_t)grid->n_y * grid->n_z;
+    if (M64 > kNoAllocMaxPixels)
+        return fail(JPET_E_INVAL, "jpet_mlem_iterate_noalloc: an image of %d x %d = %lld pixels does not fit the static scratch "
+                    "(JPET_NOALLOC_MAX_PIXELS = %d); use jpet_mlem_iterate, which allocates its workspace", grid->n_y, grid->n_z,
+                    (long long)M64, kNoAllocMaxPixels);
+    NoAllocDevice d;
+    if ((rc = noalloc_device(&d))) return rc;        // first call on this device: cudaGetSymbolAddress + one attribute query
+    const int M = (int)M64;
+    float* s = reinterpret_cast<float*>(d.base);
+    float* wT = reinterpret_cast<float*>(d.base + kNoAllocImageBytes);
+    float* accT = reinterpret_cast<float*>(d.base + 2 * kNoAllocImageBytes);
+    unsigned long long* counters = reinterpret_cast<unsigned long long*>(d.base + kNoAllocCountersAt);
+    int* meta = reinterpret_cast<int*>(d.base + kNoAllocMetaAt);
+    jpet_host::RowsPlan plan;
+    make_plan(*geometry, *sigmas, *grid, &plan);     // host arithmetic only: the constants of Eq. 7-12 in plan.dp
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // the array keeps what the previous call left: s and w are rewritten in full for this grid, the accumulator and the
+    // counters are zeroed by the pre-pass, the meta words are rewritten
+    jpet::sensitivity_kernel<<<grid_for(M), 256, 0, st>>>(s, grid->n_y, grid->n_z, grid->pixel, geometry->R, geometry->L);
+    jpet::prepass_kernel<<<grid_for(M), 256, 0, st>>>(s, rho_in_dev, wT, accT, grid->n_y, grid->n_z, counters);
+    noalloc_meta_kernel<<<1, 32, 0, st>>>(meta, (int)n);
+    jpet::mlem_rows_direct_kernel<false><<<d.sm_count * 16, 128, 0, st>>>(events_dev, 3, meta, plan.dp, wT, accT, counters, 0);
+    jpet::PeerAcc pa{};
+    pa.acc[0] = accT;
+    pa.n = 1;
+    jpet::finalise_kernel<<<grid_for(M), 256, 0, st>>>(s, rho_in_dev, pa, rho_out_dev, grid->n_y, grid->n_z);
+    g_launches += 5;
+    CUDA_TRY(cudaGetLastError());
+    return JPET_OK;
+}
+
