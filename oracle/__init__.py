@@ -83,6 +83,8 @@ def _load():
     lib.jo_get_exact_kernel.argtypes = []
     lib.jo_direct_histogram.restype = ctypes.c_uint64
     lib.jo_direct_histogram.argtypes = [p, i64, d, i, i, d, p]
+    lib.jo_direct_pixel_coords.restype = None
+    lib.jo_direct_pixel_coords.argtypes = [p, i64, d, i, i, d, p]
     lib.jo_generate_events.restype = i
     lib.jo_generate_events.argtypes = [p, i, i64, i64, d, d, d, d, ctypes.c_uint64, p]
     lib.jo_kernel_exact_events.restype = None
@@ -175,6 +177,15 @@ def direct_histogram(events, R, n_y, n_z, pixel, hist=None):
     assert h.dtype == np.uint32 and h.flags.c_contiguous and h.size == n_y * n_z
     out = _load().jo_direct_histogram(ev.ctypes.data, ev.shape[0], R, n_y, n_z, pixel, h.ctypes.data)
     return h, int(out)
+
+
+def direct_pixel_coords(events, R, n_y, n_z, pixel) -> np.ndarray:
+    """Eq. 2 in fp64: (c_y, c_z) of every event in pixels from the lower edge of the grid, float64 [n, 2]; the event lies in
+    pixel (floor c_y, floor c_z). NaN for events with a non-finite component."""
+    ev = _events_f32(events)
+    out = np.empty((ev.shape[0], 2), dtype=np.float64)
+    _load().jo_direct_pixel_coords(ev.ctypes.data, ev.shape[0], R, n_y, n_z, pixel, out.ctypes.data)
+    return out
 
 
 def generate_events(phantom, n, R, L, sigma_z, sigma_dl, seed, first=0) -> np.ndarray:

@@ -410,29 +410,35 @@ int jo_num_threads(void)
 }
 
 /* ---- direct reconstruction (Eq. 2; Fig. 4b): histogram of the reconstructed points ------------------
- * Every event is reconstructed to (y~, z~) with Eq. 2 and counted in the pixel that contains the point; pixel
- * (iy, iz) covers [y_c - pixel/2, y_c + pixel/2) x [z_c - pixel/2, z_c + pixel/2).  The pixel index is an integer
- * decided by floating point, so both sides take that decision in the SAME precision, the kernel's: IEEE binary32,
- * round to nearest, in the order written in include/jpet.h / DESIGN.md section 6 (this file is compiled with
- * -ffp-contract=off, so the only fused operations are the fmaf calls written here):
- *     t = (z_u - z_d) * inv2R,  sec = sqrt(fma(t, t, 1)),  y~ = (-0.5 dl) / sec,  z~ = fma(y~, t, 0.5 (z_u + z_d)),
- *     iy = floor(fma(y~, inv_px, oy)),  oy = (n_y - 1) / 2 + 1/2   (likewise iz)
- * with inv2R = fp32(1 / (2 R)), inv_px = fp32(1 / pixel).  hist (uint32 [n_y*n_z]) is INCREMENTED.
- * Returns the number of events outside the grid (or with a non-finite component).                           */
+ * Every event is reconstructed to (y~, z~) with Eq. 2 (jo_eq2, fp64) and counted in the pixel that contains the point.
+ * Pixel (iy, iz) covers [y_c - pixel/2, y_c + pixel/2) x [z_c - pixel/2, z_c + pixel/2) around its centre (y_c, z_c) of the
+ * grid convention above, so in units of pixels from the lower edge of the grid the point has the coordinates
+ *     c_y = y~ / pixel + n_y / 2,     c_z = z~ / pixel + n_z / 2
+ * and lies in pixel (floor(c_y), floor(c_z)) when 0 <= c_y < n_y and 0 <= c_z < n_z; otherwise (or when a component of
+ * the event is not finite) it is outside.  Nothing else: no precision is matched to any other implementation.  An fp32
+ * implementation decides the same pixel except for points that lie within its rounding error of a pixel border; tests
+ * that compare one with this function read the border distance from jo_direct_pixel_coords.
+ * jo_direct_pixel_coords: coords[2 j] = c_y, coords[2 j + 1] = c_z of event j (NaN for a non-finite event).
+ * jo_direct_histogram: hist (uint32 [n_y*n_z]) is INCREMENTED; returns the number of events outside.              */
+void jo_direct_pixel_coords(const float *events, int64_t n, double R, int n_y, int n_z, double pixel, double *coords)
+{
+    for (int64_t j = 0; j < n; ++j) {
+        double e[3];
+        jo_eq2((double)events[3 * j + 0], (double)events[3 * j + 1], (double)events[3 * j + 2], R, e);
+        const int finite = isfinite(e[0]) && isfinite(e[1]) && isfinite(e[2]);
+        coords[2 * j + 0] = finite ? e[1] / pixel + 0.5 * (double)n_y : NAN;
+        coords[2 * j + 1] = finite ? e[2] / pixel + 0.5 * (double)n_z : NAN;
+    }
+}
+
 uint64_t jo_direct_histogram(const float *events, int64_t n, double R, int n_y, int n_z, double pixel, uint32_t *hist)
 {
-    const float inv2R = (float)(1.0 / (2.0 * (double)(float)R)), inv_px = (float)(1.0 / (double)(float)pixel);
-    const float oy = (float)(0.5 * (n_y - 1) + 0.5), oz = (float)(0.5 * (n_z - 1) + 0.5);
     uint64_t outside = 0;
     for (int64_t j = 0; j < n; ++j) {
-        const float zu = events[3 * j + 0], zd = events[3 * j + 1], dl = events[3 * j + 2];
-        const float t = (zu - zd) * inv2R;
-        const float sec = sqrtf(fmaf(t, t, 1.0f));
-        const float y_t = (-0.5f * dl) / sec;
-        const float z_t = fmaf(y_t, t, 0.5f * (zu + zd));
-        const float fy = floorf(fmaf(y_t, inv_px, oy)), fz = floorf(fmaf(z_t, inv_px, oz));
-        if (!(fy >= 0.0f && fy < (float)n_y && fz >= 0.0f && fz < (float)n_z)) { outside++; continue; }
-        hist[(size_t)(int)fy * (size_t)n_z + (size_t)(int)fz] += 1u;
+        double c[2];
+        jo_direct_pixel_coords(events + 3 * j, 1, R, n_y, n_z, pixel, c);
+        if (!(c[0] >= 0.0 && c[0] < (double)n_y && c[1] >= 0.0 && c[1] < (double)n_z)) { outside++; continue; }   /* NaN: outside */
+        hist[(size_t)floor(c[0]) * (size_t)n_z + (size_t)floor(c[1])] += 1u;
     }
     return outside;
 }

@@ -227,7 +227,7 @@ def test_mlem_in_exact_mode_uses_the_integral(oracle):
 # ------------------------------------------------------------------------------------------------------
 def test_direct_histogram_puts_noise_free_events_into_the_emitting_pixel(oracle):
     """Eq. 2 inverts Eq. 1, so an unsmeared event is counted in the pixel that contains its emission
-    point (points within 1e-3 pixel of a pixel border are left out: fp32)."""
+    point (points within 1e-3 pixel of a pixel border are left out: the events are rounded to fp32)."""
     cfg = synth.CONFIGS["fig4"]
     ev, truth = synth.noise_free_events(20000, cfg.R, cfg.L, seed=3, y_max=0.45 * cfg.n_y * cfg.pixel)
     fy = truth[:, 0] / cfg.pixel + 0.5 * (cfg.n_y - 1) + 0.5
@@ -239,6 +239,33 @@ def test_direct_histogram_puts_noise_free_events_into_the_emitting_pixel(oracle)
     got, outside = oracle.direct_histogram(ev[safe].astype(np.float32), cfg.R, cfg.n_y, cfg.n_z, cfg.pixel)
     assert (got == want).all() and outside == int((safe & ~inside).sum())
     assert int(got.sum()) + outside == int(safe.sum())
+
+
+def test_direct_pixel_coords_invert_the_forward_model(oracle):
+    """jo_direct_pixel_coords is Eq. 2 in fp64 plus the grid convention: for unsmeared events of the forward model (synth:
+    Eq. 1 and the strip geometry, no Eq. 2) it returns the emission point in pixels from the lower grid edge - up to the
+    rounding of the events to fp32 (|z| <= 250 mm, |dl| <= 600 mm: <= 3e-5 mm, 1e-5 pixel of 4 mm) - and the histogram is
+    its floor; a wrong sign, a swapped axis or a half-pixel shift fail here."""
+    from types import SimpleNamespace
+
+    fig4 = synth.CONFIGS["fig4"]
+    cfg = SimpleNamespace(R=fig4.R, L=fig4.L, n_y=25, n_z=40, pixel=4.0)   # smaller than the emission region: some points fall outside
+    ev, truth = synth.noise_free_events(5000, cfg.R, cfg.L, seed=9, y_max=0.45 * fig4.n_y * fig4.pixel)
+    ev32 = ev.astype(np.float32)
+    c = oracle.direct_pixel_coords(ev32, cfg.R, cfg.n_y, cfg.n_z, cfg.pixel)
+    ys = (np.arange(cfg.n_y) - 0.5 * (cfg.n_y - 1)) * cfg.pixel          # pixel centres as the header defines them
+    zs = (np.arange(cfg.n_z) - 0.5 * (cfg.n_z - 1)) * cfg.pixel
+    want_y = (truth[:, 0] - (ys[0] - 0.5 * cfg.pixel)) / cfg.pixel       # distance from the lower edge of pixel row 0
+    want_z = (truth[:, 1] - (zs[0] - 0.5 * cfg.pixel)) / cfg.pixel
+    assert np.max(np.abs(c[:, 0] - want_y)) < 2e-5 and np.max(np.abs(c[:, 1] - want_z)) < 2e-5
+    inside = (c[:, 0] >= 0) & (c[:, 0] < cfg.n_y) & (c[:, 1] >= 0) & (c[:, 1] < cfg.n_z)
+    assert 0.1 * len(c) < inside.sum() < 0.9 * len(c)                    # both cases occur
+    want = np.zeros((cfg.n_y, cfg.n_z), dtype=np.uint32)
+    np.add.at(want, (np.floor(c[inside, 0]).astype(int), np.floor(c[inside, 1]).astype(int)), 1)
+    got, outside = oracle.direct_histogram(ev32, cfg.R, cfg.n_y, cfg.n_z, cfg.pixel)
+    assert (got == want).all() and outside == int((~inside).sum())
+    bad = np.array([[np.nan, 0, 0], [0, np.inf, 0], [0, 0, -np.inf]], dtype=np.float32)
+    assert np.isnan(oracle.direct_pixel_coords(bad, cfg.R, cfg.n_y, cfg.n_z, cfg.pixel)).all()
 
 
 def test_direct_histogram_conventions(oracle):
