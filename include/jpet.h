@@ -204,7 +204,9 @@ int jpet_ipc_close(void *dev_ptr);
  *   "force_direct" 1 = skip the shared-memory tiled path: every event goes through the direct kernel
  *                  (w from global memory, red.global.add into the image); 0 = automatic
  *   "chunk"        events per work item of the tiled path; 0 = automatic
- *   "sub_tile_z"   width in pixels of the image sub-tiles the events are sorted by; 0 = automatic
+ *   "sub_tile_z"   width in pixels of the image sub-tiles the events are sorted by; 0 = automatic.  A forced width whose
+ *                  regions do not fit shared memory is not replaced by another: every event then takes the direct kernel
+ *                  ("last_tiled" reads 0)
  *   "ctas_per_sm"  cap on resident CTAs per SM for the persistent grid; 0 = automatic
  *   "poly_off"     1 = never evaluate the exponent of Eq. 7 as a polynomial in u (always rsqrt + ex2); 0 = automatic:
  *                  the plan bounds the truncation error and picks degree 3, 4, 5 or the closed form

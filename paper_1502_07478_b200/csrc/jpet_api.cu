@@ -374,7 +374,10 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
         const double ag = std::fabs((double)gamma);
         const double g_rel = 2.0 * ag * std::fabs((double)a3) * y_max * szm * szm * (t_max / std::sqrt(1.0 + t_max * t_max)) / g.R;
         const double g_ba = 6.0 / std::sqrt(2.0) * ag * szm * sg.sigma_dl;
-        const double xb = 2.0 * (t_max / (1.0 + t_max * t_max)) * y_max * u_max / (R2 + y_max * y_max) / (0.95 - g_rel - 2.0 * dls * y_max * g.R / (R2 + y_max * y_max));
+        // |t| / sec^2 = |t| / (1 + t^2) grows up to |t| = 1, where it is 1/2, and falls beyond: its largest value over
+        // |t| <= t_max is at t_max only while t_max < 1 (strips longer than 2 R reach |t| = 1)
+        const double tf = t_max < 1.0 ? t_max / (1.0 + t_max * t_max) : 0.5;
+        const double xb = 2.0 * tf * y_max * u_max / (R2 + y_max * y_max) / (0.95 - g_rel - 2.0 * dls * y_max * g.R / (R2 + y_max * y_max));
         const double eb = 1.1 * std::pow(3.0 * y_max / std::sqrt(R2 + y_max * y_max) + g_ba, 2.0);
         // What has to be small is the error of a kernel value against the event's largest one (the image tolerance is
         // relative to the image maximum).  At the fraction s = |u| / u_max of the central half chord |x| <= xb s; the tail
@@ -433,8 +436,8 @@ void make_plan(const jpet_geometry& g, const jpet_sigmas& sg, const jpet_grid& g
     const int cta_warps = c.NWE * c.NG;
     size_t smem = 0;
     {
-        int best_sz = 4;
-        size_t best_warps = 0;
+        int best_sz = g_opt.sz > 0 ? (int)g_opt.sz : 4;      // a forced width is never replaced: if its regions do not fit,
+        size_t best_warps = 0;                                //  smem > budget below sends every event to the direct kernel
         for (int sz : {8, 4}) {
             if (g_opt.sz > 0) sz = (int)g_opt.sz;
             const size_t need = n_regions * sizeof(float) * (size_t)p.HS * (sz + 2 * p.Hz) + tab_bytes;

@@ -99,22 +99,13 @@ def test_pieces_fit_their_register_slots(name):
     assert len(seen) >= (p["nr_max"] - p["nr_min"] + 1) // 2
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
-def test_degree_of_the_exponent_polynomial_keeps_the_truncation_small(name):
-    """DESIGN.md 6.3: along a row ln P = -1/2 (q - ba^2 / D) - 1/2 ln D with D = delta (1 + x) is expanded in x = eps u /
-    delta and cut after u^degree.  What the plan bounds is the error of a kernel value against the event's largest one
-    (the image tolerance is relative to the image maximum): the neglected terms, in log2 units, times P / P_peak.  The
-    plan's degree must keep that below its own bound (2e-5) everywhere in the 3-sigma ellipse - on its boundary, where x is
-    largest but P is e^-4.5 of the peak, and inside, where P is large but x small; one degree less must be worse.
-    Quadratic forms typed from Eq. 8-10 with the diagonal C^-1 (fp64)."""
-    cfg = synth.CONFIGS[name]
-    deg = plan_of(cfg)["degree"]
-    assert deg in (3, 4, 5)
-    ev = synth.config_events(cfg, n=1500).astype(np.float64)
+def worst_truncation(cfg, ev, degrees):
+    """max over sampled (event, row, pixel) of |series cut after u^d - exact| * P / P_peak in log2 units, for every d in
+    `degrees` (see the test below).  Quadratic forms typed from Eq. 8-10 with the diagonal C^-1 (fp64)."""
     R, iz2, il2, k = cfg.R, 1 / cfg.sigma_z**2, 1 / cfg.sigma_dl**2, 2.0
     y_lim = 0.5 * cfg.n_y * cfg.pixel
     rng = np.random.default_rng(4)
-    worst = {deg - 1: 0.0, deg: 0.0}
+    worst = {d: 0.0 for d in degrees}
     for zu, zd, dl in ev:
         t = (zu - zd) / (2 * R)
         sec2 = 1 + t * t
@@ -146,5 +137,54 @@ def test_degree_of_the_exponent_polynomial_keeps_the_truncation_small(name):
             series = -0.5 * np.log(delta) + sum((0.5 * e[n] + (0 if n == 0 else -0.5 * (-1) ** (n + 1) * kap**n / n)) * u**n
                                                 for n in range(d + 1))
             worst[d] = max(worst[d], float(np.max(np.abs(series - exact) * weight)) * 1.4427)
+    return worst
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+def test_degree_of_the_exponent_polynomial_keeps_the_truncation_small(name):
+    """DESIGN.md 6.3: along a row ln P = -1/2 (q - ba^2 / D) - 1/2 ln D with D = delta (1 + x) is expanded in x = eps u /
+    delta and cut after u^degree.  What the plan bounds is the error of a kernel value against the event's largest one
+    (the image tolerance is relative to the image maximum): the neglected terms, in log2 units, times P / P_peak.  The
+    plan's degree must keep that below its own bound (2e-5) everywhere in the 3-sigma ellipse - on its boundary, where x is
+    largest but P is e^-4.5 of the peak, and inside, where P is large but x small; one degree less must be worse."""
+    cfg = synth.CONFIGS[name]
+    deg = plan_of(cfg)["degree"]
+    assert deg in (3, 4, 5)
+    worst = worst_truncation(cfg, synth.config_events(cfg, n=1500).astype(np.float64), (deg - 1, deg))
     assert worst[deg] <= 2e-5, worst
     assert worst[deg - 1] > worst[deg]
+
+
+def test_truncation_bound_holds_when_the_strips_are_longer_than_2R():
+    """|x| = |eps u / delta| is proportional to |t| / (1 + t^2), which peaks at |t| = 1 - for L > 2 R the
+    largest tilt t_max = (L + 8 sigma_z) / (2 R) is beyond the peak, and a bound evaluated at t_max under-estimates x.
+    Brute force over unsmeared events of the forward model spanning all tilts (R = 100, L = 600: |t| up to 2.9): the degree
+    the plan picks must keep the weighted truncation below the plan's 2e-5, and one degree less must not (the geometry is
+    chosen at that edge: with the bound taken at t_max the plan picked degree 4, whose tail is 3e-5)."""
+    from types import SimpleNamespace
+
+    cfg = SimpleNamespace(R=100.0, L=600.0, n_y=60, n_z=240, pixel=2.5, sigma_z=6.0, sigma_dl=30.0)
+    deg = plan_of(cfg)["degree"]
+    ev, _ = synth.noise_free_events(3000, cfg.R, cfg.L, seed=1, y_max=0.5 * cfg.n_y * cfg.pixel)
+    assert np.max(np.abs(ev[:, 0] - ev[:, 1]) / (2 * cfg.R)) > 2.5 and np.min(np.abs(ev[:, 0] - ev[:, 1]) / (2 * cfg.R)) < 0.05
+    worst = worst_truncation(cfg, ev, (3, 4, 5))
+    assert deg in (0, 3, 4, 5)
+    if deg:
+        assert worst[deg] <= 2e-5, (deg, worst)
+    assert deg == 5 and worst[4] > 2e-5, (deg, worst)      # degree 4 is not enough here, degree 5 is (and has a shape that fits)
+
+
+def test_forced_sub_tile_width_that_does_not_fit_goes_direct():
+    """a forced "sub_tile_z" whose regions exceed shared memory used to be replaced silently by 4; now the
+    plan keeps the caller's width and sends every event to the direct kernel (tiled = 0); a width that fits is used."""
+    cfg = synth.CONFIGS["cfg5"]
+    try:
+        jp.jpet_set_option("sub_tile_z", 256)
+        p = plan_of(cfg)
+        assert p["tiled"] == 0 and p["smem_bytes"] == 0
+        jp.jpet_set_option("sub_tile_z", 4)
+        p = plan_of(cfg)
+        assert p["tiled"] == 1 and p["Sz"] == 4
+    finally:
+        jp.jpet_set_option("sub_tile_z", 0)
+    assert plan_of(cfg)["tiled"] == 1
