@@ -7,8 +7,11 @@ summed, and every rank runs the pointwise finalise.  Two ways to sum:
 
   "p2p"   the sum is fused into the finalise kernel: every rank maps its peers' accumulators once (cudaIpc handles
           exchanged through torch.distributed) and jpet_mlem_end_peers reads all of them over NVLink in rank order, so all
-          ranks get bit-identical images.  Two host barriers per iteration order the accumulators' life cycle (all
-          written before any is read; all read before any is zeroed again).
+          ranks get bit-identical images.  Two host-side collectives per iteration order the accumulators' life cycle:
+          an all-gather of the ranks' current handles once every accumulator is written (it is the "all written before any
+          is read" barrier, and it makes the decision to re-map a peer the same on every rank - a rank whose workspace was
+          re-allocated is seen by all the others, none waits alone in a collective), and a barrier after the finalise
+          (all read before any is zeroed again).  Scaling beyond one GPU is unmeasured.
   "nccl"  one in-place NCCL all-reduce (sum) of the accumulator view, then the plain jpet_mlem_end.
 
 This module only orchestrates calls of the C-ABI binding (or of another object with the same five methods: the
@@ -52,6 +55,18 @@ class _BindingEngine:
 
         torch.cuda.current_stream().synchronize()
 
+    def ipc_export(self, acc) -> bytes:
+        return self.jp.jpet_ipc_export(acc.data_ptr())
+
+    def ipc_open(self, handle: bytes):
+        return self.jp.jpet_ipc_open(handle)
+
+    def ipc_close(self, peer) -> None:
+        self.jp.jpet_ipc_close(peer)
+
+    def own_peer(self, acc):
+        return acc.data_ptr()
+
 
 class ShardedMlem:
     """One MLEM iteration (Eq. 3) over events sharded across the ranks of a torch.distributed process group."""
@@ -64,37 +79,37 @@ class ShardedMlem:
         self.rank = self.dist.get_rank() if self.dist else 0
         self.mode = mode
         self.engine = engine if engine is not None else _BindingEngine()
-        self._own_ptr = None          # device pointer of this rank's accumulator the peer mappings were made for
-        self._peers = None            # device pointers of all ranks' accumulators, in rank order (own one included)
-        self._opened = []
+        self._handles = None          # per rank: the handle its current mapping was opened from (own rank: exported)
+        self._peers = None            # all ranks' accumulators in rank order: own pointer, peer mappings
+        self._opened = {}             # rank -> mapping this process opened (and must close)
 
     # ---- peer mappings (p2p mode) ----------------------------------------------------------------------------------
-    def _map_peers(self, acc):
-        ptr = acc.data_ptr()
-        if self._peers is not None and ptr == self._own_ptr:
-            return
-        self.close()
-        import paper_1502_07478_b200 as jp
-
+    def _exchange_handles(self, acc):
+        """Collective, every iteration: all ranks publish the handle of their current accumulator; every rank re-opens
+        exactly the peers whose handle differs from the one its mapping came from.  Whether anything is re-mapped is thus
+        decided from data all ranks share - a rank whose workspace was released and re-allocated (another pointer, or the
+        same pointer with a new allocation behind it: the handle differs) cannot leave the others waiting in a collective
+        it never enters, and no stale mapping survives.  Called after this rank's accumulator is complete, it is also the
+        barrier before the peers' accumulators are read."""
+        e = self.engine
         handles = [None] * self.world
-        self.dist.all_gather_object(handles, jp.jpet_ipc_export(ptr))
+        self.dist.all_gather_object(handles, e.ipc_export(acc))
         peers = []
         for r, h in enumerate(handles):
             if r == self.rank:
-                peers.append(ptr)
-            else:
-                p = jp.jpet_ipc_open(h)
-                self._opened.append(p)
-                peers.append(p)
-        self._own_ptr, self._peers = ptr, peers
+                peers.append(e.own_peer(acc))
+                continue
+            if self._handles is None or self._handles[r] != h:
+                if r in self._opened:
+                    e.ipc_close(self._opened.pop(r))
+                self._opened[r] = e.ipc_open(h)
+            peers.append(self._opened[r])
+        self._handles, self._peers = handles, peers
 
     def close(self):
-        if self._opened:
-            import paper_1502_07478_b200 as jp
-
-            for p in self._opened:
-                jp.jpet_ipc_close(p)
-        self._opened, self._peers, self._own_ptr = [], None, None
+        for p in self._opened.values():
+            self.engine.ipc_close(p)
+        self._opened, self._peers, self._handles = {}, None, None
 
     # ---- the iteration ---------------------------------------------------------------------------------------------
     def iterate(self, events_shard, geom, rho_in, rho_out):
@@ -109,9 +124,8 @@ class ShardedMlem:
             self.dist.all_reduce(e.accumulator(), op=self.dist.ReduceOp.SUM)
             e.end(rho_in, rho_out)
         else:
-            self._map_peers(e.accumulator())
-            e.sync()
-            self.dist.barrier()               # every accumulator is complete
+            e.sync()                          # this rank's accumulator is complete ...
+            self._exchange_handles(e.accumulator())      # ... and, past this collective, so is every other rank's
             e.end_peers(rho_in, rho_out, self._peers)
             e.sync()
             self.dist.barrier()               # every rank has read every accumulator: the next begin may zero them

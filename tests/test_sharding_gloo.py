@@ -129,3 +129,82 @@ def test_single_rank_needs_no_process_group(oracle):
     out = sm.iterate(torch.from_numpy(events), geom, rho, torch.empty_like(rho))
     want, _, _ = oracle.mlem_iterate(events, *geom, np.ones((cfg.n_y, cfg.n_z)))
     assert np.max(np.abs(out.numpy().reshape(cfg.n_y, cfg.n_z) - want)) <= 1e-12 * want.max()
+
+
+# ---- p2p mode: the decision to re-map a peer is taken from data every rank has -------------------------
+class HandleEngine:
+    """Stand-in for the cudaIpc side of the p2p mode: a "handle" names (rank, allocation generation); opening one gives a
+    token.  Records what ShardedMlem opens, closes and passes to the finalise."""
+
+    def __init__(self, rank):
+        self.rank, self.generation, self.log, self.finalised_with = rank, 0, [], []
+
+    def begin(self, geom, rho_in):
+        pass
+
+    def accumulate(self, events):
+        pass
+
+    def accumulator(self):
+        return ("acc", self.rank, self.generation)
+
+    def sync(self):
+        pass
+
+    def ipc_export(self, acc):
+        return b"%d:%d" % (acc[1], acc[2])
+
+    def ipc_open(self, handle):
+        self.log.append(("open", handle))
+        return ("mapped", handle)
+
+    def ipc_close(self, peer):
+        self.log.append(("close", peer[1]))
+
+    def own_peer(self, acc):
+        return acc
+
+    def end_peers(self, rho_in, rho_out, peers):
+        self.finalised_with.append(list(peers))
+
+
+def _remap_worker(rank, world, port, q):
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+
+    from paper_1502_07478_b200.sharding import ShardedMlem
+
+    dist.init_process_group("gloo")
+    eng = HandleEngine(rank)
+    sm = ShardedMlem(dist, mode="p2p", engine=eng)
+    for it in range(4):
+        if it == 2 and rank == 1:
+            eng.generation = 1          # rank 1 alone lost its workspace (jpet_release, a grown grid) between iterations
+        sm.iterate(None, None, None, None)
+    sm.close()
+    dist.destroy_process_group()
+    q.put((rank, eng.log, eng.finalised_with))
+
+
+def test_p2p_remap_is_decided_collectively():
+    """Rank 1's accumulator is re-allocated after two iterations, rank 0's is not.  Both must keep entering the same
+    collectives (no hang), rank 0 must drop its stale mapping of rank 1 and open the new one exactly once, and rank 1 must
+    not re-open rank 0's."""
+    import torch.multiprocessing as mp
+
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_remap_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted((q.get(timeout=120) for _ in procs), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (_, log0, fin0), (_, log1, fin1) = got
+    assert log0 == [("open", b"1:0"), ("close", b"1:0"), ("open", b"1:1"), ("close", b"1:1")]
+    assert log1 == [("open", b"0:0"), ("close", b"0:0")]
+    assert fin0 == [[("acc", 0, 0), ("mapped", b"1:0")]] * 2 + [[("acc", 0, 0), ("mapped", b"1:1")]] * 2
+    assert fin1 == [[("mapped", b"0:0"), ("acc", 1, 0)]] * 2 + [[("mapped", b"0:0"), ("acc", 1, 1)]] * 2
