@@ -25,6 +25,7 @@ events, the accumulators are summed, every rank finalises); per-GPU work is fixe
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import statistics
@@ -256,9 +257,10 @@ def measure(dev: Device, ranks: Ranks, cfg, ev_d, steps, warmup, sharded=None):
         else:
             jp.jpet_mlem_iterate(ev_d, *g, src, dst)
 
+    if warmup + steps < 1:
+        raise ValueError("measure() needs at least one iteration (warmup + steps >= 1)")
     for i in range(warmup):
         iterate(rho[i & 1], rho[(i + 1) & 1])
-    n_evals, n_skipped = jp.jpet_get_counters()
     torch.cuda.synchronize()
     ranks.barrier()
     torch.cuda.synchronize()
@@ -279,6 +281,7 @@ def measure(dev: Device, ranks: Ranks, cfg, ev_d, steps, warmup, sharded=None):
     ranks.barrier()
     torch.cuda.synchronize()
     launches = jp.jpet_launch_count() - launches0
+    n_evals, n_skipped = jp.jpet_get_counters()                       # of the last iteration run (every iteration counts the same)
     kernel_launches = jp.jpet_get_option("last_kernel_launches")      # event-kernel launches per step (one per batch)
     jp.jpet_set_option("time_kernel", 0)
     step_ms = [a.elapsed_time(d) for a, d in pairs]
@@ -321,7 +324,11 @@ def roofline_of(dev: Device, cfg, n_events, m, peaks, peak_kind):
             "peak_source": f"{dev.n_sm} SMs x 16 MUFU/clk / 2 MUFU per eval (algorithmic, SURVEY.md 8(d)) x {sm_mhz:.0f} MHz ({peak_kind} sm_max_mhz)",
             "bounds": bounds, "binding_bound": "shared_memory_12_B_per_eval" if peak_smem < peak_run else "sfu_as_run",
             "frac_of_binding_bound": achieved / binding,
-            "traffic": measured, "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r2_traffic.json)",
+            "traffic": measured, "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
+            "traffic_source": "profiles/r2_traffic.json: an ncu --set full capture of commit a2db65d, NOT re-measured by this run; "
+                              "null when csrc/mlem_rows.cuh has changed since that capture",
+            "bound_note": "bound / peak / frac are the ALGORITHMIC SFU roofline of SURVEY.md 8(d) (2 MUFU per evaluation), kept so "
+                          "that rounds stay comparable; what limits the kernel as it runs is binding_bound / frac_of_binding_bound",
             "traffic_model": model, "traffic_model_note": "64 B record read per event + 8 B per pixel; the shared-memory regions move "
             f"{l2_model / 1e6:.0f} MB per launch through L2",
             "algorithmic_bytes": algorithmic, "traffic_over_algorithmic": (measured or model) / algorithmic,
@@ -343,7 +350,12 @@ def ncu_traffic(name, n_events, batches):
     bytes per event of one launch, measured; null when the workload has no capture)."""
     path = os.path.join(ROOT, "profiles", "r2_traffic.json")
     try:
-        per_event = json.load(open(path))["dram_bytes_per_event"].get(name)
+        rec = json.load(open(path))
+        per_event = rec["dram_bytes_per_event"].get(name)
+        # a profiler figure read from a committed file, not measured by this run: only valid for the kernel it was taken on
+        src = open(os.path.join(ROOT, rec["kernel_source"]), "rb").read()
+        if hashlib.sha256(src).hexdigest()[:16] != rec["kernel_source_sha256_16"]:
+            return None
     except Exception:
         return None
     return None if per_event is None else per_event * n_events / batches
