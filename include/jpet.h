@@ -166,7 +166,10 @@ int jpet_direct_histogram(const float *events_dev, int64_t n, const jpet_geometr
 
 /* Event simulation on the device (the recipe of DESIGN.md section 5, phantom rule
  * PAPER.md:245): event slot i = first + k (k = 0..n-1) is drawn from its own counter-based random stream
- * Philox4x32-10(key = seed, counter = (slot, attempt, 0, 0)): attempt a = 0, 1, ... draws (y, z) uniform in the
+ * Philox4x32-10(key = (seed low word, seed high word), counter = (slot low word, slot high word, attempt, block)); a 32-bit
+ * output word x becomes the uniform ((x >> 8) + 0.5) 2^-24.  Block 0 of an attempt gives (u0, u1, u2, u3): position, the
+ * acceptance draw and the angle; block 1 of the accepted attempt gives the four uniforms of the two Box-Muller pairs
+ * (csrc/generator.cuh has the exact order).  Attempt a = 0, 1, ... draws (y, z) uniform in the
  * phantom's bounding rectangle, accepts it with probability intensity / max intensity (first primitive in the list
  * wins), draws theta uniform on (-pi/2, pi/2), keeps the emission if both strips are hit, and smears
  * (z_u, z_d, dl) with N(0, sigma_z), N(0, sigma_z), N(0, sigma_dl) (Box-Muller).  Slot i is therefore the same event

@@ -231,7 +231,7 @@ __device__ __forceinline__ void walk_pair(Walk& s, float& p0, float& p1) {
 // pair to cost the 4-warp schedulers about as much as the block's own arithmetic - and every block is one basic
 // block of BW / 2 independent pixel pairs for the scheduler to interleave.  All pairs are masked by the lane's own
 // pixel count.
-// BW (template parameter): pixels per block, 4 or 8.
+// BW (template parameter): pixels per block - 8, 16 or 32 in the shipped shapes (rows_launch.h).
 
 // DEG > 0: the pairs of a block in LOCKSTEP - all u' pairs, then one Horner step for every pair, ..., then the ex2, the
 // masks and the denominator terms (two accumulators).  ptxas keeps source order: written pair after pair it issued the

@@ -1,5 +1,6 @@
-"""The N > 1 plumbing of bench.py (replicas only: barrier + max over ranks, rank-0 reporting), run as two gloo
-processes on CPU.  No GPU and no product kernels are involved: the data path has no collective."""
+"""The N > 1 plumbing of bench.py (barrier + max over ranks, rank-0 reporting, per-rank seeds), run as two gloo processes
+on CPU.  No GPU and no product kernels are involved.  The data path itself shards the events over the ranks and sums the
+ranks' accumulators once per iteration (paper_1502_07478_b200/sharding.py; its host logic is tests/test_sharding_gloo.py)."""
 import os
 import socket
 import sys
