@@ -198,6 +198,44 @@ int leave(Workspace& w, cudaStream_t st) {
     return JPET_OK;
 }
 
+// Every way out of a call that has passed enter() - success or error - records the ordering event (the next call, on
+// whatever stream, is ordered behind everything this call managed to queue), and a host-buffer call also waits for its
+// two internal streams: no asynchronous copy may still be reading the caller's host buffers, and no ring slot may still
+// be in flight, once the call has returned - also when it returns an error.  finish() is the success path and reports
+// its own failures; the destructor covers the early returns and keeps the error text of the failure that caused them.
+struct CallScope {
+    Workspace& w;
+    cudaStream_t st;
+    bool host;
+    bool done = false;
+    CallScope(Workspace& w_, cudaStream_t st_, bool host_ = false) : w(w_), st(st_), host(host_) {}
+    CallScope(const CallScope&) = delete;
+    CallScope& operator=(const CallScope&) = delete;
+    int finish() {
+        done = true;
+        int rc = leave(w, st);
+        if (host) {
+            cudaError_t e1 = cudaStreamSynchronize(st), e2 = cudaStreamSynchronize(w.copy_stream);
+            if (!rc && (e1 != cudaSuccess || e2 != cudaSuccess)) {
+                (void)cudaGetLastError();
+                rc = fail(JPET_E_CUDA, "cudaStreamSynchronize failed: %s", cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
+            }
+        }
+        return rc;
+    }
+    ~CallScope() {
+        if (done) return;
+        const std::string text = g_err;
+        (void)leave(w, st);
+        if (host) {
+            (void)cudaStreamSynchronize(st);
+            if (w.copy_stream) (void)cudaStreamSynchronize(w.copy_stream);
+        }
+        (void)cudaGetLastError();
+        g_err = text;
+    }
+};
+
 double sigma_z_max(const jpet_sigmas& sg) { return (double)sg.sigma_z * (1.0 + (double)g_opt.sz_eta); }
 
 int validate(const jpet_geometry* g, const jpet_sigmas* sg, const jpet_grid* gr) {
@@ -769,7 +807,9 @@ int reconstruct_host_impl(const float* events_host, int64_t n, const jpet_geomet
     if ((rc = ensure_host_path(w, stage_bytes))) return rc;
     cudaStream_t ks = w.compute_stream;
     if ((rc = enter(w, ks))) return rc;
+    CallScope scope(w, ks, true);
     w.slot_used[0] = w.slot_used[1] = false;       // nothing of an earlier call is in flight: every host call ends synchronised
+                                                   // on both internal streams, error returns included (CallScope)
     float* cur = w.rho_a;
     float* nxt = w.rho_b;
     if (rho_init_host) {
@@ -800,10 +840,7 @@ int reconstruct_host_impl(const float* events_host, int64_t n, const jpet_geomet
         }
     }
     CUDA_TRY(cudaMemcpyAsync(rho_out_host, cur, sizeof(float) * M, cudaMemcpyDeviceToHost, ks));
-    if ((rc = leave(w, ks))) return rc;
-    CUDA_TRY(cudaStreamSynchronize(ks));
-    CUDA_TRY(cudaStreamSynchronize(w.copy_stream));
-    return JPET_OK;
+    return scope.finish();
 }
 
 void release_ws(Workspace& w) {
@@ -823,46 +860,6 @@ void release_ws(Workspace& w) {
     if (w.compute_stream) cudaStreamDestroy(w.compute_stream);
 }
 
-}  // namespace
-
-// ---------------------------------------------------------------------------------------------------------
-extern "C" {
-
-int jpet_sensitivity(const jpet_geometry* geometry, const jpet_grid* grid, float* s_dev, void* cuda_stream) {
-    g_err.clear();
-    int rc = validate(geometry, nullptr, grid);
-    if (rc) return rc;
-    if (!s_dev) return fail(JPET_E_INVAL, "NULL s_dev");
-    const int M = grid->n_y * grid->n_z;
-    jpet::sensitivity_kernel<<<grid_for(M), 256, 0, (cudaStream_t)cuda_stream>>>(s_dev, grid->n_y, grid->n_z, grid->pixel,
-                                                                               geometry->R, geometry->L);
-    g_launches++;
-    CUDA_TRY(cudaGetLastError());
-    return JPET_OK;
-}
-
-int jpet_mlem_begin(const jpet_geometry* geometry, const jpet_sigmas* sigmas, const jpet_grid* grid,
-                    const float* rho_in_dev, void* cuda_stream) {
-    g_err.clear();
-    int rc = validate(geometry, sigmas, grid);
-    if (rc) return rc;
-    Workspace* w = nullptr;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    if ((rc = current_ws(&w)) || (rc = enter(*w, st))) return rc;
-    if ((rc = do_begin(*w, geometry, sigmas, grid, rho_in_dev, st))) return rc;
-    return leave(*w, st);
-}
-
-int jpet_mlem_accumulate(const float* events_dev, int64_t n_batch, void* cuda_stream) {
-    g_err.clear();
-    Workspace* w = device_ws();
-    if (!w || !w->open) return fail(JPET_E_INVAL, "jpet_mlem_accumulate without jpet_mlem_begin");
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    int rc = enter(*w, st);
-    if (rc) return rc;
-    if ((rc = do_accumulate(*w, events_dev, n_batch, st))) return rc;
-    return leave(*w, st);
-}
 // ---- jpet_mlem_iterate_noalloc: one iteration whose scratch is a fixed array inside the library image ------------------
 // Some users of this library must not, or cannot, allocate device memory at the moment they need an iteration: an
 // acquisition or monitoring loop with a latency budget (cudaMalloc / cudaFree stall every stream of the device while they
@@ -907,6 +904,48 @@ __global__ void noalloc_meta_kernel(int* __restrict__ meta, int n) {
     if (i < jpet::kMetaWords) meta[i] = i == jpet::kMetaDirectCount ? n : 0;
 }
 
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------------
+extern "C" {
+
+int jpet_sensitivity(const jpet_geometry* geometry, const jpet_grid* grid, float* s_dev, void* cuda_stream) {
+    g_err.clear();
+    int rc = validate(geometry, nullptr, grid);
+    if (rc) return rc;
+    if (!s_dev) return fail(JPET_E_INVAL, "NULL s_dev");
+    const int M = grid->n_y * grid->n_z;
+    jpet::sensitivity_kernel<<<grid_for(M), 256, 0, (cudaStream_t)cuda_stream>>>(s_dev, grid->n_y, grid->n_z, grid->pixel,
+                                                                               geometry->R, geometry->L);
+    g_launches++;
+    CUDA_TRY(cudaGetLastError());
+    return JPET_OK;
+}
+
+int jpet_mlem_begin(const jpet_geometry* geometry, const jpet_sigmas* sigmas, const jpet_grid* grid,
+                    const float* rho_in_dev, void* cuda_stream) {
+    g_err.clear();
+    int rc = validate(geometry, sigmas, grid);
+    if (rc) return rc;
+    Workspace* w = nullptr;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = current_ws(&w)) || (rc = enter(*w, st))) return rc;
+    CallScope scope(*w, st);
+    if ((rc = do_begin(*w, geometry, sigmas, grid, rho_in_dev, st))) return rc;
+    return scope.finish();
+}
+
+int jpet_mlem_accumulate(const float* events_dev, int64_t n_batch, void* cuda_stream) {
+    g_err.clear();
+    Workspace* w = device_ws();
+    if (!w || !w->open) return fail(JPET_E_INVAL, "jpet_mlem_accumulate without jpet_mlem_begin");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = enter(*w, st);
+    if (rc) return rc;
+    CallScope scope(*w, st);
+    if ((rc = do_accumulate(*w, events_dev, n_batch, st))) return rc;
+    return scope.finish();
+}
 
 int jpet_mlem_end(const float* rho_in_dev, float* rho_out_dev, void* cuda_stream) {
     g_err.clear();
@@ -915,8 +954,9 @@ int jpet_mlem_end(const float* rho_in_dev, float* rho_out_dev, void* cuda_stream
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = enter(*w, st);
     if (rc) return rc;
+    CallScope scope(*w, st);
     if ((rc = do_end(*w, rho_in_dev, rho_out_dev, nullptr, 0, st))) return rc;
-    return leave(*w, st);
+    return scope.finish();
 }
 
 int jpet_mlem_end_peers(const float* rho_in_dev, float* rho_out_dev, const float* const* peer_acc_dev, int32_t n_peers,
@@ -928,8 +968,9 @@ int jpet_mlem_end_peers(const float* rho_in_dev, float* rho_out_dev, const float
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = enter(*w, st);
     if (rc) return rc;
+    CallScope scope(*w, st);
     if ((rc = do_end(*w, rho_in_dev, rho_out_dev, peer_acc_dev, n_peers, st))) return rc;
-    return leave(*w, st);
+    return scope.finish();
 }
 
 int jpet_mlem_accumulator(float** acc_dev, int64_t* n_floats) {
@@ -979,10 +1020,11 @@ int jpet_mlem_iterate(const float* events_dev, int64_t n, const jpet_geometry* g
     cudaStream_t st = (cudaStream_t)cuda_stream;
     Workspace* w = nullptr;
     if ((rc = current_ws(&w)) || (rc = enter(*w, st))) return rc;
+    CallScope scope(*w, st);
     if ((rc = do_begin(*w, geometry, sigmas, grid, rho_in_dev, st))) return rc;
     if ((rc = do_accumulate(*w, events_dev, n, st))) return rc;
     if ((rc = do_end(*w, rho_in_dev, rho_out_dev, nullptr, 0, st))) return rc;
-    return leave(*w, st);
+    return scope.finish();
 }
 
 int jpet_reconstruct(const float* events_dev, int64_t n, const jpet_geometry* geometry, const jpet_sigmas* sigmas,
@@ -997,6 +1039,7 @@ int jpet_reconstruct(const float* events_dev, int64_t n, const jpet_geometry* ge
     cudaStream_t st = (cudaStream_t)cuda_stream;
     Workspace* w = nullptr;
     if ((rc = current_ws(&w)) || (rc = enter(*w, st))) return rc;
+    CallScope scope(*w, st);
     const int M = grid->n_y * grid->n_z;
     if ((rc = ensure_images(*w, M))) return rc;
     // ping-pong through the workspace so that rho_out may alias rho_init and is written once per iteration
@@ -1009,10 +1052,10 @@ int jpet_reconstruct(const float* events_dev, int64_t n, const jpet_geometry* ge
     }
     if (n_iter == 0) {
         if (cur != rho_out_dev) CUDA_TRY(cudaMemcpyAsync(rho_out_dev, cur, sizeof(float) * M, cudaMemcpyDeviceToDevice, st));
-        return leave(*w, st);
+        return scope.finish();
     }
     if ((rc = iterate_many(*w, events_dev, n, geometry, sigmas, grid, cur, rho_out_dev, n_iter, st))) return rc;
-    return leave(*w, st);
+    return scope.finish();
 }
 
 int jpet_mlem_iterate_host(const float* events_host, int64_t n, const jpet_geometry* geometry, const jpet_sigmas* sigmas,
@@ -1088,6 +1131,7 @@ int jpet_direct_histogram(const float* events_dev, int64_t n, const jpet_geometr
     if ((rc = current_ws(&w))) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if ((rc = enter(*w, st))) return rc;
+    CallScope scope(*w, st);
     if (!w->counters) CUDA_TRY(cudaMalloc(&w->counters, 4 * sizeof(unsigned long long)));
     CUDA_TRY(cudaMemsetAsync(w->counters + 3, 0, sizeof(unsigned long long), st));
     jpet::HistParams h;
@@ -1107,7 +1151,7 @@ int jpet_direct_histogram(const float* events_dev, int64_t n, const jpet_geometr
         g_launches++;
         CUDA_TRY(cudaGetLastError());
     }
-    if ((rc = leave(*w, st))) return rc;
+    if ((rc = scope.finish())) return rc;
     if (n_outside_host) {
         unsigned long long out = 0;
         CUDA_TRY(cudaMemcpyAsync(&out, w->counters + 3, sizeof out, cudaMemcpyDeviceToHost, st));
@@ -1307,9 +1351,6 @@ int64_t jpet_plan_describe(const jpet_geometry* geometry, const jpet_sigmas* sig
 
 const char* jpet_shape_name(int32_t shape) { return shape >= 0 && shape < kNumShapes ? kShapes[shape].name : ""; }
 
-int jpet_abi_version(void) { return JPET_ABI_VERSION; }
-
-}  // extern "C"
 int jpet_mlem_iterate_noalloc(const float* events_dev, int64_t n, const jpet_geometry* geometry, const jpet_sigmas* sigmas,
                               const jpet_grid* grid, const float* rho_in_dev, float* rho_out_dev, void* cuda_stream) {
     g_err.clear();
@@ -1350,3 +1391,6 @@ int jpet_mlem_iterate_noalloc(const float* events_dev, int64_t n, const jpet_geo
     return JPET_OK;
 }
 
+int jpet_abi_version(void) { return JPET_ABI_VERSION; }
+
+}  // extern "C"

@@ -365,6 +365,32 @@ def test_degree_classes_do_not_change_the_image(jp, oracle, name, n, low):
     jp.jpet_set_option("degree_classes_off", 1)
     try:
         one, (ne1, ns1) = gpu_iterate(jp, ev, cfg, rho)
+def test_an_error_return_leaves_the_stream_ordering_intact(jp):
+    """every way out of a call that has entered the workspace records the ordering event, error returns
+    included, and keeps the text of the error that caused it.  An accumulate that fails its argument check on a second
+    stream, in the middle of an iteration that runs on two streams, must not disturb the iteration."""
+    import ctypes
+
+    import torch
+
+    cfg = synth.CONFIGS["cfg2"]
+    ev = torch.from_numpy(synth.config_events(cfg, n=200_000)).cuda()
+    rho = torch.ones(cfg.n_y * cfg.n_z, device="cuda")
+    want, got = torch.empty_like(rho), torch.empty_like(rho)
+    jp.jpet_mlem_iterate(ev, *geom(cfg), rho, want)
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    lib = jp.binding.load()
+    jp.jpet_mlem_begin(*geom(cfg), rho, stream=s1)
+    jp.jpet_mlem_accumulate(ev[:100_000], stream=s1)
+    assert lib.jpet_mlem_accumulate(None, 5, ctypes.c_void_p(s2.cuda_stream)) == jp.binding.JPET_E_INVAL
+    assert "NULL events" in jp.jpet_last_error()
+    jp.jpet_mlem_accumulate(ev[100_000:], stream=s2)
+    jp.jpet_mlem_end(rho, got, stream=s1)
+    torch.cuda.synchronize()
+    assert float((got - want).abs().max() / want.max()) <= 1e-5
+
+
         assert jp.jpet_get_option("last_variant_low") == -1
     finally:
         jp.jpet_set_option("degree_classes_off", 0)
