@@ -3,8 +3,9 @@
 // event, one 32-bit atomic increment.
 //
 // The pixel index is an integer decided by floating point, so the arithmetic is pinned: IEEE fp32, round to nearest,
-// in exactly this order (no approximate MUFU, no contraction beyond the fused multiply-adds written here) - the
-// oracle takes the same decisions in the same precision and the counts agree bit for bit:
+// in exactly this order (no approximate MUFU, no contraction beyond the fused multiply-adds written here), whatever the
+// compiler flags.  The oracle is Eq. 2 in fp64 + floor: counts agree exactly for every event farther than the fp32
+// rounding error (about 2^-21 (|c| + 1) pixels) from a pixel border, the others land in an adjacent pixel (R24):
 //     t   = (z_u - z_d) * inv2R                      inv2R = fp32(1 / (2 R))
 //     sec = sqrt(fma(t, t, 1))
 //     y~  = (-0.5 * dl) / sec                        z~ = fma(y~, t, 0.5 * (z_u + z_d))
@@ -41,14 +42,18 @@ direct_histogram_kernel(const float* __restrict__ events, int n, const __grid_co
     if (use_smem)
         for (int b = tid; b < M; b += kBinBlock) hs[b] = 0u;
     int outside = 0;
-    for (int base = blockIdx.x * kBinTile; base < n; base += gridDim.x * kBinTile) {
+    // 64-bit walk: with one tile per block the stride gridDim.x * kBinTile is about n, and base + stride passes 2^31 for
+    // n > 2^30 events (n itself is at most 2^31 - 1)
+    const long long stride = (long long)gridDim.x * kBinTile;
+    for (long long base64 = (long long)blockIdx.x * kBinTile; base64 < n; base64 += stride) {
+        const int base = (int)base64;
         __syncthreads();                                   // previous tile consumed (and the histogram zeroed)
         load_event_tile(events, n, base, tile);
         __syncthreads();
 #pragma unroll
         for (int q = 0; q < kBinPer; ++q) {
             const int k = q * kBinBlock + tid;
-            if (base + k < n) {
+            if (k < n - base) {
                 const int px = direct_pixel(tile[3 * k], tile[3 * k + 1], tile[3 * k + 2], h);
                 if (px < 0) ++outside;
                 else atomicAdd(use_smem ? hs + px : hist + px, 1u);

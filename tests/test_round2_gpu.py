@@ -1,5 +1,5 @@
 """GPU parity of the rows SURVEY.md section 8(f) added in round 2, through the C-ABI binding against the CPU oracle on the same
-seeded inputs: per-event sigma_z (f1), the direct-reconstruction histogram (f2, bit-exact), event sharding with the
+seeded inputs: per-event sigma_z (f1), the direct-reconstruction histogram (f2: equal to Eq. 2 in fp64 away from pixel borders), event sharding with the
 accumulator sum fused into the finalise kernel (f3), the device event generator and the exact-kernel mode (f4); plus the
 host ring path and the stream ordering of the workspace.  Run on the B200 box with  pytest -m gpu."""
 import math
@@ -96,11 +96,54 @@ def test_position_dependent_sigma_z(jp, oracle, name, n, eta, frac):
 
 
 # ---- (f2) direct reconstruction histogram (Eq. 2, Fig. 4b) -------------------------------------------------------------
+def histogram_agrees_with_fp64(oracle, ev, cfg, got, got_outside, before=None):
+    """The rule for an integer decided by floating point (R24).  The oracle is Eq. 2 in fp64 and a floor; the
+    kernel computes in fp32, so a point closer to a pixel border than the fp32 rounding error may be counted on the other
+    side.  With c = (c_y, c_z) the oracle's fp64 pixel coordinates, an event is BORDERLINE when a border b in {0 .. n}
+    lies within eps = 2^-18 (|c| + 1) pixels of c on either axis (fp32 evaluates c to about 2^-21 (|c| + 1): eight times
+    closer).  Then: (i) the counts of all other events equal the oracle's exactly - the kernel's histogram minus the
+    oracle's histogram of the decided events is >= 0 everywhere and sums to the number of borderline events; (ii) every
+    borderline event is in one of the pixels next to its border(s) - per pixel (and for "outside") the remainder does not
+    exceed the number of borderline events that have it among their candidates.  Returns (borderline fraction, fraction
+    counted in another pixel than the oracle's)."""
+    n_y, n_z = cfg.n_y, cfg.n_z
+    c = oracle.direct_pixel_coords(ev, cfg.R, n_y, n_z, cfg.pixel)
+    finite = ~np.isnan(c).any(axis=1)
+    cf = np.where(finite[:, None], c, -1e6)                                     # non-finite events: decidedly outside
+    b = np.stack([np.clip(np.rint(cf[:, 0]), 0, n_y), np.clip(np.rint(cf[:, 1]), 0, n_z)], axis=1)
+    near_ax = np.abs(cf - b) <= 2.0 ** -18 * (np.abs(cf) + 1.0)
+    near = near_ax.any(axis=1)
+    want_d, out_d = oracle.direct_histogram(ev[~near], cfg.R, n_y, n_z, cfg.pixel, hist=None if before is None else before.copy())
+    resid = got.astype(np.int64) - want_d.astype(np.int64)
+    resid_out = got_outside - out_d
+    assert (resid >= 0).all() and resid_out >= 0
+    assert int(resid.sum()) + resid_out == int(near.sum())
+    cap = np.zeros((n_y, n_z), dtype=np.int64)
+    cap_out = 0
+    fl = np.floor(cf).astype(np.int64)
+    for j in np.nonzero(near)[0]:
+        cand = [([int(b[j, a]) - 1, int(b[j, a])] if near_ax[j, a] else [int(fl[j, a])]) for a in (0, 1)]
+        pixels = {(iy, iz) if (0 <= iy < n_y and 0 <= iz < n_z) else None for iy in cand[0] for iz in cand[1]}
+        for q in pixels:
+            if q is None:
+                cap_out += 1
+            else:
+                cap[q] += 1
+    assert (resid <= cap).all() and resid_out <= cap_out
+    want_all, out_all = oracle.direct_histogram(ev, cfg.R, n_y, n_z, cfg.pixel, hist=None if before is None else before.copy())
+    moved = (int(np.abs(got.astype(np.int64) - want_all.astype(np.int64)).sum()) + abs(got_outside - out_all)) / 2
+    n = max(len(ev), 1)
+    return float(near.sum()) / n, moved / n
+
+
 @pytest.mark.parametrize("name,n", [("fig4", 1_000_003), ("cfg2", 300_000), ("cfg5", 1_000_000), ("cfg1", 0)])
-def test_direct_histogram_is_bit_exact(jp, oracle, name, n):
-    """Integer work: every count equals the oracle's (both take the pixel decision in IEEE fp32 in the same order).  fig4's
-    image fits the per-block shared-memory histogram, the others take global atomics; a slice at an odd offset takes the
-    scalar loads; a second call increments."""
+def test_direct_histogram_against_the_fp64_oracle(jp, oracle, name, n):
+    """Integer work decided by floating point: every count equals the count of Eq. 2 in fp64 + floor, except for events within
+    eps of a pixel border, which must sit in an adjacent pixel (histogram_agrees_with_fp64).  The borderline fraction is what
+    eps predicts for points spread evenly over the pixels (about 4 eps: two axes, both sides of a border; at most
+    4 x 2^-18 x (n_max + 1) x 1.5), and the events that really are counted across a border are at most a quarter of them.
+    fig4's image fits the per-block shared-memory histogram, the others take global atomics; a slice at an odd offset takes
+    the scalar loads; a second call increments."""
     import torch
 
     cfg = synth.CONFIGS[name]
@@ -111,14 +154,38 @@ def test_direct_histogram_is_bit_exact(jp, oracle, name, n):
     hist = torch.zeros(cfg.n_y * cfg.n_z, dtype=torch.int32, device="cuda")
     ev_d = torch.from_numpy(ev).cuda()
     outside = jp.jpet_direct_histogram(ev_d, cfg.R, cfg.L, cfg.n_y, cfg.n_z, cfg.pixel, hist)
-    want, want_out = oracle.direct_histogram(ev, cfg.R, cfg.n_y, cfg.n_z, cfg.pixel)
-    got = hist.cpu().numpy().view(np.uint32).reshape(cfg.n_y, cfg.n_z)
-    assert outside == want_out and (got == want).all()
+    got = hist.cpu().numpy().view(np.uint32).reshape(cfg.n_y, cfg.n_z).copy()
     assert int(got.sum()) + outside == n
+    near, moved = histogram_agrees_with_fp64(oracle, ev, cfg, got, outside)
+    print(f"{name}: borderline fraction {near:.2e}, counted across a border {moved:.2e}")
+    assert near <= 6.0 * 2.0 ** -18 * (max(cfg.n_y, cfg.n_z) + 1) and moved <= 0.25 * near + 2.0 / max(n, 1)
     if n:
         assert jp.jpet_direct_histogram(ev_d[1:70001], cfg.R, cfg.L, cfg.n_y, cfg.n_z, cfg.pixel, hist, count_outside=False) is None
-        want2, _ = oracle.direct_histogram(ev[1:70001], cfg.R, cfg.n_y, cfg.n_z, cfg.pixel, hist=want.copy())
-        assert (hist.cpu().numpy().view(np.uint32).reshape(cfg.n_y, cfg.n_z) == want2).all()
+        got2 = hist.cpu().numpy().view(np.uint32).reshape(cfg.n_y, cfg.n_z)
+        assert int(got2.sum()) - int(got.sum()) <= 70000
+        out2 = 70000 - (int(got2.sum()) - int(got.sum()))
+        histogram_agrees_with_fp64(oracle, ev[1:70001], cfg, got2, out2, before=got)
+
+
+def test_direct_histogram_beyond_2_30_events(jp):
+    """The global-atomic path walks one tile per block, so its stride is about n: past 2^30 events a 32-bit tile offset
+    wraps.  One call over 2^30 + 2^20 + 5 device-generated events (12.9 GB) must count every event once
+    and give, count by count, the sum of two calls over the halves (each below 2^30)."""
+    import torch
+
+    cfg = synth.CONFIGS["cfg2"]
+    n = (1 << 30) + (1 << 20) + 5
+    ev_d = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+    jp.jpet_generate_events(cfg.phantom, n, cfg.R, cfg.L, cfg.sigma_z, cfg.sigma_dl, 11, ev_d)
+    whole = torch.zeros(cfg.n_y * cfg.n_z, dtype=torch.int32, device="cuda")
+    halves = torch.zeros_like(whole)
+    out_whole = jp.jpet_direct_histogram(ev_d, cfg.R, cfg.L, cfg.n_y, cfg.n_z, cfg.pixel, whole)
+    out_halves = sum(jp.jpet_direct_histogram(part, cfg.R, cfg.L, cfg.n_y, cfg.n_z, cfg.pixel, halves)
+                     for part in (ev_d[: n // 2], ev_d[n // 2:]))
+    assert int(whole.sum(dtype=torch.int64)) + out_whole == n
+    assert out_whole == out_halves and bool((whole == halves).all())
+    del ev_d
+    torch.cuda.empty_cache()
 
 
 # ---- (f3) event sharding: private accumulators summed in the finalise kernel (PAPER.md:157) ----------------------------
@@ -298,6 +365,32 @@ def test_calls_on_different_streams_are_ordered(jp, oracle):
     assert ne > 0 and float((b2 - b).abs().max() / b.max()) <= 1e-5
 
 
+def test_an_error_return_leaves_the_stream_ordering_intact(jp):
+    """ADVICE round 2: every way out of a call that has entered the workspace records the ordering event, error returns
+    included, and keeps the text of the error that caused it.  An accumulate that fails its argument check on a second
+    stream, in the middle of an iteration that runs on two streams, must not disturb the iteration."""
+    import ctypes
+
+    import torch
+
+    cfg = synth.CONFIGS["cfg2"]
+    ev = torch.from_numpy(synth.config_events(cfg, n=200_000)).cuda()
+    rho = torch.ones(cfg.n_y * cfg.n_z, device="cuda")
+    want, got = torch.empty_like(rho), torch.empty_like(rho)
+    jp.jpet_mlem_iterate(ev, *geom(cfg), rho, want)
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    lib = jp.binding.load()
+    jp.jpet_mlem_begin(*geom(cfg), rho, stream=s1)
+    jp.jpet_mlem_accumulate(ev[:100_000], stream=s1)
+    assert lib.jpet_mlem_accumulate(None, 5, ctypes.c_void_p(s2.cuda_stream)) == jp.binding.JPET_E_INVAL
+    assert "NULL events" in jp.jpet_last_error()
+    jp.jpet_mlem_accumulate(ev[100_000:], stream=s2)
+    jp.jpet_mlem_end(rho, got, stream=s1)
+    torch.cuda.synchronize()
+    assert float((got - want).abs().max() / want.max()) <= 1e-5
+
+
 # ---- (f3) the sharded iteration across two PROCESSES (one GPU: the ranks' kernels never wait on one another) ------------
 def _p2p_worker(rank, world, port, n_events, n_iter, q):
     os.environ.update(RANK=str(rank), LOCAL_RANK="0", WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
@@ -365,32 +458,6 @@ def test_degree_classes_do_not_change_the_image(jp, oracle, name, n, low):
     jp.jpet_set_option("degree_classes_off", 1)
     try:
         one, (ne1, ns1) = gpu_iterate(jp, ev, cfg, rho)
-def test_an_error_return_leaves_the_stream_ordering_intact(jp):
-    """ADVICE round 2: every way out of a call that has entered the workspace records the ordering event, error returns
-    included, and keeps the text of the error that caused it.  An accumulate that fails its argument check on a second
-    stream, in the middle of an iteration that runs on two streams, must not disturb the iteration."""
-    import ctypes
-
-    import torch
-
-    cfg = synth.CONFIGS["cfg2"]
-    ev = torch.from_numpy(synth.config_events(cfg, n=200_000)).cuda()
-    rho = torch.ones(cfg.n_y * cfg.n_z, device="cuda")
-    want, got = torch.empty_like(rho), torch.empty_like(rho)
-    jp.jpet_mlem_iterate(ev, *geom(cfg), rho, want)
-    torch.cuda.synchronize()
-    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
-    lib = jp.binding.load()
-    jp.jpet_mlem_begin(*geom(cfg), rho, stream=s1)
-    jp.jpet_mlem_accumulate(ev[:100_000], stream=s1)
-    assert lib.jpet_mlem_accumulate(None, 5, ctypes.c_void_p(s2.cuda_stream)) == jp.binding.JPET_E_INVAL
-    assert "NULL events" in jp.jpet_last_error()
-    jp.jpet_mlem_accumulate(ev[100_000:], stream=s2)
-    jp.jpet_mlem_end(rho, got, stream=s1)
-    torch.cuda.synchronize()
-    assert float((got - want).abs().max() / want.max()) <= 1e-5
-
-
         assert jp.jpet_get_option("last_variant_low") == -1
     finally:
         jp.jpet_set_option("degree_classes_off", 0)
