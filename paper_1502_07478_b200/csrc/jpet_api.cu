@@ -1140,14 +1140,18 @@ int jpet_direct_histogram(const float* events_dev, int64_t n, const jpet_geometr
     h.inv_px = (float)(1.0 / (double)grid->pixel);
     h.oy = (float)(0.5 * (grid->n_y - 1) + 0.5);
     h.oz = (float)(0.5 * (grid->n_z - 1) + 0.5);
-    if (n > 0) {
-        const int M = grid->n_y * grid->n_z;
-        const int use_smem = M <= jpet::kHistSmemMax;
-        const size_t smem = kTileBytes + (use_smem ? sizeof(unsigned int) * (size_t)M : 0);
-        const int tiles = (int)((n + jpet::kBinTile - 1) / jpet::kBinTile);
+    // at most 2^30 events per launch: the kernel walks its tiles with 32-bit offsets, and with one tile per block the stride
+    // is about the launch size (base + stride < 2^31); 2^30 events keep every launch's first event 16-byte aligned
+    constexpr int64_t kHistMaxLaunch = 1ll << 30;
+    const int M = grid->n_y * grid->n_z;
+    const int use_smem = M <= jpet::kHistSmemMax;
+    const size_t smem = kTileBytes + (use_smem ? sizeof(unsigned int) * (size_t)M : 0);
+    for (int64_t off = 0; off < n; off += kHistMaxLaunch) {
+        const int64_t nl = std::min<int64_t>(kHistMaxLaunch, n - off);
+        const int tiles = (int)((nl + jpet::kBinTile - 1) / jpet::kBinTile);
         // shared-memory histograms: a persistent grid (one flush per block); global atomics: one tile per block
         const int blocks = use_smem ? std::min(tiles, w->sm_count * 4) : tiles;
-        jpet::direct_histogram_kernel<<<blocks, jpet::kBinBlock, smem, st>>>(events_dev, (int)n, h, hist_dev, w->counters + 3, use_smem);
+        jpet::direct_histogram_kernel<<<blocks, jpet::kBinBlock, smem, st>>>(events_dev + 3 * off, (int)nl, h, hist_dev, w->counters + 3, use_smem);
         g_launches++;
         CUDA_TRY(cudaGetLastError());
     }
